@@ -1,0 +1,7 @@
+"""B200-native batched semi-global affine-gap alignment (SOAP3-dp gapped-alignment stage).
+
+The product is the C-ABI library ``libsdp.so`` (``include/sdp.h``) built from ``csrc/``; this
+package is its thin Python binding plus the seeded input generators. There is no CPU fallback:
+every entry point raises if the CUDA library is missing.
+"""
+__all__ = ["workloads"]
