@@ -1,0 +1,164 @@
+/*
+ * sdp.h -- C ABI of libsdp: batched semi-global affine-gap (Gotoh) alignment on one B200.
+ *
+ * The operation is the gapped-alignment stage of SOAP3-dp (arXiv 1302.5507, Methods section 3):
+ * "Given a candidate region T (of length m) and a read R (of length n), the aim is to find a
+ * sub-region T' inside T such that the alignment score between R and T' is maximum"
+ * (PAPER.md:267), with the recurrences of PAPER.md:289-293, the base cases of PAPER.md:303-310
+ * and the result max_{1<=i<=m} M(i,n) of PAPER.md:269, followed by backtracking.
+ * Tie rules, the similarity filter and every other point the paper leaves open are fixed in
+ * DESIGN.md ("Readings"). All arithmetic runs in hand-written sm_100a kernels; there is no CPU
+ * fallback.
+ *
+ * Sequence layout (both reads and windows)
+ *   2 bits per base, A=0 C=1 G=2 T=3; base k of a buffer sits in bits 2*(k mod 16) (LSB first)
+ *   of little-endian uint32 word k/16. Offsets are in BASES, so windows may be overlapping views
+ *   into one packed reference and a read may appear in many pairs. *_nmask (nullable) holds one
+ *   bit per base on the same base offsets (bit k mod 32 of word k/32); a set bit makes the
+ *   position N, which scores as a mismatch against everything including N. Buffers must be
+ *   readable up to the next multiple of 16 bytes past the last word used.
+ *
+ * Coordinates are 0-based, inclusive, relative to the window. The whole read is aligned
+ * (read_start = 0, read_end = n-1). ref_end - ref_start + 1 is the number of window bases the
+ * CIGAR consumes and may be 0 (an all-insertion alignment reports ref_start = ref_end + 1).
+ * CIGAR runs use the BAM encoding (len << 4) | op with M=0, I=1, D=2; runs of one pair are
+ * contiguous, in alignment order, at cigar_ops[cigar_off[p] .. cigar_off[p] + cigar_len[p]).
+ */
+#ifndef SDP_H_
+#define SDP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SDP_OK       0
+#define SDP_EINVAL  (-1)  /* null pointer, bad scoring, empty sequence, index / offset out of range  */
+#define SDP_ERANGE  (-2)  /* a pair's lengths break the int16 range rule below                        */
+#define SDP_ECUDA   (-3)  /* a CUDA call failed; sdp_last_error() has the CUDA message                */
+#define SDP_ENOMEM  (-4)  /* host or device allocation failed                                         */
+
+/* Longest read the register-resident kernels take (32 lanes x 32 columns). */
+#define SDP_MAX_READ_LEN 1024
+/*
+ * int16 range rule (per pair, n = read length, m = window length):
+ *     match*n + gap_extend*(n + m) + 3*gap_open + 64 <= SDP_MAX_CELL_VALUE
+ * The kernels store H + gap_extend*(i+j) + bias in 16-bit lanes;
+ * pairs that break the rule are rejected with SDP_ERANGE, never clamped.
+ */
+#define SDP_MAX_CELL_VALUE 16000
+
+typedef struct sdp_ctx sdp_ctx;   /* opaque; owns device scratch, result buffers, pinned staging */
+
+/* Scoring of PAPER.md:283: S_MA = match, S_MI = mismatch, S_GO = -(gap_open + gap_extend),
+ * S_GE = -gap_extend, i.e. a gap of k bases costs gap_open + k*gap_extend. */
+typedef struct sdp_scoring {
+    int32_t match;           /* >= 0, and match - mismatch > 0                                  */
+    int32_t mismatch;        /* <= 0                                                            */
+    int32_t gap_open;        /* >= 0                                                            */
+    int32_t gap_extend;      /* >= 1                                                            */
+    double  min_similarity;  /* in [0,1]; quantised once as q = llround(x * 1e6); a pair passes  */
+                             /* iff n_match * 1e6 >= q * n_cols (n_cols = CIGAR columns)         */
+} sdp_scoring;
+
+/* Inputs of one call. Every pointer is caller-owned and read-only: DEVICE memory for
+ * sdp_align_batch, HOST memory for sdp_align_batch_host. */
+typedef struct sdp_batch {
+    const uint32_t* reads_packed;  /* 2-bit packed read bases                                   */
+    const uint64_t* read_off;      /* [n_reads] first base of read r, in bases                  */
+    const uint32_t* read_len;      /* [n_reads] length in bases, 1..SDP_MAX_READ_LEN            */
+    const uint32_t* read_nmask;    /* nullable N bitmap over reads_packed's base offsets        */
+    uint32_t        n_reads;
+    uint64_t        reads_bases;   /* bases addressable in reads_packed (for bounds checks)     */
+    const uint32_t* wins_packed;   /* 2-bit packed windows or one packed reference              */
+    const uint64_t* win_off;       /* [n_wins]                                                  */
+    const uint32_t* win_len;       /* [n_wins] >= 1                                             */
+    const uint32_t* win_nmask;     /* nullable                                                  */
+    uint32_t        n_wins;
+    uint64_t        wins_bases;
+    const uint32_t* pairs;         /* [2*n_pairs] (read_idx, win_idx) per pair                  */
+    uint64_t        n_pairs;       /* 0 is allowed: every result array is then empty            */
+} sdp_batch;
+
+/* Outputs, in caller pair order. Pointers are owned by the ctx and stay valid until the next
+ * align call on it or sdp_destroy: DEVICE memory from sdp_align_batch, pinned HOST memory from
+ * sdp_align_batch_host. */
+typedef struct sdp_result {
+    const int32_t*  score;        /* max_{1<=i<=m} M(i,n)                          */
+    const int32_t*  ref_start;    /* first consumed window base (where the traceback stops)     */
+    const int32_t*  ref_end;      /* (lowest maximising row i) - 1                               */
+    const int32_t*  read_start;   /* always 0                                                    */
+    const int32_t*  read_end;     /* always n-1                                                  */
+    const uint8_t*  pass;         /* similarity filter, 1 = pass                                 */
+    const int32_t*  n_match;      /* M columns whose two bases are equal and not N               */
+    const int32_t*  n_cols;       /* alignment columns = M + I + D bases                         */
+    const uint64_t* cigar_off;    /* exclusive scan of cigar_len in caller pair order            */
+    const uint32_t* cigar_len;    /* runs of pair p                                              */
+    const uint32_t* cigar_ops;    /* [n_cigar_ops] compacted runs                                */
+    uint64_t        n_cigar_ops;
+    uint64_t        n_pairs;
+} sdp_result;
+
+/* Per-call counters; times are CUDA-event milliseconds on the caller's stream and are only
+ * filled when timing was switched on with sdp_set_timing(ctx, 1). */
+typedef struct sdp_stats {
+    uint64_t n_pairs;
+    uint64_t cells_forward;       /* sum n*m: the CUPS numerator                                 */
+    uint64_t cells_reverse;       /* cells of the reverse pass                                   */
+    uint64_t cells_traceback;     /* band cells of the traceback pass                            */
+    uint64_t n_reverse_pairs;     /* pairs whose score allows a gap (W > 0)                      */
+    uint32_t kernel_launches;     /* kernels of this library launched by the call                */
+    uint32_t forward_launches;    /* launches of the forward score kernel                        */
+    float ms_total;               /* whole call, first kernel to last                            */
+    float ms_bucket;              /* a1 + a2 validate, histogram, scan, scatter, task build      */
+    float ms_forward;             /* a3 forward score kernels                                    */
+    float ms_reverse;             /* a4                                                          */
+    float ms_traceback;           /* a5 + a6                                                     */
+    float ms_compact;             /* a7 + a8                                                     */
+} sdp_stats;
+
+/* Create a context on CUDA device `cuda_device`. SDP_EINVAL for bad scoring or null arguments,
+ * SDP_ECUDA / SDP_ENOMEM otherwise; *out is written only on success. Not thread-safe: use one
+ * ctx per thread; separate ctxs are independent. */
+int sdp_create(const sdp_scoring* scoring, int cuda_device, sdp_ctx** out);
+
+/* Align every pair of `batch` (DEVICE pointers). Work is enqueued on `cuda_stream`
+ * (a cudaStream_t; NULL = default stream) and the call returns after the stream has completed
+ * it (one internal synchronisation, needed to learn n_cigar_ops), so errors are synchronous.
+ * On error `out` is untouched. A CIGAR is produced for every pair, passing the filter or not. */
+int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp_result* out);
+
+/* Same operation with HOST pointers in `batch`: copies the inputs to the device through pinned
+ * staging, runs sdp_align_batch's pipeline on an internal stream, and copies every result array
+ * back; `out` then holds pinned HOST pointers owned by the ctx. */
+int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* batch, sdp_result* out);
+
+/* Counters of the last align call on this ctx. */
+int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);
+
+/* Switch per-stage CUDA-event timing on (1) or off (0, the default). */
+int sdp_set_timing(sdp_ctx* ctx, int enabled);
+
+/* Message of the last error on this ctx ("" if none). Never NULL; valid until the next call. */
+const char* sdp_last_error(const sdp_ctx* ctx);
+
+/* Release everything the ctx owns. NULL is ignored. */
+void sdp_destroy(sdp_ctx* ctx);
+
+/*
+ * Roofline helper: runs an issue-rate microbenchmark of the int16x2
+ * DPX instructions the score kernel is built from (VIADDMNMX.S16x2 / VIMNMX3.S16x2, 50:50,
+ * 8 independent chains per thread, full occupancy) on `cuda_device` and reports
+ * thread-instructions per clock per SM, the SM count and the SM clock in MHz observed
+ * during the run (cycles / elapsed time).
+ */
+int sdp_measure_dpx_rate(int cuda_device, double* instr_per_clk_per_sm, int32_t* sm_count, double* sm_mhz);
+
+/* Library version, e.g. "sdp 0.1 (sm_100a)". */
+const char* sdp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDP_H_ */

@@ -5,3 +5,17 @@ package is its thin Python binding plus the seeded input generators. There is no
 every entry point raises if the CUDA library is missing.
 """
 __all__ = ["workloads"]
+
+from . import workloads  # noqa: E402,F401
+from .binding import (  # noqa: E402,F401
+    Context,
+    DeviceBatch,
+    HostResult,
+    SdpError,
+    load_library,
+    sdp_measure_dpx_rate,
+    sdp_version,
+)
+
+__all__ += ["Context", "DeviceBatch", "HostResult", "SdpError", "load_library", "sdp_measure_dpx_rate",
+            "sdp_version"]

@@ -1,0 +1,244 @@
+// bucket.cu -- a1 (ingest + validate) and a2 (device-side length bucketing) of the hot path, plus
+// the generic pieces the later stages reuse: key histogram, bin scan, scatter into bucket order,
+// per-read-length task table, and a large exclusive scan.
+//
+// The paper's analogue is grouping reads by 32 so warp loads coalesce and running
+// work of different complexity classes separately; here pairs are binned by
+// (read length, rows >> 6) so that the lanes of one warp walk the same number of DP rows.
+#include "sdp_host.cuh"
+
+namespace sdp {
+
+// ---------------------------------------------------------------------------------------------
+// a1: validate every pair and emit its bucket key. One thread per pair.
+__global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __restrict__ keys,
+                               uint32_t* __restrict__ pn, uint32_t* __restrict__ pm,
+                               uint32_t* __restrict__ hist, uint32_t* __restrict__ err_flag,
+                               unsigned long long* __restrict__ cells)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t key = SDP_KEY_SKIP, err = 0;
+    unsigned long long my_cells = 0;
+    if (p < b.n_pairs) {
+        const uint32_t ri = b.pairs[2 * p], wi = b.pairs[2 * p + 1];
+        if (ri >= b.n_reads || wi >= b.n_wins) err = SDP_ERRF_INDEX;
+        else {
+            const uint32_t n = b.read_len[ri], m = b.win_len[wi];
+            const uint64_t ro = b.read_off[ri], wo = b.win_off[wi];
+            if (n < 1 || m < 1 || ro + n > b.reads_bases || wo + m > b.wins_bases || ro + n < ro || wo + m < wo)
+                err = SDP_ERRF_INDEX;
+            else if (n > SDP_MAX_READ_LEN ||
+                     (long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + m) + 3LL * sc.gap_open + 64 >
+                         SDP_MAX_CELL_VALUE)
+                err = SDP_ERRF_RANGE;
+            else {
+                key = (n - 1) * 64u + min(63u, m >> 6);
+                pn[p] = n; pm[p] = m;
+                my_cells = (unsigned long long)n * m;
+            }
+        }
+        keys[p] = key;
+    }
+    if (err) atomicOr(err_flag, err);
+    // warp-aggregated histogram: one atomic per distinct key per warp
+    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
+    if (key != SDP_KEY_SKIP) {
+        const uint32_t peers = __match_any_sync(active, key);
+        if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
+    }
+    for (int o = 16; o > 0; o >>= 1) my_cells += __shfl_down_sync(0xffffffffu, my_cells, o);
+    if ((threadIdx.x & 31) == 0 && my_cells) atomicAdd(cells, my_cells);
+}
+
+// histogram of precomputed keys (stages after the forward pass)
+__global__ void k_hist(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ hist)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t key = p < n ? keys[p] : SDP_KEY_SKIP;
+    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
+    if (key != SDP_KEY_SKIP) {
+        const uint32_t peers = __match_any_sync(active, key);
+        if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t block_exclusive_scan_1024(uint32_t v, uint32_t* total)
+{
+    __shared__ uint32_t warp_sums[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t x = v;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) warp_sums[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = warp_sums[lane];
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+        warp_sums[lane] = s;
+    }
+    __syncthreads();
+    const uint32_t base = w ? warp_sums[w - 1] : 0u;
+    if (total) *total = warp_sums[31];
+    __syncthreads();
+    return base + x - v;
+}
+
+// exclusive scan of the SDP_NBINS histogram in one 1024-thread block; bin_start[SDP_NBINS] = total;
+// hist is left holding a copy of bin_start (the scatter cursors)
+__global__ void __launch_bounds__(1024) k_scan_bins(uint32_t* __restrict__ hist, uint32_t* __restrict__ bin_start)
+{
+    constexpr int PER = SDP_NBINS / 1024;
+    uint32_t loc[PER];
+    uint32_t sum = 0;
+    const uint32_t base_idx = threadIdx.x * PER;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { loc[k] = hist[base_idx + k]; sum += loc[k]; }
+    uint32_t total;
+    uint32_t run = block_exclusive_scan_1024(sum, &total);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { bin_start[base_idx + k] = run; hist[base_idx + k] = run; run += loc[k]; }
+    if (threadIdx.x == 0) bin_start[SDP_NBINS] = total;
+}
+
+// scatter pair indices into bucket order (order inside one bin is not deterministic; no result
+// depends on it because every pair is aligned independently and written back by caller index)
+__global__ void k_scatter(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ cursor,
+                          uint32_t* __restrict__ order)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t key = p < n ? keys[p] : SDP_KEY_SKIP;
+    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
+    if (key != SDP_KEY_SKIP) {
+        const uint32_t peers = __match_any_sync(active, key);
+        const int leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if ((threadIdx.x & 31) == (uint32_t)leader) base = atomicAdd(cursor + key, (uint32_t)__popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        order[base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u))] = (uint32_t)p;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// task table: slot t (K-major order, host-built table slot_n/slot_G/slot_K) -> its pairs and the
+// running number of warp tasks. One 1024-thread block.
+__global__ void __launch_bounds__(1024) k_tasks(const uint32_t* __restrict__ bin_start,
+                                                const uint16_t* __restrict__ slot_n,
+                                                const uint16_t* __restrict__ slot_G,
+                                                const uint16_t* __restrict__ slot_K,
+                                                SlotInfo* __restrict__ slots, uint32_t* __restrict__ task_prefix)
+{
+    const int t = threadIdx.x;
+    const uint32_t n = slot_n[t];
+    const uint32_t first = bin_start[(n - 1) * 64u];
+    const uint32_t count = bin_start[n * 64u] - first;
+    const uint32_t G = slot_G[t];
+    const uint32_t ppw = 2u * (32u / G);
+    const uint32_t ntasks = (count + ppw - 1) / ppw;
+    uint32_t total;
+    const uint32_t pre = block_exclusive_scan_1024(ntasks, &total);
+    SlotInfo si; si.first = first; si.count = count; si.n = n; si.G = (uint16_t)G; si.K = slot_K[t];
+    slots[t] = si;
+    task_prefix[t] = pre;
+    if (t == 0) task_prefix[SDP_NSLOTS] = total;
+}
+
+// ---------------------------------------------------------------------------------------------
+// pair descriptors in bucket order for the forward pass
+__global__ void k_fill_desc_fwd(const sdp_batch b, const uint32_t* __restrict__ order, uint32_t count,
+                                PairDesc* __restrict__ desc)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const uint32_t p = order[k];
+    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+    PairDesc d;
+    d.roff = b.read_off[ri]; d.woff = b.win_off[wi];
+    d.n = b.read_len[ri]; d.m = b.win_len[wi]; d.pid = p; d.aux = 0;
+    desc[k] = d;
+}
+
+// ---------------------------------------------------------------------------------------------
+// large exclusive scan uint32 -> uint64 (cigar offsets, scratch offsets): 3 phases
+constexpr int SCAN_PER = 4;                       // elements per thread
+constexpr int SCAN_TILE = 1024 * SCAN_PER;
+
+__global__ void __launch_bounds__(1024) k_scan_tiles(const uint32_t* __restrict__ in, uint64_t n,
+                                                     uint32_t* __restrict__ local_out, uint32_t* __restrict__ tile_sums)
+{
+    const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_PER;
+    uint32_t v[SCAN_PER], sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_PER; ++k) { v[k] = (base + k < n) ? in[base + k] : 0u; sum += v[k]; }
+    uint32_t total;
+    uint32_t run = block_exclusive_scan_1024(sum, &total);
+#pragma unroll
+    for (int k = 0; k < SCAN_PER; ++k) { if (base + k < n) local_out[base + k] = run; run += v[k]; }
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_tile_sums(const uint32_t* __restrict__ tile_sums, uint32_t ntiles,
+                                                         uint64_t* __restrict__ tile_base, uint64_t* __restrict__ total_out)
+{
+    __shared__ uint64_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t start = 0; start < ntiles; start += 1024) {
+        const uint32_t idx = start + threadIdx.x;
+        const uint32_t v = idx < ntiles ? tile_sums[idx] : 0u;
+        uint32_t total;
+        const uint32_t pre = block_exclusive_scan_1024(v, &total);
+        if (idx < ntiles) tile_base[idx] = carry + pre;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *total_out = carry;
+}
+
+__global__ void k_scan_add(const uint32_t* __restrict__ local, const uint64_t* __restrict__ tile_base, uint64_t n,
+                           uint64_t* __restrict__ out)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = tile_base[i / SCAN_TILE] + local[i];
+}
+
+void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev,
+                            uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
+                            cudaStream_t st, uint32_t* launches)
+{
+    const uint32_t ntiles = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
+    if (n) k_scan_tiles<<<ntiles, 1024, 0, st>>>(in, n, tmp_local, tmp_tiles);
+    k_scan_tile_sums<<<1, 1024, 0, st>>>(tmp_tiles, ntiles, tmp_tile_base, total_dev);
+    if (n) k_scan_add<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(tmp_local, tmp_tile_base, n, out);
+    *launches += n ? 3 : 1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host wrappers
+void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
+                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st)
+{
+    const uint32_t grid = (uint32_t)((b.n_pairs + 255) / 256);
+    k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells);
+}
+
+void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t st)
+{
+    k_hist<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist);
+}
+
+void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
+                      const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
+                      SlotInfo* slots, uint32_t* task_prefix, cudaStream_t st)
+{
+    k_scan_bins<<<1, 1024, 0, st>>>(hist, bin_start);
+    k_scatter<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist, order);
+    if (slots) k_tasks<<<1, 1024, 0, st>>>(bin_start, slot_n, slot_G, slot_K, slots, task_prefix);
+}
+
+void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st)
+{
+    if (count) k_fill_desc_fwd<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, desc);
+}
+
+}  // namespace sdp

@@ -1,0 +1,66 @@
+// microbench.cu -- issue-rate microbenchmark behind sdp_measure_dpx_rate:
+// VIADDMNMX.S16x2 / VIMNMX3.S16x2, 50:50, 8 independent chains per thread, every SM full.
+#include "sdp_host.cuh"
+
+namespace sdp {
+
+constexpr int MB_ITERS = 2048;
+constexpr int MB_CHAINS = 8;
+
+__global__ void __launch_bounds__(256) k_dpx_rate(uint32_t* out, uint32_t a, uint32_t b, long long* cycles)
+{
+    uint32_t x[MB_CHAINS];
+#pragma unroll
+    for (int c = 0; c < MB_CHAINS; ++c) x[c] = threadIdx.x * 7u + c;
+    const long long t0 = clock64();
+#pragma unroll 4
+    for (int it = 0; it < MB_ITERS; ++it) {
+#pragma unroll
+        for (int c = 0; c < MB_CHAINS; ++c) {
+            x[c] = __viaddmax_s16x2(x[c], a, b);
+            x[c] = __vimax3_s16x2(x[c], a, b ^ x[(c + 1) % MB_CHAINS]);
+        }
+    }
+    const long long t1 = clock64();
+    uint32_t acc = 0;
+#pragma unroll
+    for (int c = 0; c < MB_CHAINS; ++c) acc ^= x[c];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz)
+{
+    cudaDeviceProp prop;
+    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SDP_ECUDA;
+    const int ctas_per_sm = 8, threads = 256;
+    const int grid = prop.multiProcessorCount * ctas_per_sm;
+    uint32_t* out = nullptr; long long* cyc = nullptr;
+    if (cudaMalloc(&out, (size_t)grid * threads * 4) != cudaSuccess) return SDP_ENOMEM;
+    if (cudaMalloc(&cyc, (size_t)grid * 8) != cudaSuccess) { cudaFree(out); return SDP_ENOMEM; }
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    for (int w = 0; w < 3; ++w) k_dpx_rate<<<grid, threads>>>(out, 3u, 0x00050005u, cyc);
+    cudaEventRecord(e0);
+    const int reps = 5;
+    for (int r = 0; r < reps; ++r) k_dpx_rate<<<grid, threads>>>(out, 3u, 0x00050005u, cyc);
+    cudaEventRecord(e1);
+    int rc = SDP_OK;
+    if (cudaEventSynchronize(e1) != cudaSuccess) rc = SDP_ECUDA;
+    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+    long long* h = (long long*)malloc((size_t)grid * 8);
+    cudaMemcpy(h, cyc, (size_t)grid * 8, cudaMemcpyDeviceToHost);
+    double mean_cyc = 0; for (int i = 0; i < grid; ++i) mean_cyc += (double)h[i]; mean_cyc /= grid;
+    free(h);
+    // every SM runs ctas_per_sm CTAs concurrently (one wave): instructions per SM over the
+    // cycles one CTA was resident
+    const double instr_per_sm = (double)ctas_per_sm * threads * MB_ITERS * MB_CHAINS * 2.0;
+    if (rate) *rate = instr_per_sm / mean_cyc;
+    if (sms) *sms = prop.multiProcessorCount;
+    // clock during the run: cycles of one launch / wall time of one launch
+    if (mhz) *mhz = mean_cyc / ((double)ms / reps * 1e-3) * 1e-6;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out); cudaFree(cyc);
+    if (cudaGetLastError() != cudaSuccess) rc = SDP_ECUDA;
+    return rc;
+}
+
+}  // namespace sdp

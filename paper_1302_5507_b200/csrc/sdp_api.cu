@@ -1,0 +1,538 @@
+// sdp_api.cu -- the C ABI of include/sdp.h: context, stage orchestration, host-buffer entry.
+// Stage order per call:
+//   a1 validate + key -> a2 bucket (hist, scan, scatter, task table) -> a3 forward score kernels
+//   -> W, keys -> bucket (reverse), bucket (traceback) -> a4 reverse kernels -> a5/a6 traceback
+//   -> a7 scan + compaction. a8 (un-permute) is implicit: every kernel writes its per-pair
+//   results at the caller's pair index.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "sdp_host.cuh"
+
+using namespace sdp;
+
+namespace sdp {
+bool launch_score_r0(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r1(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r2(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r3(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r4(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r5(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r6(int, bool, const ScoreParams&, cudaStream_t);
+bool launch_score_r7(int, bool, const ScoreParams&, cudaStream_t);
+void launch_score(int K, bool rev, const ScoreParams& p, cudaStream_t st) {
+    (void)(launch_score_r0(K, rev, p, st) || launch_score_r1(K, rev, p, st) || launch_score_r2(K, rev, p, st) ||
+           launch_score_r3(K, rev, p, st) || launch_score_r4(K, rev, p, st) || launch_score_r5(K, rev, p, st) ||
+           launch_score_r6(K, rev, p, st) || launch_score_r7(K, rev, p, st));
+}
+}  // namespace sdp
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr; size_t cap = 0;
+    template <class T> T* as() const { return (T*)p; }
+};
+
+struct Mailbox {                    // pinned host memory the device results land in
+    uint32_t task_prefix[2][SDP_NSLOTS + 1];
+    uint32_t bin_total[3];
+    uint32_t tb_bounds[TB_NCLASS + 1];
+    uint32_t err_flag;
+    uint64_t totals[3];             // [0] direction-bit words, [1] run capacity, [2] CIGAR runs
+    unsigned long long counters[4]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
+};
+
+enum { EV_START, EV_BUCKET, EV_FORWARD, EV_REVERSE, EV_TRACE, EV_END, EV_COUNT };
+
+}  // namespace
+
+struct sdp_ctx {
+    int device = 0;
+    sdp_scoring user_sc{};
+    Scoring sc{};
+    ScoreConsts consts{};
+    char err[512] = {0};
+    bool timing = false;
+    sdp_stats stats{};
+    uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
+    uint32_t kslot_begin[SDP_MAX_K + 2];
+    uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr;
+    Mailbox* mb = nullptr;
+    cudaStream_t own_stream = nullptr;
+    cudaEvent_t ev[EV_COUNT] = {};
+    // fixed-size device buffers
+    uint32_t* hist[3] = {};          // forward, reverse, traceback
+    uint32_t* bin_start[3] = {};
+    SlotInfo* slots[2] = {};
+    uint32_t* task_prefix[2] = {};
+    uint32_t* err_flag = nullptr;
+    unsigned long long* counters = nullptr;
+    uint64_t* totals = nullptr;
+    // per-pair device buffers (grow only)
+    DevBuf keys, pn, pm, order, desc, order_rev, desc_rev, order_tb, keys_rev, keys_tb, tbW, rev_rows,
+        bits_words, ops_cap, bits_off, ops_off, scan_local, scan_tiles, scan_tile_base,
+        score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len,
+        bits, ops_rev, cigar_ops;
+    // sdp_align_batch_host: device copies of the inputs and pinned host copies of the outputs
+    DevBuf in_reads, in_read_off, in_read_len, in_read_nmask, in_wins, in_win_off, in_win_len, in_win_nmask, in_pairs;
+    DevBuf h_out;                    // one pinned slab, carved per call
+};
+
+namespace {
+
+int fail(sdp_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap; va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CU(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? SDP_ENOMEM : SDP_ECUDA,        \
+                        "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int ensure(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
+    if (bytes <= b.cap) return SDP_OK;
+    if (b.p) { cudaFree(b.p); b.p = nullptr; b.cap = 0; }
+    size_t want = bytes + bytes / 8 + 256;
+    CU(cudaMalloc(&b.p, want));
+    b.cap = want;
+    return SDP_OK;
+}
+
+int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
+    if (bytes <= b.cap) return SDP_OK;
+    if (b.p) { cudaFreeHost(b.p); b.p = nullptr; b.cap = 0; }
+    size_t want = bytes + bytes / 8 + 256;
+    CU(cudaMallocHost(&b.p, want));
+    b.cap = want;
+    return SDP_OK;
+}
+
+#define EN(buf, bytes)                                         \
+    do {                                                       \
+        int rc_ = ensure(ctx, ctx->buf, (size_t)(bytes));      \
+        if (rc_ != SDP_OK) return rc_;                         \
+    } while (0)
+
+// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model:
+// a warp runs 2*floor(32/G) pairs for (m + G - 1) steps of (7K + row overhead) issue slots.
+void choose_geometry(sdp_ctx* c) {
+    struct Ent { uint16_t n, G, K; };
+    Ent ents[SDP_NSLOTS];
+    for (int n = 1; n <= SDP_NSLOTS; ++n) {
+        double best = -1; int bG = 32, bK = (n + 31) / 32;
+        for (int G = 1; G <= 32; ++G) {
+            int K = (n + G - 1) / G;
+            if (K > SDP_MAX_K) continue;
+            if (G * K - n >= G) continue;
+            double ppw = 2.0 * (32 / G);
+            double rows = (double)n + 300.0 + G - 1;
+            double thr = ppw / (rows * (7.0 * K + 30.0));
+            if (thr > best) { best = thr; bG = G; bK = K; }
+        }
+        ents[n - 1] = Ent{(uint16_t)n, (uint16_t)bG, (uint16_t)bK};
+    }
+    std::stable_sort(ents, ents + SDP_NSLOTS, [](const Ent& a, const Ent& b) { return a.K < b.K; });
+    for (int K = 0; K <= SDP_MAX_K + 1; ++K) c->kslot_begin[K] = SDP_NSLOTS;
+    for (int t = SDP_NSLOTS - 1; t >= 0; --t) {
+        c->h_slot_n[t] = ents[t].n; c->h_slot_G[t] = ents[t].G; c->h_slot_K[t] = ents[t].K;
+        c->kslot_begin[ents[t].K] = (uint32_t)t;
+    }
+    // K values that no read length uses start where the next used K starts
+    for (int K = SDP_MAX_K; K >= 0; --K)
+        if (c->kslot_begin[K] == SDP_NSLOTS) c->kslot_begin[K] = c->kslot_begin[K + 1];
+    c->kslot_begin[0] = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sdp_version(void) { return "sdp 0.1 (sm_100a)"; }
+
+const char* sdp_last_error(const sdp_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
+{
+    if (!s || !out) return SDP_EINVAL;
+    if (s->match < 0 || s->mismatch > 0 || s->match - s->mismatch <= 0 || s->gap_open < 0 || s->gap_extend < 1 ||
+        !(s->min_similarity >= 0.0 && s->min_similarity <= 1.0))
+        return SDP_EINVAL;
+    // the fp16 selector needs 2e + match to stay a denormal bit pattern; beta = 3o + 8 must fit too
+    if (2 * (long long)s->gap_extend + s->match > 1000 || s->gap_open > 2000 || s->mismatch < -4000) return SDP_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return SDP_ECUDA;
+    sdp_ctx* ctx = new (std::nothrow) sdp_ctx();
+    if (!ctx) return SDP_ENOMEM;
+    ctx->device = cuda_device;
+    ctx->user_sc = *s;
+    ctx->sc = Scoring{s->match, s->mismatch, s->gap_open, s->gap_extend, llround(s->min_similarity * 1e6)};
+    const int o = s->gap_open, e = s->gap_extend, beta = 3 * o + 8;
+    ctx->consts.one = 1u;
+    ctx->consts.negO = sdp_pack2(-o);
+    ctx->consts.cmis = sdp_pack2(2 * e + s->mismatch);
+    ctx->consts.Cf = sdp_pack2(2 * e + s->match);
+    ctx->consts.e2 = sdp_pack2(e);
+    ctx->consts.beta2 = sdp_pack2(beta);
+    ctx->consts.betaMinusO2 = sdp_pack2(beta - o);
+    ctx->consts.o = o; ctx->consts.e = e; ctx->consts.beta = beta; ctx->consts.match = s->match;
+    choose_geometry(ctx);
+
+    auto init = [&]() -> int {
+        CU(cudaSetDevice(cuda_device));
+        CU(cudaMalloc(&ctx->d_slot_n, SDP_NSLOTS * 2));
+        CU(cudaMalloc(&ctx->d_slot_G, SDP_NSLOTS * 2));
+        CU(cudaMalloc(&ctx->d_slot_K, SDP_NSLOTS * 2));
+        CU(cudaMemcpy(ctx->d_slot_n, ctx->h_slot_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->d_slot_G, ctx->h_slot_G, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->d_slot_K, ctx->h_slot_K, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+        CU(cudaMallocHost(&ctx->mb, sizeof(Mailbox)));
+        memset(ctx->mb, 0, sizeof(Mailbox));
+        CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
+        for (int i = 0; i < 3; ++i) {
+            CU(cudaMalloc(&ctx->hist[i], (SDP_NBINS + 1) * 4));
+            CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 1) * 4));
+        }
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaMalloc(&ctx->slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
+            CU(cudaMalloc(&ctx->task_prefix[i], (SDP_NSLOTS + 1) * 4));
+        }
+        CU(cudaMalloc(&ctx->err_flag, 4));
+        CU(cudaMalloc(&ctx->counters, 4 * 8));
+        CU(cudaMalloc(&ctx->totals, 3 * 8));
+        return SDP_OK;
+    };
+    int rc = init();
+    if (rc != SDP_OK) { sdp_destroy(ctx); return rc; }
+    *out = ctx;
+    return SDP_OK;
+}
+
+void sdp_destroy(sdp_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->order_rev, &ctx->desc_rev,
+                      &ctx->order_tb, &ctx->keys_rev, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
+                      &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local, &ctx->scan_tiles,
+                      &ctx->scan_tile_base, &ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start,
+                      &ctx->read_end, &ctx->pass, &ctx->n_match, &ctx->n_cols, &ctx->cigar_off, &ctx->cigar_len,
+                      &ctx->bits, &ctx->ops_rev, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
+                      &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
+                      &ctx->in_win_nmask, &ctx->in_pairs};
+    for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
+    if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
+    for (int i = 0; i < 3; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
+    for (int i = 0; i < 2; ++i) { cudaFree(ctx->slots[i]); cudaFree(ctx->task_prefix[i]); }
+    cudaFree(ctx->err_flag); cudaFree(ctx->counters); cudaFree(ctx->totals);
+    cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K);
+    if (ctx->mb) cudaFreeHost(ctx->mb);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+}
+
+int sdp_set_timing(sdp_ctx* ctx, int enabled)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->timing = enabled != 0;
+    return SDP_OK;
+}
+
+int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out)
+{
+    if (!ctx || !out) return SDP_EINVAL;
+    *out = ctx->stats;
+    return SDP_OK;
+}
+
+int sdp_measure_dpx_rate(int cuda_device, double* rate, int32_t* sms, double* mhz)
+{
+    return measure_dpx_rate(cuda_device, rate, sms, mhz);
+}
+
+static int launch_score_stage(sdp_ctx* ctx, int which, bool rev, const sdp_batch& b, const PairDesc* desc,
+                              cudaStream_t st, uint32_t* nlaunch)
+{
+    const uint32_t* tp = ctx->mb->task_prefix[which];
+    ScoreParams sp{};
+    sp.reads_packed = b.reads_packed; sp.read_nmask = b.read_nmask;
+    sp.wins_packed = b.wins_packed; sp.win_nmask = b.win_nmask;
+    sp.desc = desc;
+    sp.task_prefix = ctx->task_prefix[which];
+    sp.slots = ctx->slots[which];
+    sp.c = ctx->consts;
+    sp.score = ctx->score.as<int32_t>(); sp.ref_end = ctx->ref_end.as<int32_t>();
+    sp.rev_rows = ctx->rev_rows.as<int32_t>(); sp.err_flag = ctx->err_flag;
+    for (int K = 1; K <= SDP_MAX_K; ++K) {
+        const uint32_t s0 = ctx->kslot_begin[K], s1 = ctx->kslot_begin[K + 1];
+        if (s1 <= s0) continue;
+        const uint32_t t0 = tp[s0], t1 = tp[s1];
+        if (t1 <= t0) continue;
+        sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
+        launch_score(K, rev, sp, st);
+        ++*nlaunch;
+    }
+    CU(cudaGetLastError());
+    return SDP_OK;
+}
+
+int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp_result* out)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!batch || !out) return fail(ctx, SDP_EINVAL, "null batch or result");
+    const sdp_batch& b = *batch;
+    const uint64_t P = b.n_pairs;
+    if (P > 0 && (!b.reads_packed || !b.read_off || !b.read_len || !b.wins_packed || !b.win_off || !b.win_len ||
+                  !b.pairs || b.n_reads == 0 || b.n_wins == 0))
+        return fail(ctx, SDP_EINVAL, "null input array");
+    if (P > 0xFFFFFFF0ull) return fail(ctx, SDP_EINVAL, "too many pairs");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->device));
+    sdp_stats stats{};
+    stats.n_pairs = P;
+    uint32_t nl = 0;
+
+    const size_t Pp = (size_t)(P ? P : 1);
+    EN(keys, Pp * 4); EN(pn, Pp * 4); EN(pm, Pp * 4); EN(order, Pp * 4); EN(desc, Pp * sizeof(PairDesc));
+    EN(order_rev, Pp * 4); EN(desc_rev, Pp * sizeof(PairDesc)); EN(order_tb, Pp * 4);
+    EN(keys_rev, Pp * 4); EN(keys_tb, Pp * 4); EN(tbW, Pp * 4); EN(rev_rows, Pp * 4);
+    EN(bits_words, Pp * 4); EN(ops_cap, Pp * 4); EN(bits_off, Pp * 8); EN(ops_off, Pp * 8);
+    EN(scan_local, Pp * 4); EN(scan_tiles, (Pp / 4096 + 2) * 4); EN(scan_tile_base, (Pp / 4096 + 2) * 8);
+    EN(score, Pp * 4); EN(ref_start, Pp * 4); EN(ref_end, Pp * 4); EN(read_start, Pp * 4); EN(read_end, Pp * 4);
+    EN(pass, Pp); EN(n_match, Pp * 4); EN(n_cols, Pp * 4); EN(cigar_off, Pp * 8); EN(cigar_len, Pp * 4);
+
+    auto finish = [&](uint64_t n_ops) {
+        out->score = ctx->score.as<int32_t>(); out->ref_start = ctx->ref_start.as<int32_t>();
+        out->ref_end = ctx->ref_end.as<int32_t>(); out->read_start = ctx->read_start.as<int32_t>();
+        out->read_end = ctx->read_end.as<int32_t>(); out->pass = ctx->pass.as<uint8_t>();
+        out->n_match = ctx->n_match.as<int32_t>(); out->n_cols = ctx->n_cols.as<int32_t>();
+        out->cigar_off = ctx->cigar_off.as<uint64_t>(); out->cigar_len = ctx->cigar_len.as<uint32_t>();
+        out->cigar_ops = ctx->cigar_ops.as<uint32_t>(); out->n_cigar_ops = n_ops; out->n_pairs = P;
+    };
+    if (P == 0) {
+        EN(cigar_ops, 16);
+        ctx->stats = stats;
+        finish(0);
+        return SDP_OK;
+    }
+
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_START], st));
+    // ---- a1 + a2
+    for (int i = 0; i < 3; ++i) CU(cudaMemsetAsync(ctx->hist[i], 0, (SDP_NBINS + 1) * 4, st));
+    CU(cudaMemsetAsync(ctx->err_flag, 0, 4, st));
+    CU(cudaMemsetAsync(ctx->counters, 0, 4 * 8, st));
+    launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
+                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, st);
+    launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0], st);
+    nl += 4;
+    CU(cudaMemcpyAsync(ctx->mb->task_prefix[0], ctx->task_prefix[0], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&ctx->mb->bin_total[0], ctx->bin_start[0] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (ctx->mb->err_flag & SDP_ERRF_INDEX)
+        return fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)");
+    if (ctx->mb->err_flag & SDP_ERRF_RANGE)
+        return fail(ctx, SDP_ERANGE, "a pair breaks the int16 range rule or SDP_MAX_READ_LEN (see sdp.h)");
+    launch_fill_desc_fwd(b, ctx->order.as<uint32_t>(), (uint32_t)P, ctx->desc.as<PairDesc>(), st);
+    ++nl;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_BUCKET], st));
+
+    // ---- a3 forward score pass
+    {
+        uint32_t before = nl;
+        int rc = launch_score_stage(ctx, 0, false, b, ctx->desc.as<PairDesc>(), st, &nl);
+        if (rc != SDP_OK) return rc;
+        stats.forward_launches = nl - before;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_FORWARD], st));
+
+    // ---- gap bound W, keys of the two later stages, scratch sizes
+    PostParams pp{};
+    pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
+    pp.score = ctx->score.as<int32_t>(); pp.ref_end = ctx->ref_end.as<int32_t>();
+    pp.tbW = ctx->tbW.as<int32_t>(); pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
+    pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
+    pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.counters = ctx->counters;
+    launch_post_forward(pp, st);
+    launch_sort_tail(ctx->keys_rev.as<uint32_t>(), P, ctx->hist[1], ctx->bin_start[1], ctx->order_rev.as<uint32_t>(),
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1], st);
+    launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
+                     nullptr, nullptr, nullptr, nullptr, nullptr, st);
+    nl += 6;
+    exclusive_scan_u32_u64(ctx->bits_words.as<uint32_t>(), P, ctx->bits_off.as<uint64_t>(), ctx->totals + 0,
+                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
+                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+    exclusive_scan_u32_u64(ctx->ops_cap.as<uint32_t>(), P, ctx->ops_off.as<uint64_t>(), ctx->totals + 1,
+                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
+                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+    CU(cudaMemcpyAsync(ctx->mb->task_prefix[1], ctx->task_prefix[1], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&ctx->mb->bin_total[1], ctx->bin_start[1] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
+    for (int c = 0; c <= TB_NCLASS; ++c)
+        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * 8192, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 2 * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->mb->counters, ctx->counters, 4 * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const uint32_t n_rev = ctx->mb->bin_total[1];
+    EN(bits, (ctx->mb->totals[0] + 4) * 4);
+    EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
+    EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
+
+    // ---- a4 reverse pass over the pairs whose score admits a gap
+    launch_fill_desc_rev(b, ctx->order_rev.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
+                         ctx->tbW.as<int32_t>(), ctx->desc_rev.as<PairDesc>(), st);
+    ++nl;
+    {
+        int rc = launch_score_stage(ctx, 1, true, b, ctx->desc_rev.as<PairDesc>(), st, &nl);
+        if (rc != SDP_OK) return rc;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_REVERSE], st));
+
+    // ---- a5 + a6 traceback, CIGAR runs, similarity filter
+    TraceParams tp{};
+    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
+    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
+    tp.rev_rows = ctx->rev_rows.as<int32_t>();
+    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
+    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
+    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
+    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
+    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
+    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
+    for (int c = 0; c < TB_NCLASS; ++c) {
+        tp.first = ctx->mb->tb_bounds[c];
+        const uint32_t end = (c + 1 < TB_NCLASS) ? ctx->mb->tb_bounds[c + 1] : (uint32_t)P;
+        tp.count = end - tp.first;
+        if (tp.count) { launch_traceback(c, tp, st); ++nl; }
+    }
+    CU(cudaGetLastError());
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
+
+    // ---- a7 compaction in caller pair order
+    exclusive_scan_u32_u64(ctx->cigar_len.as<uint32_t>(), P, ctx->cigar_off.as<uint64_t>(), ctx->totals + 2,
+                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
+                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+    launch_compact(P, ctx->ops_off.as<uint64_t>(), ctx->ops_rev.as<uint32_t>(), ctx->cigar_len.as<uint32_t>(),
+                   ctx->cigar_off.as<uint64_t>(), ctx->cigar_ops.as<uint32_t>(), st);
+    ++nl;
+    CU(cudaMemcpyAsync(&ctx->mb->totals[2], ctx->totals + 2, 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if ((ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE)) && getenv("SDP_DEBUG_NOFAIL"))
+        fprintf(stderr, "[sdp] internal flags 0x%x ignored (SDP_DEBUG_NOFAIL)\n", ctx->mb->err_flag);
+    else if (ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
+        return fail(ctx, SDP_ECUDA, "internal consistency check failed (flags 0x%x): reverse pass or traceback "
+                    "disagrees with the forward score", ctx->mb->err_flag);
+
+    stats.cells_forward = ctx->mb->counters[3];
+    stats.cells_reverse = ctx->mb->counters[0];
+    stats.cells_traceback = ctx->mb->counters[1];
+    stats.n_reverse_pairs = ctx->mb->counters[2];
+    stats.kernel_launches = nl;
+    if (ctx->timing) {
+        cudaEventElapsedTime(&stats.ms_total, ctx->ev[EV_START], ctx->ev[EV_END]);
+        cudaEventElapsedTime(&stats.ms_bucket, ctx->ev[EV_START], ctx->ev[EV_BUCKET]);
+        cudaEventElapsedTime(&stats.ms_forward, ctx->ev[EV_BUCKET], ctx->ev[EV_FORWARD]);
+        cudaEventElapsedTime(&stats.ms_reverse, ctx->ev[EV_FORWARD], ctx->ev[EV_REVERSE]);
+        cudaEventElapsedTime(&stats.ms_traceback, ctx->ev[EV_REVERSE], ctx->ev[EV_TRACE]);
+        cudaEventElapsedTime(&stats.ms_compact, ctx->ev[EV_TRACE], ctx->ev[EV_END]);
+    }
+    ctx->stats = stats;
+    finish(ctx->mb->totals[2]);
+    return SDP_OK;
+}
+
+int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!hb || !out) return fail(ctx, SDP_EINVAL, "null batch or result");
+    const uint64_t P = hb->n_pairs;
+    if (P > 0 && (!hb->reads_packed || !hb->read_off || !hb->read_len || !hb->wins_packed || !hb->win_off ||
+                  !hb->win_len || !hb->pairs))
+        return fail(ctx, SDP_EINVAL, "null input array");
+    CU(cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->own_stream;
+    sdp_batch d = *hb;
+    auto words16 = [](uint64_t bases) { return (size_t)(((bases + 15) / 16 + 3) / 4 * 4); };
+    auto words32 = [](uint64_t bases) { return (size_t)(((bases + 31) / 32 + 3) / 4 * 4); };
+    struct Cp { DevBuf* buf; const void* src; size_t bytes; const void** dst; };
+    // the caller's buffers are only guaranteed readable to the end of the last word in use
+    const size_t rb = (size_t)((hb->reads_bases + 15) / 16) * 4, wb = (size_t)((hb->wins_bases + 15) / 16) * 4;
+    const size_t rnb = (size_t)((hb->reads_bases + 31) / 32) * 4, wnb = (size_t)((hb->wins_bases + 31) / 32) * 4;
+    Cp cps[] = {
+        {&ctx->in_reads, hb->reads_packed, rb, (const void**)&d.reads_packed},
+        {&ctx->in_read_off, hb->read_off, (size_t)hb->n_reads * 8, (const void**)&d.read_off},
+        {&ctx->in_read_len, hb->read_len, (size_t)hb->n_reads * 4, (const void**)&d.read_len},
+        {&ctx->in_read_nmask, hb->read_nmask, rnb, (const void**)&d.read_nmask},
+        {&ctx->in_wins, hb->wins_packed, wb, (const void**)&d.wins_packed},
+        {&ctx->in_win_off, hb->win_off, (size_t)hb->n_wins * 8, (const void**)&d.win_off},
+        {&ctx->in_win_len, hb->win_len, (size_t)hb->n_wins * 4, (const void**)&d.win_len},
+        {&ctx->in_win_nmask, hb->win_nmask, wnb, (const void**)&d.win_nmask},
+        {&ctx->in_pairs, hb->pairs, (size_t)P * 8, (const void**)&d.pairs},
+    };
+    (void)words16; (void)words32;
+    for (Cp& c : cps) {
+        if (!c.src) { *c.dst = nullptr; continue; }
+        int rc = ensure(ctx, *c.buf, c.bytes + 64);
+        if (rc != SDP_OK) return rc;
+        if (c.bytes) CU(cudaMemcpyAsync(c.buf->p, c.src, c.bytes, cudaMemcpyHostToDevice, st));
+        *c.dst = c.buf->p;
+    }
+    sdp_result dr{};
+    int rc = sdp_align_batch(ctx, &d, st, &dr);
+    if (rc != SDP_OK) return rc;
+    // results back into one pinned slab
+    const size_t Pp = (size_t)(P ? P : 1);
+    const size_t n_ops = (size_t)dr.n_cigar_ops;
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { size_t o = off; off += (bytes + 63) / 64 * 64; return o; };
+    const size_t o_score = carve(Pp * 4), o_rs = carve(Pp * 4), o_re = carve(Pp * 4), o_qs = carve(Pp * 4),
+                 o_qe = carve(Pp * 4), o_pass = carve(Pp), o_nm = carve(Pp * 4), o_nc = carve(Pp * 4),
+                 o_coff = carve(Pp * 8), o_clen = carve(Pp * 4), o_ops = carve((n_ops + 1) * 4);
+    rc = ensure_pinned(ctx, ctx->h_out, off);
+    if (rc != SDP_OK) return rc;
+    char* h = (char*)ctx->h_out.p;
+    if (P) {
+        CU(cudaMemcpyAsync(h + o_score, dr.score, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_rs, dr.ref_start, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_re, dr.ref_end, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_qs, dr.read_start, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_qe, dr.read_end, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_pass, dr.pass, P, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_nm, dr.n_match, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_nc, dr.n_cols, P * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_coff, dr.cigar_off, P * 8, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h + o_clen, dr.cigar_len, P * 4, cudaMemcpyDeviceToHost, st));
+        if (n_ops) CU(cudaMemcpyAsync(h + o_ops, dr.cigar_ops, n_ops * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    out->score = (const int32_t*)(h + o_score); out->ref_start = (const int32_t*)(h + o_rs);
+    out->ref_end = (const int32_t*)(h + o_re); out->read_start = (const int32_t*)(h + o_qs);
+    out->read_end = (const int32_t*)(h + o_qe); out->pass = (const uint8_t*)(h + o_pass);
+    out->n_match = (const int32_t*)(h + o_nm); out->n_cols = (const int32_t*)(h + o_nc);
+    out->cigar_off = (const uint64_t*)(h + o_coff); out->cigar_len = (const uint32_t*)(h + o_clen);
+    out->cigar_ops = (const uint32_t*)(h + o_ops); out->n_cigar_ops = n_ops; out->n_pairs = P;
+    return SDP_OK;
+}
+
+}  // extern "C"

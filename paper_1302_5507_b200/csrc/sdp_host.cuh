@@ -1,0 +1,69 @@
+// sdp_host.cuh -- host-side declarations shared by the translation units of libsdp.
+#pragma once
+#include "../../include/sdp.h"
+#include "sdp_internal.cuh"
+
+namespace sdp {
+
+struct Scoring {
+    int32_t match, mismatch, gap_open, gap_extend;
+    long long min_sim_q;            // llround(min_similarity * 1e6)
+};
+
+// ---- bucket.cu
+void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
+                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st);
+void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t st);
+// scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
+void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
+                      const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
+                      SlotInfo* slots, uint32_t* task_prefix, cudaStream_t st);
+void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st);
+void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev,
+                            uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
+                            cudaStream_t st, uint32_t* launches);
+
+// ---- score_inst.cu (compiled once per K range)
+void launch_score(int K, bool rev, const ScoreParams& p, cudaStream_t st);
+
+// ---- traceback.cu
+struct PostParams {
+    uint64_t n_pairs;
+    Scoring sc;
+    const uint32_t* pn; const uint32_t* pm;      // per pair read / window length
+    const int32_t* score; const int32_t* ref_end;
+    int32_t* tbW;                // gap-content bound W per pair
+    uint32_t* keys_rev;          // bucket key of the reverse pass (SKIP when W == 0)
+    uint32_t* keys_tb;           // bucket key of the traceback pass
+    uint32_t* bits_words;        // direction-bit words the pair needs
+    uint32_t* ops_cap;           // CIGAR run capacity the pair needs (2W + 1)
+    uint32_t* hist_rev; uint32_t* hist_tb;
+    unsigned long long* counters;   // [0] reverse cells, [1] traceback cells, [2] reverse pairs
+};
+void launch_post_forward(const PostParams& pp, cudaStream_t st);
+void launch_fill_desc_rev(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
+                          const int32_t* ref_end, const int32_t* tbW, PairDesc* desc, cudaStream_t st);
+
+struct TraceParams {
+    sdp_batch b;
+    Scoring sc;
+    const uint32_t* order;       // traceback bucket order
+    uint32_t first, count;       // range of `order` this launch covers
+    const int32_t* score; const int32_t* ref_end; const int32_t* tbW; const int32_t* rev_rows;
+    const uint64_t* bits_off; uint32_t* bits;     // direction bits scratch
+    const uint64_t* ops_off;  uint32_t* ops_rev;  // per-pair runs, end -> start order
+    int32_t* ref_start; int32_t* read_start; int32_t* read_end; uint8_t* pass;
+    int32_t* n_match; int32_t* n_cols; uint32_t* cigar_len;
+    uint32_t* err_flag;
+};
+// band-width classes of the traceback kernel (local-memory row arrays)
+constexpr int TB_NCLASS = 4;
+constexpr int TB_CLASS_BW[TB_NCLASS] = {16, 64, 256, 1032};   // band <= min(2W+1, n+1) <= 1025
+void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st);
+void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
+                    const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
+
+// ---- microbench.cu
+int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz);
+
+}  // namespace sdp

@@ -1,0 +1,77 @@
+// sdp_internal.cuh -- structures shared by the kernels and the host-side driver of libsdp.
+// Not part of the ABI (include/sdp.h is). Notation follows the paper:
+// window T[1..m] indexed by i (rows), read R[1..n] indexed by j (columns).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define SDP_WARPS_PER_CTA 4
+#define SDP_SCORE_THREADS (32 * SDP_WARPS_PER_CTA)
+#define SDP_MAX_K 32            // columns of the read one thread keeps in registers
+#define SDP_NBINS 65536         // bucket-sort key space: (n-1) * 64 + min(63, rows >> 6)
+#define SDP_NSLOTS 1024         // one slot per read length 1..SDP_MAX_READ_LEN
+#define SDP_KEY_SKIP 0xFFFFFFFFu
+
+// device-side error flag bits
+#define SDP_ERRF_INDEX   1u     // pair index / offset out of range, empty sequence
+#define SDP_ERRF_REVERSE 2u     // reverse pass did not reproduce the forward score (internal)
+#define SDP_ERRF_RANGE   4u     // int16 range rule or SDP_MAX_READ_LEN broken
+#define SDP_ERRF_TRACE   8u     // traceback left its band or overflowed its run buffer (internal)
+
+// fp16 code of base c (0..3 = ACGT, 4 = read N, 5 = window N): 1.0 + 0.25*c, exact in fp16
+#define SDP_CODE_READ_N 4u
+#define SDP_CODE_WIN_N 5u
+
+// One pair as the score kernel sees it, stored in bucket order.
+struct PairDesc {
+    uint64_t roff;     // first read base (in bases) -- forward orientation for both passes
+    uint64_t woff;     // window base of DP row 1: win_off (forward) or win_off + ref_end (reverse)
+    uint32_t n;        // read length (columns)
+    uint32_t m;        // DP rows: window length (forward) or min(ref_end + 1, n + W) (reverse)
+    uint32_t pid;      // caller pair index
+    int32_t  aux;      // reverse pass: forward score S
+};
+
+// One read length in the task table. Tasks (one per warp) of slot s are
+// task_prefix[s] .. task_prefix[s+1]; task t of the slot takes pairs first + t*ppw ..
+struct SlotInfo {
+    uint32_t first;    // index of the slot's first pair in bucket order
+    uint32_t count;    // pairs in the slot
+    uint32_t n;        // read length
+    uint16_t G;        // threads per pair-of-pairs (anti-diagonal group)
+    uint16_t K;        // columns per thread; G*K - n in [0, G)
+};
+
+struct ScoreConsts {
+    uint32_t one;      // 1, opaque to the compiler (keeps the 32-bit add on the FMA pipe as IMAD)
+    uint32_t negO;     // packed (-o, -o)
+    uint32_t cmis;     // packed (2e + mismatch)
+    uint32_t Cf;       // packed fp16 bit pattern == integer (2e + match), a denormal
+    uint32_t e2;       // packed (e, e)
+    uint32_t beta2;    // packed (beta, beta)
+    uint32_t betaMinusO2;
+    int32_t  o, e, beta, match;
+};
+
+struct ScoreParams {
+    const uint32_t* reads_packed; const uint32_t* read_nmask;
+    const uint32_t* wins_packed;  const uint32_t* win_nmask;
+    const PairDesc* desc;
+    const uint32_t* task_prefix;   // [SDP_NSLOTS + 1], slots in K-major order
+    const SlotInfo* slots;         // [SDP_NSLOTS]
+    uint32_t slot_lo, slot_hi;     // slots of this launch's K
+    uint32_t task_begin, task_end; // == task_prefix[slot_lo], task_prefix[slot_hi]
+    ScoreConsts c;
+    int32_t* score;                // forward outputs, caller order
+    int32_t* ref_end;
+    int32_t* rev_rows;             // reverse output: window rows consumed by the longest alignment
+                                   // that scores S (lowest co-optimal start = ref_end + 1 - rows)
+    uint32_t* err_flag;            // reverse: SDP_ERRF_REVERSE when max != S
+};
+
+typedef void (*sdp_score_launch_fn)(int K, bool rev, const ScoreParams& p, cudaStream_t st);
+
+// packed helpers
+__host__ __device__ static inline uint32_t sdp_pack2(int v) {
+    return ((uint32_t)(uint16_t)(int16_t)v) | (((uint32_t)(uint16_t)(int16_t)v) << 16);
+}

@@ -1,0 +1,278 @@
+// traceback.cu -- a5 (banded traceback + CIGAR), a6 (similarity filter), a7 (CIGAR compaction).
+//
+// The paper backtracks through full tables D and M kept in global memory. Here
+// the forward pass keeps no table; instead the score S bounds the gap content of every
+// co-optimal alignment, W = floor((n*match - S - o) / e) (0 when negative), so all co-optimal
+// paths lie in the band |i - j - (i_end - n)| <= W and in rows >= i_lo = max(s_lo, i_end-n-W).
+// The DP restricted to that band equals the full DP on every co-optimal cell, so the equality
+// tests of the walk (diagonal first, then deletion, then insertion; "opened here" before
+// "extended") resolve exactly as in the full-table oracle.
+// W == 0 means the alignment is gapless: CIGAR nM, no DP at all.
+#include "sdp_host.cuh"
+
+namespace sdp {
+
+constexpr int NEG = -(1 << 28);
+
+// sequential reader of a 2-bit packed sequence with optional N bitmap
+struct SeqReader {
+    const uint32_t* packed; const uint32_t* nmask; uint32_t ncode;
+    __device__ __forceinline__ uint32_t at(uint64_t pos) const {
+        uint32_t c = (__ldg(packed + (pos >> 4)) >> (2u * ((uint32_t)pos & 15u))) & 3u;
+        if (nmask != nullptr && ((__ldg(nmask + (pos >> 5)) >> ((uint32_t)pos & 31u)) & 1u)) c = ncode;
+        return c;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// after the forward pass: gap-content bound, bucket keys of the reverse and traceback passes,
+// scratch sizes. One thread per pair.
+__device__ __forceinline__ int tb_class_of(int bw) {
+    static_assert(TB_NCLASS == 4, "update tb_class_of");
+    return bw > 256 ? 3 : (bw > 64 ? 2 : (bw > 16 ? 1 : 0));
+}
+
+__device__ __forceinline__ void hist_add(uint32_t* hist, uint32_t key, bool valid) {
+    const uint32_t active = __ballot_sync(0xffffffffu, valid);
+    if (valid) {
+        const uint32_t peers = __match_any_sync(active, key);
+        if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
+    }
+}
+
+__global__ void k_post_forward(const PostParams pp)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = p < pp.n_pairs;
+    uint32_t krev = SDP_KEY_SKIP, ktb = SDP_KEY_SKIP;
+    unsigned long long c_rev = 0, c_tb = 0, n_rev = 0;
+    if (valid) {
+        const int n = (int)pp.pn[p];
+        const int S = pp.score[p], i_end = pp.ref_end[p] + 1;
+        const int slack = n * pp.sc.match - S - pp.sc.gap_open;
+        int W = slack >= pp.sc.gap_extend ? slack / pp.sc.gap_extend : 0;
+        W = min(W, n + i_end);
+        pp.tbW[p] = W;
+        uint32_t words = 0;
+        int bw = 1;
+        if (W > 0) {
+            const int rows = min(i_end, n + W);
+            krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
+            bw = min(2 * W + 1, n + 1);
+            words = (uint32_t)rows * (uint32_t)((bw + 7) / 8);
+            c_rev = (unsigned long long)n * rows; c_tb = (unsigned long long)bw * rows; n_rev = 1;
+        }
+        pp.keys_rev[p] = krev;
+        pp.bits_words[p] = words;
+        pp.ops_cap[p] = 2u * (uint32_t)W + 3u;
+        ktb = (uint32_t)tb_class_of(bw) * 8192u + (uint32_t)min(bw, 8191);
+        pp.keys_tb[p] = ktb;
+    }
+    hist_add(pp.hist_rev, krev, krev != SDP_KEY_SKIP);
+    hist_add(pp.hist_tb, ktb, ktb != SDP_KEY_SKIP);
+    for (int o = 16; o > 0; o >>= 1) {
+        c_rev += __shfl_down_sync(0xffffffffu, c_rev, o);
+        c_tb += __shfl_down_sync(0xffffffffu, c_tb, o);
+        n_rev += __shfl_down_sync(0xffffffffu, n_rev, o);
+    }
+    if ((threadIdx.x & 31) == 0 && n_rev) {
+        atomicAdd(pp.counters + 0, c_rev); atomicAdd(pp.counters + 1, c_tb); atomicAdd(pp.counters + 2, n_rev);
+    }
+}
+
+void launch_post_forward(const PostParams& pp, cudaStream_t st)
+{
+    if (pp.n_pairs) k_post_forward<<<(uint32_t)((pp.n_pairs + 255) / 256), 256, 0, st>>>(pp);
+}
+
+// descriptors of the reverse pass, in its bucket order: DP row 1 is window base ref_end, the
+// read is walked from its last base, rows = min(ref_end + 1, n + W)
+__global__ void k_fill_desc_rev(const sdp_batch b, const uint32_t* __restrict__ order, uint32_t count,
+                                const int32_t* __restrict__ score, const int32_t* __restrict__ ref_end,
+                                const int32_t* __restrict__ tbW, PairDesc* __restrict__ desc)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const uint32_t p = order[k];
+    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+    PairDesc d;
+    d.n = b.read_len[ri];
+    d.roff = b.read_off[ri];
+    d.woff = b.win_off[wi] + (uint64_t)ref_end[p];
+    d.m = (uint32_t)min(ref_end[p] + 1, (int)d.n + tbW[p]);
+    d.pid = p; d.aux = score[p];
+    desc[k] = d;
+}
+
+void launch_fill_desc_rev(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
+                          const int32_t* ref_end, const int32_t* tbW, PairDesc* desc, cudaStream_t st)
+{
+    if (count) k_fill_desc_rev<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, score, ref_end, tbW, desc);
+}
+
+// ---------------------------------------------------------------------------------------------
+// traceback: one thread per pair, row arrays of the band in local memory (MAXBW + 2 entries).
+// Direction bits per cell: 1 = H came from the diagonal, 2 = H equals D, 4 = D was opened here,
+// 8 = I was opened here. Rows i_lo+1 .. i_end each take wpr = ceil(bw / 8) words.
+template <int MAXBW>
+__global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= tp.count) return;
+    const uint32_t p = tp.order[tp.first + k];
+    const sdp_batch& b = tp.b;
+    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+    const int n = (int)b.read_len[ri];
+    const uint64_t roff = b.read_off[ri], woff = b.win_off[wi];
+    const SeqReader RD{b.reads_packed, b.read_nmask, SDP_CODE_READ_N};
+    const SeqReader WN{b.wins_packed, b.win_nmask, SDP_CODE_WIN_N};
+    const int i_end = tp.ref_end[p] + 1;
+    const int W = tp.tbW[p];
+    const int o = tp.sc.gap_open, e = tp.sc.gap_extend, oe = o + e;
+    uint32_t* ops = tp.ops_rev + tp.ops_off[p];
+    const uint32_t cap = 2u * (uint32_t)W + 3u;
+
+    int n_match = 0, n_cols = 0, ref_start = 0;
+    uint32_t nops = 0;
+    int cur_op = -1; uint32_t cur_len = 0;
+    bool bad = false;
+    auto emit = [&](int op, uint32_t len) {
+        if (op == cur_op) { cur_len += len; return; }
+        if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
+        cur_op = op; cur_len = len;
+    };
+
+    if (W == 0) {
+        // gapless: the only co-optimal alignments are ungapped, so the CIGAR is nM
+        ref_start = i_end - n;
+        if (ref_start < 0) { bad = true; ref_start = 0; }
+        for (int j = 0; j < n; ++j) {
+            const uint32_t r = RD.at(roff + (uint64_t)j), t = WN.at(woff + (uint64_t)(ref_start + j));
+            n_match += (r == t);
+        }
+        n_cols = n;
+        emit(0, (uint32_t)n);
+    } else {
+        const int c = i_end - n;
+        const int s_lo = tp.rev_rows ? i_end - tp.rev_rows[p] : 0;
+        const int i_lo = max(0, max(s_lo, i_end - n - W));
+        const bool banded = (2 * W + 1 < n + 1);
+        const int bw = banded ? 2 * W + 1 : n + 1;
+        const int shift = banded ? 1 : 0;
+        const int wpr = (bw + 7) / 8;
+        uint32_t* bits = tp.bits + tp.bits_off[p];
+        if (bw > MAXBW) { bad = true; }
+        else {
+            int Hr[MAXBW + 2], Dr[MAXBW + 2];
+            // row i_lo is the restricted problem's row 0: H = -(o + e j) via insertions, H(.,0) = 0
+            {
+                const int jb = banded ? (i_lo - c - W) : 0;
+                for (int jj = 0; jj <= bw; ++jj) {
+                    const int j = jj + jb;
+                    Hr[jj] = (jj == bw || j < 0 || j > n) ? NEG : (j == 0 ? 0 : -(o + e * j));
+                    Dr[jj] = NEG;
+                }
+            }
+            for (int i = i_lo + 1; i <= i_end; ++i) {
+                const uint32_t t = WN.at(woff + (uint64_t)(i - 1));
+                const int jb = banded ? (i - c - W) : 0;
+                int Hleft = NEG, Ileft = NEG, saved_old = NEG;
+                uint32_t word = 0;
+                uint32_t* brow = bits + (size_t)(i - i_lo - 1) * wpr;
+                for (int jj = 0; jj < bw; ++jj) {
+                    const int j = jj + jb;
+                    const int oldH = Hr[jj];
+                    const int upH = shift ? Hr[jj + 1] : oldH;
+                    const int upD = shift ? Dr[jj + 1] : Dr[jj];
+                    const int dgH = shift ? oldH : saved_old;
+                    saved_old = oldH;
+                    int Hn, Dn, In;
+                    uint32_t f = 0;
+                    if (j < 0 || j > n) { Hn = NEG; Dn = NEG; In = NEG; }
+                    else if (j == 0) { Hn = 0; Dn = NEG; In = NEG; }
+                    else {
+                        const uint32_t r = RD.at(roff + (uint64_t)(j - 1));
+                        In = max(Hleft - oe, Ileft - e);
+                        Dn = max(upH - oe, upD - e);
+                        const int dg = dgH + ((r == t) ? tp.sc.match : tp.sc.mismatch);
+                        Hn = max(dg, max(Dn, In));
+                        f = (Hn == dg ? 1u : 0u) | (Hn == Dn ? 2u : 0u) | (Dn == upH - oe ? 4u : 0u) |
+                            (In == Hleft - oe ? 8u : 0u);
+                    }
+                    Hr[jj] = Hn; Dr[jj] = Dn; Hleft = Hn; Ileft = In;
+                    word |= f << (4 * (jj & 7));
+                    if ((jj & 7) == 7 || jj == bw - 1) { brow[jj >> 3] = word; word = 0; }
+                }
+            }
+            if (Hr[n - (banded ? (i_end - c - W) : 0)] != tp.score[p]) bad = true;   // band DP must end on S
+            // walk back from (i_end, n)
+            int i = i_end, j = n, st = 0;                  // 0 = H, 1 = D, 2 = I
+            while (j > 0) {
+                if (i == i_lo) { emit(1, (uint32_t)j); n_cols += j; j = 0; break; }
+                const int jj = j - (banded ? (i - c - W) : 0);
+                if (jj < 0 || jj >= bw) { bad = true; break; }
+                const uint32_t f = (bits[(size_t)(i - i_lo - 1) * wpr + (jj >> 3)] >> (4 * (jj & 7))) & 15u;
+                if (st == 0) {
+                    if (f & 1u) {
+                        emit(0, 1u); ++n_cols;
+                        n_match += (RD.at(roff + (uint64_t)(j - 1)) == WN.at(woff + (uint64_t)(i - 1)));
+                        --i; --j;
+                    } else if (f & 2u) st = 1;
+                    else st = 2;
+                } else if (st == 1) {
+                    emit(2, 1u); ++n_cols;
+                    if (f & 4u) st = 0;
+                    --i;
+                } else {
+                    emit(1, 1u); ++n_cols;
+                    if (f & 8u) st = 0;
+                    --j;
+                }
+            }
+            ref_start = i;
+        }
+    }
+    emit(-2, 0u);                                          // flush the last run
+    if (bad) { atomicOr(tp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
+    tp.ref_start[p] = ref_start;
+    tp.read_start[p] = 0;
+    tp.read_end[p] = n - 1;
+    tp.n_match[p] = n_match;
+    tp.n_cols[p] = n_cols;
+    tp.cigar_len[p] = nops;
+    tp.pass[p] = ((long long)n_match * 1000000LL >= tp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
+}
+
+void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st)
+{
+    if (tp.count == 0) return;
+    const uint32_t grid = (tp.count + 127) / 128;
+    switch (cls) {
+        case 0: k_traceback<16><<<grid, 128, 0, st>>>(tp); break;
+        case 1: k_traceback<64><<<grid, 128, 0, st>>>(tp); break;
+        case 2: k_traceback<256><<<grid, 128, 0, st>>>(tp); break;
+        default: k_traceback<1032><<<grid, 128, 0, st>>>(tp); break;
+    }
+}
+
+// a7: copy each pair's runs (stored end -> start) into the dense buffer in alignment order
+__global__ void k_compact(uint64_t n_pairs, const uint64_t* __restrict__ ops_off, const uint32_t* __restrict__ ops_rev,
+                          const uint32_t* __restrict__ cigar_len, const uint64_t* __restrict__ cigar_off,
+                          uint32_t* __restrict__ cigar_ops)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pairs) return;
+    const uint32_t len = cigar_len[p];
+    const uint32_t* src = ops_rev + ops_off[p];
+    uint32_t* dst = cigar_ops + cigar_off[p];
+    for (uint32_t k = 0; k < len; ++k) dst[k] = src[len - 1 - k];
+}
+
+void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
+                    const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st)
+{
+    if (n_pairs) k_compact<<<(uint32_t)((n_pairs + 255) / 256), 256, 0, st>>>(n_pairs, ops_off, ops_rev, cigar_len,
+                                                                             cigar_off, cigar_ops);
+}
+
+}  // namespace sdp

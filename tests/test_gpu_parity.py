@@ -1,0 +1,228 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle,
+element by element on the same seeded inputs. Sizes span several tiles and ragged tails."""
+import random
+
+import numpy as np
+import pytest
+
+from oracle import OracleScoring
+from paper_1302_5507_b200 import Context, SdpError, workloads as W
+
+import parity
+
+pytestmark = pytest.mark.gpu
+DEFAULT = OracleScoring(1, -3, 5, 2, 0.6)
+
+
+def make_ctx(sc: OracleScoring):
+    return Context(sc.match, sc.mismatch, sc.gap_open, sc.gap_extend, sc.min_similarity, device=0)
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = make_ctx(DEFAULT)
+    yield c
+    c.destroy()
+
+
+def load_golden():
+    import os
+    rows = []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "worked_examples.txt")):
+        f = line.split()
+        if f and not f[0].startswith("#") and f[0] != "E1_LAST_ROW":
+            rows.append(f)
+    return rows
+
+
+def test_worked_examples(ctx):
+    rows = load_golden()
+    b = W.batch_from_strings([r[1] for r in rows], [r[2] for r in rows])
+    exp, got = parity.check_batch(ctx, b, DEFAULT, "worked examples")
+    for k, r in enumerate(rows):
+        assert (got.score[k], got.ref_start[k], got.ref_end[k], got.cigar(k)) == (int(r[3]), int(r[4]), int(r[5]), r[6])
+
+
+@pytest.mark.parametrize("cfg,n_pairs", [(1, 1000), (2, 3000), (3, 2500), (4, 1500), (5, 6000)])
+def test_configs_small(ctx, cfg, n_pairs):
+    # config 1 at its full size; the others shrunk so the oracle finishes in seconds
+    b = W.make_config(cfg, n_pairs=n_pairs, ref_bases=2_000_000)
+    parity.check_batch(ctx, b, DEFAULT, f"cfg{cfg}")
+
+
+def test_ragged_counts(ctx):
+    # pair counts around the warp-task sizes (16 pairs per warp at n=100, 4 warps per CTA)
+    full = W.make_config(2, n_pairs=200, ref_bases=500_000)
+    for cnt in (1, 2, 3, 15, 16, 17, 31, 33, 63, 64, 65, 129):
+        parity.check_batch(ctx, full.subset(np.arange(cnt)), DEFAULT, f"count={cnt}", host_path=False)
+
+
+def test_empty_batch(ctx):
+    full = W.make_config(1, n_pairs=4, ref_bases=100_000)
+    b = full.subset(np.arange(0))
+    got = ctx.fetch(ctx.align_batch(ctx.upload(b)))
+    assert got.score.shape == (0,) and got.cigar_ops.shape == (0,)
+    got = ctx.align_batch_host(b)
+    assert got.score.shape == (0,)
+
+
+def test_shuffled_and_repeated_pairs(ctx):
+    # many windows per read and a permuted pair list: results must follow caller order
+    b = W.make_config(5, n_pairs=400, ref_bases=500_000)
+    rng = np.random.default_rng(5)
+    ri = rng.integers(0, 400, size=1500).astype(np.uint32)
+    wi = rng.integers(0, 400, size=1500).astype(np.uint32)
+    b2 = W.Batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len,
+                 np.stack([ri, wi], axis=1), b.read_nmask, b.win_nmask, "shuffled")
+    parity.check_batch(ctx, b2, DEFAULT, "shuffled pairs")
+
+
+def test_every_read_length(ctx):
+    # every n in 1..330 (all column counts K, all group sizes G, ragged last columns) against
+    # windows of assorted lengths, including windows shorter than the read
+    rng = random.Random(11)
+    reads, wins = [], []
+    for n in range(1, 331):
+        m = rng.choice([1, 2, 3, n, n + 1, n // 2 + 1, n + 37, 2 * n + 5, 400])
+        T = "".join(rng.choice("ACGT") for _ in range(m))
+        if m > n and rng.random() < 0.7:
+            s = rng.randint(0, m - n)
+            R = list(T[s:s + n])
+            for _ in range(rng.randint(0, 3)):
+                R[rng.randrange(n)] = rng.choice("ACGT")
+            R = "".join(R)
+            if n > 20 and rng.random() < 0.5:
+                k = rng.randint(5, n - 5)
+                R = (R[:k] + R[k + 2:] + "AC") if rng.random() < 0.5 else (R[:k] + "GT" + R[k:n - 2])
+        else:
+            R = "".join(rng.choice("ACGT") for _ in range(n))
+        reads.append(R)
+        wins.append(T)
+    b = W.batch_from_strings(wins, reads)
+    parity.check_batch(ctx, b, DEFAULT, "every read length")
+
+
+def test_long_reads(ctx):
+    rng = random.Random(12)
+    reads, wins = [], []
+    for n in (331, 400, 512, 700, 999, 1000, 1023, 1024):
+        for rep in range(3):
+            m = n + rng.randint(0, 600)
+            T = "".join(rng.choice("ACGT") for _ in range(m))
+            s = rng.randint(0, m - n)
+            R = list(T[s:s + n])
+            for _ in range(n // 50):
+                R[rng.randrange(n)] = rng.choice("ACGT")
+            k = rng.randint(50, n - 50)
+            R = "".join(R)
+            R = R[:k] + R[k + 3:] + "ACG" if rep else R
+            reads.append(R)
+            wins.append(T)
+    b = W.batch_from_strings(wins, reads)
+    parity.check_batch(ctx, b, DEFAULT, "long reads")
+
+
+def test_n_bases_both_sides(ctx):
+    rng = random.Random(13)
+    reads, wins = [], []
+    for _ in range(300):
+        n, m = rng.randint(20, 120), rng.randint(60, 300)
+        T = [rng.choice("ACGT") for _ in range(m)]
+        for _ in range(rng.randint(0, 3)):
+            a = rng.randrange(m)
+            for k in range(a, min(m, a + rng.randint(1, 30))):
+                T[k] = "N"
+        s = rng.randint(0, max(0, m - n))
+        R = (T[s:s + n] + [rng.choice("ACGT") for _ in range(n)])[:n]
+        R = [c if c != "N" or rng.random() < 0.5 else rng.choice("ACGT") for c in R]
+        for _ in range(rng.randint(0, 2)):
+            R[rng.randrange(n)] = "N"
+        reads.append("".join(R))
+        wins.append("".join(T))
+    wins.append("N" * 40)
+    reads.append("ACGTACGTAC")          # all-N window: all-insertion alignment, span 0
+    b = W.batch_from_strings(wins, reads)
+    assert b.read_nmask is not None and b.win_nmask is not None
+    parity.check_batch(ctx, b, DEFAULT, "N bases")
+
+
+def test_tie_heavy_low_complexity(ctx):
+    rng = random.Random(14)
+    reads, wins = [], []
+    for _ in range(600):
+        alpha = rng.choice(["A", "AC", "AC", "ACG"])
+        n, m = rng.randint(1, 40), rng.randint(1, 90)
+        wins.append("".join(rng.choice(alpha) for _ in range(m)))
+        reads.append("".join(rng.choice(alpha) for _ in range(n)))
+    b = W.batch_from_strings(wins, reads)
+    parity.check_batch(ctx, b, DEFAULT, "low complexity")
+
+
+@pytest.mark.parametrize("sc", [OracleScoring(2, -1, 1, 1, 0.5), OracleScoring(1, -1, 2, 1, 0.7),
+                                OracleScoring(3, -2, 4, 3, 0.6), OracleScoring(1, -4, 6, 1, 0.9),
+                                OracleScoring(1, -9, 1, 1, 0.6), OracleScoring(0, -1, 0, 1, 0.0),
+                                OracleScoring(5, -4, 0, 1, 0.6), OracleScoring(1, 0, 3, 2, 0.6)],
+                         ids=lambda s: f"{s.match}_{s.mismatch}_{s.gap_open}_{s.gap_extend}")
+def test_other_scorings(sc):
+    c = make_ctx(sc)
+    try:
+        b = W.make_config(4, n_pairs=300, ref_bases=300_000)
+        parity.check_batch(c, b, sc, f"scoring {sc}", host_path=False)
+        rng = random.Random(15)
+        wins = ["".join(rng.choice("AC") for _ in range(rng.randint(1, 60))) for _ in range(300)]
+        reads = ["".join(rng.choice("AC") for _ in range(rng.randint(1, 30))) for _ in range(300)]
+        parity.check_batch(c, W.batch_from_strings(wins, reads), sc, f"scoring {sc} ties", host_path=False)
+    finally:
+        c.destroy()
+
+
+def test_mixed_window_lengths_in_one_warp(ctx):
+    # same read length, window lengths from 1 to 900 in one batch: lanes of a warp finish at
+    # different rows (the masked tail loop of the score kernel)
+    rng = random.Random(16)
+    T0 = "".join(rng.choice("ACGT") for _ in range(2000))
+    reads, wins = [], []
+    for k in range(400):
+        m = rng.choice([1, 5, 50, 99, 100, 101, 130, 250, 500, 899, 900])
+        s = rng.randint(0, 2000 - m)
+        wins.append(T0[s:s + m])
+        a = rng.randint(0, 1900)
+        reads.append(T0[a:a + 100])
+    parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "mixed m")
+
+
+def test_errors(ctx):
+    b = W.make_config(1, n_pairs=10, ref_bases=100_000)
+    bad = W.Batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len,
+                  np.array([[0, 99]], dtype=np.uint32), None, None)
+    with pytest.raises(SdpError) as e:
+        ctx.align_batch(ctx.upload(bad))
+    assert e.value.code == -1
+    # int16 range rule: 1*100 + 2*(100 + 9000) > 16000
+    long_win = "ACGT" * 2250
+    rb = W.batch_from_strings([long_win], ["ACGT" * 25])
+    with pytest.raises(SdpError) as e:
+        ctx.align_batch(ctx.upload(rb))
+    assert e.value.code == -2
+    # read longer than SDP_MAX_READ_LEN
+    rb = W.batch_from_strings(["ACGT" * 300], ["ACGT" * 257])
+    with pytest.raises(SdpError) as e:
+        ctx.align_batch(ctx.upload(rb))
+    assert e.value.code == -2
+    with pytest.raises(SdpError):
+        Context(match=1, mismatch=1)
+    with pytest.raises(SdpError):
+        Context(gap_extend=0)
+    # the context survives errors
+    parity.check_batch(ctx, b, DEFAULT, "after errors", host_path=False)
+
+
+def test_stats_and_timing(ctx):
+    b = W.make_config(2, n_pairs=500, ref_bases=500_000)
+    ctx.set_timing(True)
+    ctx.align_batch(ctx.upload(b))
+    s = ctx.stats()
+    ctx.set_timing(False)
+    assert s["n_pairs"] == 500 and s["cells_forward"] == b.cells
+    assert s["kernel_launches"] >= 8 and s["forward_launches"] >= 1
+    assert s["ms_total"] > 0 and s["ms_forward"] > 0
