@@ -2,7 +2,7 @@
 
 ``python -m paper_1302_5507_b200.build`` or ``build()`` from ``__graft_entry__``. Objects are
 compiled in parallel; the score kernel is instantiated for 32 column counts x {forward,
-reverse}, split over eight translation units by ``-DSDP_K_LO/-DSDP_K_HI``.
+reverse} x {exact, padded}, split over sixteen translation units by ``-DSDP_K_LO/-DSDP_K_HI``.
 """
 from __future__ import annotations
 
@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libsdp.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
-K_RANGES = [(4 * r + 1, 4 * r + 4) for r in range(8)]
+K_RANGES = [(2 * r + 1, 2 * r + 2) for r in range(16)]
 
 
 def _nvcc() -> str:

@@ -14,22 +14,37 @@
 //    s - g at step s (anti-diagonal wavefront); H and E of the chunk's last column cross to the
 //    right neighbour with one warp shuffle each per row.
 //  * drift form: stored values are H + e*(i+j) + beta, so gap extension needs no add:
-//        E' = max(H'(i,j-1) - o, E'(i,j-1))          1 VIADDMNMX.S16x2
-//        F' = max(H'(i-1,j) - o, F'(i-1,j))          1 VIADDMNMX.S16x2
-//        t  = max(H'(i-1,j-1) + (2e+mismatch), E')   1 VIADDMNMX.S16x2
-//        H' = max3(H'(i-1,j-1) + q, t, F')           1 VIMNMX3.S16x2
+//        E' = max(H'(i,j-1) - o, E'(i,j-1))          1 VIADDMNMX.S16x2   (on the row's serial chain)
+//        F' = max(H'(i-1,j) - o, F'(i-1,j))          1 VIADDMNMX.S16x2   (off the chain)
+//        t  = max(H'(i-1,j-1) + (2e+mismatch), F')   1 VIADDMNMX.S16x2   (off the chain)
+//        H' = max3(H'(i-1,j-1) + q, t, E')           1 VIMNMX3.S16x2     (on the chain)
 //    where q = (2e+match) when the bases are equal and a large negative number otherwise. q comes
-//    from the otherwise idle FMA pipe: base codes are fp16 values (1 + c/4), d = r - t (HADD2),
+//    from the otherwise idle FMA pipe: base codes are fp16 values, d = r - t (HADD2),
 //    q = fma(d, -d, C) (HFMA2) with C the fp16 DENORMAL whose bit pattern is the integer 2e+match;
 //    d == 0 gives exactly C, d != 0 gives a negative half whose bit pattern read as int16 is below
-//    -12000. The add H' + q is a 32-bit IMAD (no carry crosses the lanes because every stored
+//    -15000. The add H' + q is a 32-bit IMAD (no carry crosses the lanes because every stored
 //    value is in [0, 16000]). Four ALU-pipe instructions per two cells.
-//  * reads whose length is not G*K: the first G*K-n threads treat their last column as absent
-//    (pass the previous column's H/E through), per int16 lane.
+//  * window rows: the 2-bit window bases of both lanes are expanded once per chunk of rows into
+//    a per-group shared-memory ring of 16-bit PRMT selectors; a row then costs one LDS.U16 and one
+//    PRMT to obtain the fp16 codes of both lanes (instead of two address computations, two global
+//    loads and the bit extraction per row and thread).
+//  * reads whose length is not G*K (PAD variant): the first G*K-n threads treat their last column
+//    as absent (pass the previous column's H/E through), per int16 lane.
 #pragma once
 #include "sdp_internal.cuh"
 
 namespace sdp {
+
+// fp16 code bytes: value byte T[c] for c = A,C,G,T, read-N (4), window-N (5). A base code is the
+// half whose two bytes are (T[c]^0x80, T[c]) on the read side and (T[c], T[c]) on the window side,
+// i.e. exact negatives of each other; all six magnitudes differ by >= 0.125 and are <= 1.94.
+#define SDP_TBL_LO 0xBFBEBDBCu      // PRMT source a: bytes 0..3 = A C G T
+#define SDP_TBL_HI 0x0000BBBAu      // PRMT source b: byte 4 = read N, byte 5 = window N
+
+__device__ __forceinline__ uint32_t read_code_half(uint32_t c) {      // c in 0..4
+    const uint32_t t = (c < 4u) ? (0xBCu + c) : 0xBAu;
+    return ((t ^ 0x80u) << 8) | t;
+}
 
 __device__ __forceinline__ uint32_t hadd2_u(uint32_t a, uint32_t b) {
     uint32_t d; asm("add.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d;
@@ -65,7 +80,7 @@ __device__ __forceinline__ uint32_t blend(uint32_t mask, uint32_t a, uint32_t b)
     return (a & mask) | (b & ~mask);
 }
 
-// base `idx` (signed, relative to word pointer `base`) of a 2-bit packed buffer, N-mask aware
+// base at position `pos` of a 2-bit packed buffer, N-mask aware
 __device__ __forceinline__ uint32_t fetch_code(const uint32_t* __restrict__ packed,
                                                const uint32_t* __restrict__ nmask,
                                                uint64_t pos, uint32_t ncode) {
@@ -78,10 +93,60 @@ __device__ __forceinline__ uint32_t fetch_code(const uint32_t* __restrict__ pack
     return c;
 }
 
-template <int K, bool REV>
-__global__ void __launch_bounds__(SDP_SCORE_THREADS)
+// 16 consecutive bases starting at base position `pos` (may lie partly outside [0, 16*nwords));
+// words outside the buffer read as 0
+__device__ __forceinline__ uint32_t load_bases16(const uint32_t* __restrict__ packed, long long pos, long long nwords) {
+    const long long w = pos >> 4;
+    const uint32_t sh = ((uint32_t)pos & 15u) * 2u;
+    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(packed + w) : 0u;
+    const uint32_t hi = (sh != 0u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(packed + w + 1) : 0u;
+    return __funnelshift_r(lo, hi, sh);
+}
+// 16 consecutive mask bits starting at bit position `pos`
+__device__ __forceinline__ uint32_t load_bits16(const uint32_t* __restrict__ bits, long long pos, long long nwords) {
+    const long long w = pos >> 5;
+    const uint32_t sh = (uint32_t)pos & 31u;
+    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(bits + w) : 0u;
+    const uint32_t hi = (sh > 16u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(bits + w + 1) : 0u;
+    return __funnelshift_r(lo, hi, sh) & 0xFFFFu;
+}
+// reverse the order of the sixteen 2-bit fields / of the low sixteen bits
+__device__ __forceinline__ uint32_t reverse_fields2(uint32_t x) {
+    x = __brev(x);
+    return ((x & 0x55555555u) << 1) | ((x >> 1) & 0x55555555u);
+}
+__device__ __forceinline__ uint32_t reverse_bits16(uint32_t x) { return __brev(x) >> 16; }
+
+// Shared-memory ring of window-row selectors: per warp SDP_RING_WORDS 32-bit words, carved into one
+// region per group. A region holds `ring` 16-bit entries (row i at slot (i-1) & (ring-1), stored at
+// position slot + 32) plus a 32-entry mirror of the ring's tail in front of it, so that thread g
+// can read row s-g at position ((s-1) & (ring-1)) + 32 - g without a wrap test.
+struct RingGeom {
+    int chunk, ring, stride_w;
+};
+__device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups) {
+    RingGeom r;
+    if (G == 1)      { r.chunk = 32; r.stride_w = 49; }
+    else if (G == 2) { r.chunk = 32; r.stride_w = 50; }
+    else {
+        r.chunk = 128;
+        const int want = (32 / ngroups) & 31;             // bank offset between neighbouring groups
+        r.stride_w = 144 + ((want - 144) & 31);           // >= (256 + 32) / 2 words, == want (mod 32)
+    }
+    r.ring = 2 * r.chunk;
+    return r;
+}
+
+// resident CTAs per SM the register budget is sized for: 128 registers up to K = 21, 168 above
+#ifndef SDP_SCORE_MIN_CTAS
+#define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)
+#endif
+
+template <int K, bool REV, bool PAD>
+__global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))
 score_kernel(const ScoreParams P)
 {
+    __shared__ uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];
     const int lane = threadIdx.x & 31;
     const uint32_t task = P.task_begin + blockIdx.x * SDP_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (task >= P.task_end) return;                       // warp-uniform
@@ -103,12 +168,12 @@ score_kernel(const ScoreParams P)
     int q = lane / G;
     int g = lane - q * G;
     const bool in_group = q < ngroups;
-    if (!in_group) { q = 0; g = (G > 2) ? 1 : 0; }        // spare lanes shadow group 0, write nothing
+    if (!in_group) { q = 0; g = 1; }                      // spare lanes (G >= 3) shadow group 0, write nothing
     const bool hasA = in_group && (2 * q < cnt);
     const bool hasB = in_group && (2 * q + 1 < cnt);
     const PairDesc dA = P.desc[first + (hasA ? 2 * q : 0)];
     const PairDesc dB = hasB ? P.desc[first + 2 * q + 1] : dA;
-    const bool is_first = (g == 0);
+    const bool is_first = in_group && (g == 0);
     const bool is_last = in_group && (g == G - 1);
 
     const int nA = (int)dA.n, nB = (int)dB.n;
@@ -117,7 +182,7 @@ score_kernel(const ScoreParams P)
     const int Mmax = __reduce_max_sync(0xffffffffu, max(mA, mB));
 
     // ---- columns of this thread: the first pad = G*K - n threads skip their last column
-    const int padA = G * K - nA, padB = G * K - nB;
+    const int padA = PAD ? G * K - nA : 0, padB = PAD ? G * K - nB : 0;
     const bool skipA = g < padA, skipB = g < padB;
     const int startA = g * K - min(g, padA), startB = g * K - min(g, padB);
     const int realA = K - (skipA ? 1 : 0), realB = K - (skipB ? 1 : 0);
@@ -136,58 +201,116 @@ score_kernel(const ScoreParams P)
             int r = startB + k;
             cB = fetch_code(P.reads_packed, P.read_nmask, dB.roff + (uint64_t)(REV ? nB - 1 - r : r), SDP_CODE_READ_N);
         }
-        rh[k] = (0x3C00u + (cA << 8)) | ((0x3C00u + (cB << 8)) << 16);
+        rh[k] = read_code_half(cA) | (read_code_half(cB) << 16);
         H[k] = h_row0;
         F[k] = 0u;                                        // F'(0,j) = -inf: 0 <= beta - 2o
     }
 
-    const uint32_t one = P.c.one, negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf;
+    // ---- window-row selector ring of this group
+    const RingGeom rg = ring_geometry(G, ngroups);
+    uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
+    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
+    const long long win_words = (long long)P.wins_words, nm_words = (long long)P.win_nmask_words;
+
+    auto fill_ring = [&](const int s0) {                  // rows s0+1 .. s0+chunk
+        if (!in_group) return;
+        for (int u = g; u < rg.chunk / 16; u += G) {
+            const int r0 = s0 + 16 * u;                   // 0-based row of the unit's first entry
+            uint32_t a = 0u, b = 0u, na = 0u, nb = 0u;
+            if (r0 < mA) {
+                a = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)dA.woff - r0 - 15, win_words))
+                        : load_bases16(P.wins_packed, (long long)dA.woff + r0, win_words);
+                if (P.win_nmask != nullptr)
+                    na = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)dA.woff - r0 - 15, nm_words))
+                             : load_bits16(P.win_nmask, (long long)dA.woff + r0, nm_words);
+            }
+            if (r0 < mB) {
+                b = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)dB.woff - r0 - 15, win_words))
+                        : load_bases16(P.wins_packed, (long long)dB.woff + r0, win_words);
+                if (P.win_nmask != nullptr)
+                    nb = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)dB.woff - r0 - 15, nm_words))
+                             : load_bits16(P.win_nmask, (long long)dB.woff + r0, nm_words);
+            }
+            const int slot0 = r0 & (rg.ring - 1);
+            uint32_t* dst = ring_w + 16 + (slot0 >> 1);
+            uint32_t* mir = (slot0 >= rg.ring - 32) ? ring_w + ((slot0 - (rg.ring - 32)) >> 1) : nullptr;
+#pragma unroll
+            for (int tt = 0; tt < 8; ++tt) {
+                // two rows -> two 16-bit selectors (idxA * 0x11 | idxB * 0x1100)
+                const uint32_t x = (a >> (4 * tt)) & 0xFu, y = (b >> (4 * tt)) & 0xFu;
+                uint32_t w = ((x * 0x44011u) & 0x00330033u) | (((y * 0x44011u) << 8) & 0x33003300u);
+                if (na | nb) {                            // window N -> table index 5
+                    const uint32_t ma = (na >> (2 * tt)) & 3u, mb = (nb >> (2 * tt)) & 3u;
+                    if (ma & 1u) w = (w & 0xFFFFFF00u) | 0x00000055u;
+                    if (ma & 2u) w = (w & 0xFF00FFFFu) | 0x00550000u;
+                    if (mb & 1u) w = (w & 0xFFFF00FFu) | 0x00005500u;
+                    if (mb & 2u) w = (w & 0x00FFFFFFu) | 0x55000000u;
+                }
+                dst[tt] = w;
+                if (mir != nullptr) mir[tt] = w;
+            }
+        }
+    };
+
+    const uint32_t one = P.c.one, negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, e2 = P.c.e2;
+    const uint32_t notfirst = is_first ? 0u : 0xFFFFFFFFu;
+    // boundary column 0 as seen by the group's first thread: H'(i,0) = beta + e*i (forward, free
+    // start) or beta - o (reverse, start anchored: a leading deletion of i bases costs o + e*i)
+    uint32_t fv = is_first ? (REV ? P.c.betaMinusO2 : P.c.beta2) : 0u;
+    const uint32_t fstep = (is_first && !REV) ? e2 : 0u;
     uint32_t hout = h_row0, eout = 0u;
     uint32_t hdiag = is_first ? P.c.beta2 : h_row0;       // H'(0, left boundary column)
-    uint32_t drift = 0u;                                  // packed e*i of the row this thread is on
-    uint32_t best = REV ? h_row0 : 0x80008000u;           // reverse: row 0 (all-insertion) counts
+    // running maximum of H(i,n) in the drift frame of the current row: best += e per row, so that
+    // H'(i,n) can be compared with it directly. Reverse: row 0 (all-insertion) counts.
+    uint32_t best = REV ? h_row0 : 0x80008000u;
     int idxA = 0, idxB = 0;
 
-    auto row_step = [&](const int i, auto slow_tag) {
+    // One DP row of this thread's K columns. Hs = H'(i-1, .) is only read, Hn receives H'(i, .):
+    // two register sets that swap roles from row to row, so that no H' value is ever copied (the
+    // diagonal term of column k is accumulated in Hn[k] before the serial chain reaches it).
+    auto row_step = [&](const int i, const uint16_t* rp, auto slow_tag, const uint32_t (&Hs)[K], uint32_t (&Hn)[K]) {
         constexpr bool SLOW = decltype(slow_tag)::value;
         uint32_t hin = __shfl_up_sync(0xffffffffu, hout, 1);
         uint32_t ein = __shfl_up_sync(0xffffffffu, eout, 1);
-        if (SLOW && i < 1) return;                        // this thread has not reached row 1 yet
-        drift = __vadd2(drift, P.c.e2);
-        if (is_first) {
-            hin = REV ? P.c.betaMinusO2 : __vadd2(P.c.beta2, drift);
-            ein = 0u;
+        if (SLOW && i < 1) {                              // this thread has not reached row 1 yet
+#pragma unroll
+            for (int k = 0; k < K; ++k) Hn[k] = Hs[k];
+            return;
         }
-        // window bases of row i for both lanes -> negated fp16 codes
-        const int iA = min(i, mA), iB = min(i, mB);
-        const uint32_t tA = fetch_code(P.wins_packed, P.win_nmask,
-                                       REV ? dA.woff - (uint64_t)(iA - 1) : dA.woff + (uint64_t)(iA - 1), SDP_CODE_WIN_N);
-        const uint32_t tB = fetch_code(P.wins_packed, P.win_nmask,
-                                       REV ? dB.woff - (uint64_t)(iB - 1) : dB.woff + (uint64_t)(iB - 1), SDP_CODE_WIN_N);
-        const uint32_t nt = (0xBC00u + (tA << 8)) | ((0xBC00u + (tB << 8)) << 16);
+        fv = __vadd2(fv, fstep);
+        hin = (hin & notfirst) | fv;
+        ein = ein & notfirst;
+        // negated fp16 codes of the window bases of row i, both lanes
+        const uint32_t nt = __byte_perm(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
 
-        uint32_t Hd = hdiag, Hl = hin, E = ein;
+        uint32_t Hl = hin, E = ein;
         uint32_t Hsk = hin, Esk = ein;                    // outputs if the last column is skipped
+        uint32_t t1;
+        Hn[0] = imad_add(one, hdiag, hfma2_negsq(hadd2_u(rh[0], nt), Cf));
+        F[0] = __viaddmax_s16x2(Hs[0], negO, F[0]);
+        t1 = __viaddmax_s16x2(hdiag, cmis, F[0]);
         hdiag = hin;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const uint32_t d = hadd2_u(rh[k], nt);
-            const uint32_t qv = hfma2_negsq(d, Cf);
-            const uint32_t dg = imad_add(one, Hd, qv);
+            uint32_t t1_n = 0u;
+            if (k + 1 < K) {                              // off-chain work of column k+1
+                Hn[k + 1] = imad_add(one, Hs[k], hfma2_negsq(hadd2_u(rh[k + 1], nt), Cf));
+                F[k + 1] = __viaddmax_s16x2(Hs[k + 1], negO, F[k + 1]);
+                t1_n = __viaddmax_s16x2(Hs[k], cmis, F[k + 1]);
+            }
             E = __viaddmax_s16x2(Hl, negO, E);
-            F[k] = __viaddmax_s16x2(H[k], negO, F[k]);
-            const uint32_t t1 = __viaddmax_s16x2(Hd, cmis, E);
-            const uint32_t Hn = __vimax3_s16x2(dg, t1, F[k]);
-            Hd = H[k]; H[k] = Hn; Hl = Hn;
-            if (k == K - 2) { Hsk = Hn; Esk = E; }
+            Hl = __vimax3_s16x2(Hn[k], t1, E);
+            Hn[k] = Hl;
+            t1 = t1_n;
+            if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }
-        hout = blend(skipmask, Hsk, Hl);
-        eout = blend(skipmask, Esk, E);
+        if (PAD) { hout = blend(skipmask, Hsk, Hl); eout = blend(skipmask, Esk, E); }
+        else     { hout = Hl; eout = E; }
 
         if (is_last) {
-            // running maximum of H(i,n) = H'(i,n) - e*i - (beta + e*n); strict > keeps the lowest
-            // row (forward), >= keeps the highest (reverse)
-            uint32_t cmp = __vsub2(Hl, drift);
+            // strict > keeps the lowest row (forward), >= keeps the highest (reverse)
+            best = __vadd2(best, e2);
+            uint32_t cmp = Hl;
             if (SLOW) {
                 const uint32_t ok = (i <= mA ? 0x0000FFFFu : 0u) | (i <= mB ? 0xFFFF0000u : 0u);
                 cmp = blend(ok, cmp, 0x80008000u);
@@ -204,17 +327,41 @@ score_kernel(const ScoreParams P)
             }
         }
     };
+    auto row_step1 = [&](const int i, const uint16_t* rp, auto slow_tag) {
+        uint32_t H2[K];
+        row_step(i, rp, slow_tag, H, H2);
+#pragma unroll
+        for (int k = 0; k < K; ++k) H[k] = H2[k];
+    };
 
-    int s = 1;
-    for (; s < G; ++s) row_step(s - g, std::true_type{});                   // fill: some threads idle
-    const int fast_end = Mmin + G - 1;
-    for (; s <= fast_end; ++s) row_step(s - g, std::false_type{});          // steady state
-    const int all_end = Mmax + G - 1;
-    for (; s <= all_end; ++s) row_step(s - g, std::true_type{});            // lanes with fewer rows done
+    // step s: thread g works on row s - g. Steps 1..G-1 fill the wavefront, steps up to
+    // Mmin+G-1 are the steady state (two rows per iteration), the rest drain lanes whose
+    // window is longer.
+    const int fast_end = Mmin + G - 1, all_end = Mmax + G - 1;
+    for (int s0 = 0; s0 < all_end; s0 += rg.chunk) {
+        fill_ring(s0);
+        __syncwarp();
+        const int send = min(s0 + rg.chunk, all_end);
+        const uint16_t* rp = rp0 + (s0 & (rg.ring - 1));
+        int s = s0 + 1;
+#pragma unroll 1
+        for (; s <= min(send, G - 1); ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+        const int fe = min(send, fast_end);
+#pragma unroll 1
+        for (; s + 1 <= fe; s += 2, rp += 2) {
+            uint32_t H2[K];
+            row_step(s - g, rp, std::false_type{}, H, H2);
+            row_step(s + 1 - g, rp + 1, std::false_type{}, H2, H);
+        }
+        if (s <= fe) { row_step1(s - g, rp, std::false_type{}); ++s; ++rp; }
+#pragma unroll 1
+        for (; s <= send; ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+    }
 
     if (is_last) {
+        // best = H'(idx,n) + e*(Mmax - idx) = H(idx,n) + e*(n + Mmax) + beta
         const int bA = (int)(int16_t)(best & 0xFFFFu), bB = (int)(int16_t)(best >> 16);
-        const int sA = bA - P.c.beta - P.c.e * nA, sB = bB - P.c.beta - P.c.e * nB;
+        const int sA = bA - P.c.beta - P.c.e * (nA + Mmax), sB = bB - P.c.beta - P.c.e * (nB + Mmax);
         if (REV) {
             // idx = rows of the reversed window consumed by the longest alignment scoring S;
             // the lowest co-optimal start is s_lo = ref_end + 1 - idx
@@ -228,12 +375,17 @@ score_kernel(const ScoreParams P)
 }
 
 template <int K>
-static void launch_score_K(bool rev, const ScoreParams& p, cudaStream_t st) {
+static void launch_score_K(bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
     const uint32_t ntasks = p.task_end - p.task_begin;
     if (ntasks == 0) return;
     const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
-    if (rev) score_kernel<K, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-    else     score_kernel<K, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+    if (rev) {
+        if (pad) score_kernel<K, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        else     score_kernel<K, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+    } else {
+        if (pad) score_kernel<K, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        else     score_kernel<K, false, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+    }
 }
 
 }  // namespace sdp

@@ -18,18 +18,14 @@
 using namespace sdp;
 
 namespace sdp {
-bool launch_score_r0(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r1(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r2(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r3(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r4(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r5(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r6(int, bool, const ScoreParams&, cudaStream_t);
-bool launch_score_r7(int, bool, const ScoreParams&, cudaStream_t);
-void launch_score(int K, bool rev, const ScoreParams& p, cudaStream_t st) {
-    (void)(launch_score_r0(K, rev, p, st) || launch_score_r1(K, rev, p, st) || launch_score_r2(K, rev, p, st) ||
-           launch_score_r3(K, rev, p, st) || launch_score_r4(K, rev, p, st) || launch_score_r5(K, rev, p, st) ||
-           launch_score_r6(K, rev, p, st) || launch_score_r7(K, rev, p, st));
+#define SDP_SCORE_UNITS(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15)
+#define SDP_DECL(r) bool launch_score_r##r(int, bool, bool, const ScoreParams&, cudaStream_t);
+SDP_SCORE_UNITS(SDP_DECL)
+#undef SDP_DECL
+void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
+#define SDP_TRY(r) if (launch_score_r##r(K, pad, rev, p, st)) return;
+    SDP_SCORE_UNITS(SDP_TRY)
+#undef SDP_TRY
 }
 }  // namespace sdp
 
@@ -62,7 +58,7 @@ struct sdp_ctx {
     bool timing = false;
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
-    uint32_t kslot_begin[SDP_MAX_K + 2];
+    uint32_t cls_begin[2 * SDP_MAX_K + 3];   // first slot of class c = 2K + padded; [c+1] ends it
     uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr;
     Mailbox* mb = nullptr;
     cudaStream_t own_stream = nullptr;
@@ -128,10 +124,12 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
         if (rc_ != SDP_OK) return rc_;                         \
     } while (0)
 
-// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model:
-// a warp runs 2*floor(32/G) pairs for (m + G - 1) steps of (7K + row overhead) issue slots.
+// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model
+// (DESIGN.md "Score kernel"): a warp runs 2*floor(32/G) pairs for (m + G - 1) steps; a step is
+// bound by the ALU pipe at 2 cycles per instruction: 4 per column, ~11 per row, 4 more when the
+// read length is not G*K (padded variant).
 void choose_geometry(sdp_ctx* c) {
-    struct Ent { uint16_t n, G, K; };
+    struct Ent { uint16_t n, G, K, pad; };
     Ent ents[SDP_NSLOTS];
     for (int n = 1; n <= SDP_NSLOTS; ++n) {
         double best = -1; int bG = 32, bK = (n + 31) / 32;
@@ -141,21 +139,23 @@ void choose_geometry(sdp_ctx* c) {
             if (G * K - n >= G) continue;
             double ppw = 2.0 * (32 / G);
             double rows = (double)n + 300.0 + G - 1;
-            double thr = ppw / (rows * (7.0 * K + 30.0));
+            double thr = ppw / (rows * (4.0 * K + 11.0 + (G * K != n ? 4.0 : 0.0)));
             if (thr > best) { best = thr; bG = G; bK = K; }
         }
-        ents[n - 1] = Ent{(uint16_t)n, (uint16_t)bG, (uint16_t)bK};
+        ents[n - 1] = Ent{(uint16_t)n, (uint16_t)bG, (uint16_t)bK, (uint16_t)(bG * bK != n ? 1 : 0)};
     }
-    std::stable_sort(ents, ents + SDP_NSLOTS, [](const Ent& a, const Ent& b) { return a.K < b.K; });
-    for (int K = 0; K <= SDP_MAX_K + 1; ++K) c->kslot_begin[K] = SDP_NSLOTS;
+    auto cls = [](const Ent& a) { return 2 * (int)a.K + (int)a.pad; };
+    std::stable_sort(ents, ents + SDP_NSLOTS, [&](const Ent& a, const Ent& b) { return cls(a) < cls(b); });
+    const int NC = 2 * SDP_MAX_K + 2;
+    for (int k = 0; k <= NC; ++k) c->cls_begin[k] = SDP_NSLOTS;
     for (int t = SDP_NSLOTS - 1; t >= 0; --t) {
         c->h_slot_n[t] = ents[t].n; c->h_slot_G[t] = ents[t].G; c->h_slot_K[t] = ents[t].K;
-        c->kslot_begin[ents[t].K] = (uint32_t)t;
+        c->cls_begin[cls(ents[t])] = (uint32_t)t;
     }
-    // K values that no read length uses start where the next used K starts
-    for (int K = SDP_MAX_K; K >= 0; --K)
-        if (c->kslot_begin[K] == SDP_NSLOTS) c->kslot_begin[K] = c->kslot_begin[K + 1];
-    c->kslot_begin[0] = 0;
+    // classes that no read length uses start where the next used class starts
+    for (int k = NC - 1; k >= 0; --k)
+        if (c->cls_begin[k] == SDP_NSLOTS) c->cls_begin[k] = c->cls_begin[k + 1];
+    c->cls_begin[0] = 0;
 }
 
 }  // namespace
@@ -273,19 +273,20 @@ static int launch_score_stage(sdp_ctx* ctx, int which, bool rev, const sdp_batch
     ScoreParams sp{};
     sp.reads_packed = b.reads_packed; sp.read_nmask = b.read_nmask;
     sp.wins_packed = b.wins_packed; sp.win_nmask = b.win_nmask;
+    sp.wins_words = (b.wins_bases + 15) / 16; sp.win_nmask_words = (b.wins_bases + 31) / 32;
     sp.desc = desc;
     sp.task_prefix = ctx->task_prefix[which];
     sp.slots = ctx->slots[which];
     sp.c = ctx->consts;
     sp.score = ctx->score.as<int32_t>(); sp.ref_end = ctx->ref_end.as<int32_t>();
     sp.rev_rows = ctx->rev_rows.as<int32_t>(); sp.err_flag = ctx->err_flag;
-    for (int K = 1; K <= SDP_MAX_K; ++K) {
-        const uint32_t s0 = ctx->kslot_begin[K], s1 = ctx->kslot_begin[K + 1];
+    for (int cls = 2; cls <= 2 * SDP_MAX_K + 1; ++cls) {
+        const uint32_t s0 = ctx->cls_begin[cls], s1 = ctx->cls_begin[cls + 1];
         if (s1 <= s0) continue;
         const uint32_t t0 = tp[s0], t1 = tp[s1];
         if (t1 <= t0) continue;
         sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
-        launch_score(K, rev, sp, st);
+        launch_score(cls >> 1, (cls & 1) != 0, rev, sp, st);
         ++*nlaunch;
     }
     CU(cudaGetLastError());

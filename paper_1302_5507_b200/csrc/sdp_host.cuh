@@ -24,7 +24,7 @@ void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint6
                             cudaStream_t st, uint32_t* launches);
 
 // ---- score_inst.cu (compiled once per K range)
-void launch_score(int K, bool rev, const ScoreParams& p, cudaStream_t st);
+void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t st);
 
 // ---- traceback.cu
 struct PostParams {

@@ -10,6 +10,7 @@
 #define SDP_MAX_K 32            // columns of the read one thread keeps in registers
 #define SDP_NBINS 65536         // bucket-sort key space: (n-1) * 64 + min(63, rows >> 6)
 #define SDP_NSLOTS 1024         // one slot per read length 1..SDP_MAX_READ_LEN
+#define SDP_RING_WORDS 1792     // shared-memory words per warp for the window-row selector rings
 #define SDP_KEY_SKIP 0xFFFFFFFFu
 
 // device-side error flag bits
@@ -56,10 +57,12 @@ struct ScoreConsts {
 struct ScoreParams {
     const uint32_t* reads_packed; const uint32_t* read_nmask;
     const uint32_t* wins_packed;  const uint32_t* win_nmask;
+    uint64_t wins_words;           // 32-bit words addressable in wins_packed / win_nmask (loads outside
+    uint64_t win_nmask_words;      // read as 0)
     const PairDesc* desc;
-    const uint32_t* task_prefix;   // [SDP_NSLOTS + 1], slots in K-major order
+    const uint32_t* task_prefix;   // [SDP_NSLOTS + 1], slots in (K, padded) order
     const SlotInfo* slots;         // [SDP_NSLOTS]
-    uint32_t slot_lo, slot_hi;     // slots of this launch's K
+    uint32_t slot_lo, slot_hi;     // slots of this launch's (K, padded) class
     uint32_t task_begin, task_end; // == task_prefix[slot_lo], task_prefix[slot_hi]
     ScoreConsts c;
     int32_t* score;                // forward outputs, caller order
@@ -69,7 +72,6 @@ struct ScoreParams {
     uint32_t* err_flag;            // reverse: SDP_ERRF_REVERSE when max != S
 };
 
-typedef void (*sdp_score_launch_fn)(int K, bool rev, const ScoreParams& p, cudaStream_t st);
 
 // packed helpers
 __host__ __device__ static inline uint32_t sdp_pack2(int v) {
