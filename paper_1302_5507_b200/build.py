@@ -1,8 +1,8 @@
 """Build libsdp.so (hand-written sm_100a kernels + C ABI) in-tree with nvcc.
 
 ``python -m paper_1302_5507_b200.build`` or ``build()`` from ``__graft_entry__``. Objects are
-compiled in parallel; the score kernel is instantiated for 32 column counts x {forward,
-reverse} x {exact, padded}, split over sixteen translation units by ``-DSDP_K_LO/-DSDP_K_HI``.
+compiled in parallel; the score and traceback-DP kernels are instantiated for 32 column counts x
+{forward, reverse, traceback} x {exact, padded}, split over sixteen translation units by ``-DSDP_K_LO/-DSDP_K_HI``.
 """
 from __future__ import annotations
 
@@ -46,7 +46,8 @@ def _units():
              ("microbench", "microbench.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"score_r{r}", "score_inst.cu",
-                      [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_K_FN=launch_score_r{r}"]))
+                      [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_K_FN=launch_score_r{r}",
+                       f"-DSDP_T_FN=launch_trace_r{r}"]))
     return units
 
 

@@ -137,6 +137,52 @@ __device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups) {
     return r;
 }
 
+
+// Expand window rows s0+1 .. s0+chunk of both int16 lanes into the group's selector ring (thread g
+// of G takes every G-th unit of 16 rows). REV walks the window backwards from woff.
+template <bool REV>
+__device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingGeom& rg, uint32_t* ring_w,
+                                               int g, int G, int s0, uint64_t woffA, int mA, uint64_t woffB, int mB)
+{
+    const long long win_words = (long long)P.wins_words, nm_words = (long long)P.win_nmask_words;
+    for (int u = g; u < rg.chunk / 16; u += G) {
+        const int r0 = s0 + 16 * u;                       // 0-based row of the unit's first entry
+        uint32_t a = 0u, b = 0u, na = 0u, nb = 0u;
+        if (r0 < mA) {
+            a = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)woffA - r0 - 15, win_words))
+                    : load_bases16(P.wins_packed, (long long)woffA + r0, win_words);
+            if (P.win_nmask != nullptr)
+                na = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)woffA - r0 - 15, nm_words))
+                         : load_bits16(P.win_nmask, (long long)woffA + r0, nm_words);
+        }
+        if (r0 < mB) {
+            b = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)woffB - r0 - 15, win_words))
+                    : load_bases16(P.wins_packed, (long long)woffB + r0, win_words);
+            if (P.win_nmask != nullptr)
+                nb = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)woffB - r0 - 15, nm_words))
+                         : load_bits16(P.win_nmask, (long long)woffB + r0, nm_words);
+        }
+        const int slot0 = r0 & (rg.ring - 1);
+        uint32_t* dst = ring_w + 16 + (slot0 >> 1);
+        uint32_t* mir = (slot0 >= rg.ring - 32) ? ring_w + ((slot0 - (rg.ring - 32)) >> 1) : nullptr;
+#pragma unroll
+        for (int tt = 0; tt < 8; ++tt) {
+            // two rows -> two 16-bit selectors (idxA * 0x11 | idxB * 0x1100)
+            const uint32_t x = (a >> (4 * tt)) & 0xFu, y = (b >> (4 * tt)) & 0xFu;
+            uint32_t w = ((x * 0x44011u) & 0x00330033u) | (((y * 0x44011u) << 8) & 0x33003300u);
+            if (na | nb) {                                // window N -> table index 5
+                const uint32_t ma = (na >> (2 * tt)) & 3u, mb = (nb >> (2 * tt)) & 3u;
+                if (ma & 1u) w = (w & 0xFFFFFF00u) | 0x00000055u;
+                if (ma & 2u) w = (w & 0xFF00FFFFu) | 0x00550000u;
+                if (mb & 1u) w = (w & 0xFFFF00FFu) | 0x00005500u;
+                if (mb & 2u) w = (w & 0x00FFFFFFu) | 0x55000000u;
+            }
+            dst[tt] = w;
+            if (mir != nullptr) mir[tt] = w;
+        }
+    }
+}
+
 // resident CTAs per SM the register budget is sized for: 128 registers up to K = 21, 168 above
 #ifndef SDP_SCORE_MIN_CTAS
 #define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)
@@ -210,46 +256,9 @@ score_kernel(const ScoreParams P)
     const RingGeom rg = ring_geometry(G, ngroups);
     uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
     const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
-    const long long win_words = (long long)P.wins_words, nm_words = (long long)P.win_nmask_words;
 
     auto fill_ring = [&](const int s0) {                  // rows s0+1 .. s0+chunk
-        if (!in_group) return;
-        for (int u = g; u < rg.chunk / 16; u += G) {
-            const int r0 = s0 + 16 * u;                   // 0-based row of the unit's first entry
-            uint32_t a = 0u, b = 0u, na = 0u, nb = 0u;
-            if (r0 < mA) {
-                a = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)dA.woff - r0 - 15, win_words))
-                        : load_bases16(P.wins_packed, (long long)dA.woff + r0, win_words);
-                if (P.win_nmask != nullptr)
-                    na = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)dA.woff - r0 - 15, nm_words))
-                             : load_bits16(P.win_nmask, (long long)dA.woff + r0, nm_words);
-            }
-            if (r0 < mB) {
-                b = REV ? reverse_fields2(load_bases16(P.wins_packed, (long long)dB.woff - r0 - 15, win_words))
-                        : load_bases16(P.wins_packed, (long long)dB.woff + r0, win_words);
-                if (P.win_nmask != nullptr)
-                    nb = REV ? reverse_bits16(load_bits16(P.win_nmask, (long long)dB.woff - r0 - 15, nm_words))
-                             : load_bits16(P.win_nmask, (long long)dB.woff + r0, nm_words);
-            }
-            const int slot0 = r0 & (rg.ring - 1);
-            uint32_t* dst = ring_w + 16 + (slot0 >> 1);
-            uint32_t* mir = (slot0 >= rg.ring - 32) ? ring_w + ((slot0 - (rg.ring - 32)) >> 1) : nullptr;
-#pragma unroll
-            for (int tt = 0; tt < 8; ++tt) {
-                // two rows -> two 16-bit selectors (idxA * 0x11 | idxB * 0x1100)
-                const uint32_t x = (a >> (4 * tt)) & 0xFu, y = (b >> (4 * tt)) & 0xFu;
-                uint32_t w = ((x * 0x44011u) & 0x00330033u) | (((y * 0x44011u) << 8) & 0x33003300u);
-                if (na | nb) {                            // window N -> table index 5
-                    const uint32_t ma = (na >> (2 * tt)) & 3u, mb = (nb >> (2 * tt)) & 3u;
-                    if (ma & 1u) w = (w & 0xFFFFFF00u) | 0x00000055u;
-                    if (ma & 2u) w = (w & 0xFF00FFFFu) | 0x00550000u;
-                    if (mb & 1u) w = (w & 0xFFFF00FFu) | 0x00005500u;
-                    if (mb & 2u) w = (w & 0x00FFFFFFu) | 0x55000000u;
-                }
-                dst[tt] = w;
-                if (mir != nullptr) mir[tt] = w;
-            }
-        }
+        if (in_group) fill_ring_rows<REV>(P, rg, ring_w, g, G, s0, dA.woff, mA, dB.woff, mB);
     };
 
     const uint32_t one = P.c.one, negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, e2 = P.c.e2;

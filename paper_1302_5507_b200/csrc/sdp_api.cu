@@ -27,6 +27,14 @@ void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t 
     SDP_SCORE_UNITS(SDP_TRY)
 #undef SDP_TRY
 }
+#define SDP_DECL(r) bool launch_trace_r##r(int, bool, const ScoreParams&, const TraceDP&, cudaStream_t);
+SDP_SCORE_UNITS(SDP_DECL)
+#undef SDP_DECL
+void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st) {
+#define SDP_TRY(r) if (launch_trace_r##r(K, pad, p, t, st)) return;
+    SDP_SCORE_UNITS(SDP_TRY)
+#undef SDP_TRY
+}
 }  // namespace sdp
 
 namespace {
@@ -37,11 +45,11 @@ struct DevBuf {
 };
 
 struct Mailbox {                    // pinned host memory the device results land in
-    uint32_t task_prefix[2][SDP_NSLOTS + 1];
-    uint32_t bin_total[3];
+    uint32_t task_prefix[3][SDP_NSLOTS + 1];   // forward, reverse, traceback DP
+    uint32_t bin_total[4];                     // forward, reverse, thin traceback, wide traceback
     uint32_t tb_bounds[TB_NCLASS + 1];
     uint32_t err_flag;
-    uint64_t totals[3];             // [0] direction-bit words, [1] run capacity, [2] CIGAR runs
+    uint64_t totals[4];             // [0] thin direction-bit words, [1] run capacity, [2] CIGAR runs, [3] wide nibble words
     unsigned long long counters[4]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
 };
 
@@ -54,25 +62,30 @@ struct sdp_ctx {
     sdp_scoring user_sc{};
     Scoring sc{};
     ScoreConsts consts{};
+    TraceConsts tconsts{};
+    int wide_ok = 0;                 // scoring fits the x8 tagged domain of the traceback DP kernel
+    int wide_min_bw = 16;            // bands wider than this take the wide path (SDP_WIDE_MIN_BW overrides)
     char err[512] = {0};
     bool timing = false;
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
     uint32_t cls_begin[2 * SDP_MAX_K + 3];   // first slot of class c = 2K + padded; [c+1] ends it
-    uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr;
+    uint16_t h_slot_of_n[SDP_NSLOTS];        // read length - 1 -> slot
+    uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr, *d_slot_of_n = nullptr;
     Mailbox* mb = nullptr;
     cudaStream_t own_stream = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     // fixed-size device buffers
-    uint32_t* hist[3] = {};          // forward, reverse, traceback
-    uint32_t* bin_start[3] = {};
-    SlotInfo* slots[2] = {};
-    uint32_t* task_prefix[2] = {};
+    uint32_t* hist[4] = {};          // forward, reverse, thin traceback, wide traceback
+    uint32_t* bin_start[4] = {};
+    SlotInfo* slots[3] = {};         // forward, reverse, wide traceback
+    uint32_t* task_prefix[3] = {};
     uint32_t* err_flag = nullptr;
     unsigned long long* counters = nullptr;
     uint64_t* totals = nullptr;
     // per-pair device buffers (grow only)
     DevBuf keys, pn, pm, order, desc, order_rev, desc_rev, order_tb, keys_rev, keys_tb, tbW, rev_rows,
+        tb_rows, keys_wide, order_wide, desc_wide, wide_words, wide_off, wide_bits,
         bits_words, ops_cap, bits_off, ops_off, scan_local, scan_tiles, scan_tile_base,
         score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len,
         bits, ops_rev, cigar_ops;
@@ -150,6 +163,7 @@ void choose_geometry(sdp_ctx* c) {
     for (int k = 0; k <= NC; ++k) c->cls_begin[k] = SDP_NSLOTS;
     for (int t = SDP_NSLOTS - 1; t >= 0; --t) {
         c->h_slot_n[t] = ents[t].n; c->h_slot_G[t] = ents[t].G; c->h_slot_K[t] = ents[t].K;
+        c->h_slot_of_n[ents[t].n - 1] = (uint16_t)t;
         c->cls_begin[cls(ents[t])] = (uint32_t)t;
     }
     // classes that no read length uses start where the next used class starts
@@ -190,6 +204,24 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     ctx->consts.beta2 = sdp_pack2(beta);
     ctx->consts.betaMinusO2 = sdp_pack2(beta - o);
     ctx->consts.o = o; ctx->consts.e = e; ctx->consts.beta = beta; ctx->consts.match = s->match;
+    {   // traceback DP kernel: x8 scaled values with tags in the low three bits (trace_kernel.cuh)
+        const int sc8 = SDP_TB_SCALE;
+        const int qm = sc8 * (2 * e + s->match) + 7, qx = sc8 * (2 * e + s->mismatch) + 7;
+        TraceConsts& t = ctx->tconsts;
+        t.one = 1u; t.c16 = 16u; t.c8 = 8u; t.cm1 = 0xFFFFFFFFu; t.m4 = 0x00040004u;
+        t.negO_e = sdp_pack2(-sc8 * o + 1);
+        t.negO_f = sdp_pack2(-sc8 * o + 6);
+        t.qx = sdp_pack2(qx);
+        t.Cf = sdp_pack2(qm);
+        t.e2 = sdp_pack2(sc8 * e);
+        t.beta2 = sdp_pack2(sc8 * beta);
+        t.betaMinusO2 = sdp_pack2(sc8 * (beta - o));
+        t.e = e; t.beta = beta;
+        // the diagonal increment is added with a 32-bit IMAD: it must be non-negative in both lanes,
+        // and the match increment must stay an fp16 denormal bit pattern
+        ctx->wide_ok = (qx >= 0 && qm < 1024 && sc8 * beta <= 32000) ? 1 : 0;
+        if (const char* v = getenv("SDP_WIDE_MIN_BW")) ctx->wide_min_bw = atoi(v);
+    }
     choose_geometry(ctx);
 
     auto init = [&]() -> int {
@@ -200,21 +232,23 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaMemcpy(ctx->d_slot_n, ctx->h_slot_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(ctx->d_slot_G, ctx->h_slot_G, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(ctx->d_slot_K, ctx->h_slot_K, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+        CU(cudaMalloc(&ctx->d_slot_of_n, SDP_NSLOTS * 2));
+        CU(cudaMemcpy(ctx->d_slot_of_n, ctx->h_slot_of_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
         CU(cudaMallocHost(&ctx->mb, sizeof(Mailbox)));
         memset(ctx->mb, 0, sizeof(Mailbox));
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
         for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
-        for (int i = 0; i < 3; ++i) {
+        for (int i = 0; i < 4; ++i) {
             CU(cudaMalloc(&ctx->hist[i], (SDP_NBINS + 1) * 4));
             CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 1) * 4));
         }
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < 3; ++i) {
             CU(cudaMalloc(&ctx->slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
             CU(cudaMalloc(&ctx->task_prefix[i], (SDP_NSLOTS + 1) * 4));
         }
         CU(cudaMalloc(&ctx->err_flag, 4));
         CU(cudaMalloc(&ctx->counters, 4 * 8));
-        CU(cudaMalloc(&ctx->totals, 3 * 8));
+        CU(cudaMalloc(&ctx->totals, 4 * 8));
         return SDP_OK;
     };
     int rc = init();
@@ -234,13 +268,14 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->read_end, &ctx->pass, &ctx->n_match, &ctx->n_cols, &ctx->cigar_off, &ctx->cigar_len,
                       &ctx->bits, &ctx->ops_rev, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
-                      &ctx->in_win_nmask, &ctx->in_pairs};
+                      &ctx->in_win_nmask, &ctx->in_pairs, &ctx->tb_rows, &ctx->keys_wide, &ctx->order_wide,
+                      &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
-    for (int i = 0; i < 3; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
-    for (int i = 0; i < 2; ++i) { cudaFree(ctx->slots[i]); cudaFree(ctx->task_prefix[i]); }
+    for (int i = 0; i < 4; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
+    for (int i = 0; i < 3; ++i) { cudaFree(ctx->slots[i]); cudaFree(ctx->task_prefix[i]); }
     cudaFree(ctx->err_flag); cudaFree(ctx->counters); cudaFree(ctx->totals);
-    cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K);
+    cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K); cudaFree(ctx->d_slot_of_n);
     if (ctx->mb) cudaFreeHost(ctx->mb);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -266,9 +301,13 @@ int sdp_measure_dpx_rate(int cuda_device, double* rate, int32_t* sms, double* mh
     return measure_dpx_rate(cuda_device, rate, sms, mhz);
 }
 
-static int launch_score_stage(sdp_ctx* ctx, int which, bool rev, const sdp_batch& b, const PairDesc* desc,
+// which: 0 forward, 1 reverse, 2 traceback DP (trace_kernel)
+static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const PairDesc* desc,
                               cudaStream_t st, uint32_t* nlaunch)
 {
+    const bool rev = which == 1;
+    TraceDP td{};
+    td.c = ctx->tconsts; td.bits = ctx->wide_bits.as<uint32_t>(); td.bits_off = ctx->wide_off.as<uint64_t>();
     const uint32_t* tp = ctx->mb->task_prefix[which];
     ScoreParams sp{};
     sp.reads_packed = b.reads_packed; sp.read_nmask = b.read_nmask;
@@ -286,7 +325,8 @@ static int launch_score_stage(sdp_ctx* ctx, int which, bool rev, const sdp_batch
         const uint32_t t0 = tp[s0], t1 = tp[s1];
         if (t1 <= t0) continue;
         sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
-        launch_score(cls >> 1, (cls & 1) != 0, rev, sp, st);
+        if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, st);
+        else launch_score(cls >> 1, (cls & 1) != 0, rev, sp, st);
         ++*nlaunch;
     }
     CU(cudaGetLastError());
@@ -314,6 +354,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     EN(keys, Pp * 4); EN(pn, Pp * 4); EN(pm, Pp * 4); EN(order, Pp * 4); EN(desc, Pp * sizeof(PairDesc));
     EN(order_rev, Pp * 4); EN(desc_rev, Pp * sizeof(PairDesc)); EN(order_tb, Pp * 4);
     EN(keys_rev, Pp * 4); EN(keys_tb, Pp * 4); EN(tbW, Pp * 4); EN(rev_rows, Pp * 4);
+    EN(tb_rows, Pp * 4); EN(keys_wide, Pp * 4); EN(order_wide, Pp * 4); EN(desc_wide, Pp * sizeof(PairDesc));
+    EN(wide_words, Pp * 4); EN(wide_off, Pp * 8);
     EN(bits_words, Pp * 4); EN(ops_cap, Pp * 4); EN(bits_off, Pp * 8); EN(ops_off, Pp * 8);
     EN(scan_local, Pp * 4); EN(scan_tiles, (Pp / 4096 + 2) * 4); EN(scan_tile_base, (Pp / 4096 + 2) * 8);
     EN(score, Pp * 4); EN(ref_start, Pp * 4); EN(ref_end, Pp * 4); EN(read_start, Pp * 4); EN(read_end, Pp * 4);
@@ -336,7 +378,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_START], st));
     // ---- a1 + a2
-    for (int i = 0; i < 3; ++i) CU(cudaMemsetAsync(ctx->hist[i], 0, (SDP_NBINS + 1) * 4, st));
+    for (int i = 0; i < 4; ++i) CU(cudaMemsetAsync(ctx->hist[i], 0, (SDP_NBINS + 1) * 4, st));
     CU(cudaMemsetAsync(ctx->err_flag, 0, 4, st));
     CU(cudaMemsetAsync(ctx->counters, 0, 4 * 8, st));
     launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
@@ -359,7 +401,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     // ---- a3 forward score pass
     {
         uint32_t before = nl;
-        int rc = launch_score_stage(ctx, 0, false, b, ctx->desc.as<PairDesc>(), st, &nl);
+        int rc = launch_score_stage(ctx, 0, b, ctx->desc.as<PairDesc>(), st, &nl);
         if (rc != SDP_OK) return rc;
         stats.forward_launches = nl - before;
     }
@@ -369,15 +411,29 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     PostParams pp{};
     pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
     pp.score = ctx->score.as<int32_t>(); pp.ref_end = ctx->ref_end.as<int32_t>();
-    pp.tbW = ctx->tbW.as<int32_t>(); pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
+    pp.tbW = ctx->tbW.as<int32_t>(); pp.tb_rows = ctx->tb_rows.as<int32_t>();
+    pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
+    pp.keys_wide = ctx->keys_wide.as<uint32_t>();
+    pp.wide_ok = ctx->wide_ok; pp.wide_min_bw = ctx->wide_min_bw;
     pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
-    pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.counters = ctx->counters;
+    pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
     launch_sort_tail(ctx->keys_rev.as<uint32_t>(), P, ctx->hist[1], ctx->bin_start[1], ctx->order_rev.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1], st);
     launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
                      nullptr, nullptr, nullptr, nullptr, nullptr, st);
-    nl += 6;
+    launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2], st);
+    nl += 9;
+    // one region of direction nibbles per two wide pairs that share the int16x2 lanes (every slot of
+    // order_wide beyond the wide pairs reads as a zero-size region)
+    CU(cudaMemsetAsync(ctx->wide_words.p, 0, P * 4, st));
+    launch_wide_regions(ctx->order_wide.as<uint32_t>(), (uint32_t)P, ctx->bin_start[3] + SDP_NBINS, ctx->pn.as<uint32_t>(),
+                        ctx->tb_rows.as<int32_t>(), ctx->d_slot_of_n, ctx->slots[2], ctx->wide_words.as<uint32_t>(), st);
+    ++nl;
+    exclusive_scan_u32_u64(ctx->wide_words.as<uint32_t>(), P, ctx->wide_off.as<uint64_t>(), ctx->totals + 3,
+                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
+                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
     exclusive_scan_u32_u64(ctx->bits_words.as<uint32_t>(), P, ctx->bits_off.as<uint64_t>(), ctx->totals + 0,
                            ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
                            ctx->scan_tile_base.as<uint64_t>(), st, &nl);
@@ -385,32 +441,58 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
                            ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
                            ctx->scan_tile_base.as<uint64_t>(), st, &nl);
     CU(cudaMemcpyAsync(ctx->mb->task_prefix[1], ctx->task_prefix[1], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->mb->task_prefix[2], ctx->task_prefix[2], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[1], ctx->bin_start[1] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&ctx->mb->bin_total[3], ctx->bin_start[3] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
     for (int c = 0; c <= TB_NCLASS; ++c)
         CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * 8192, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 2 * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->mb->counters, ctx->counters, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const uint32_t n_rev = ctx->mb->bin_total[1];
+    const uint32_t n_wide = ctx->mb->bin_total[3];
+    const uint32_t n_thin = ctx->mb->tb_bounds[TB_NCLASS];
     EN(bits, (ctx->mb->totals[0] + 4) * 4);
     EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
     EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
+    EN(wide_bits, (ctx->mb->totals[3] + 4) * 4);
 
     // ---- a4 reverse pass over the pairs whose score admits a gap
     launch_fill_desc_rev(b, ctx->order_rev.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
                          ctx->tbW.as<int32_t>(), ctx->desc_rev.as<PairDesc>(), st);
     ++nl;
     {
-        int rc = launch_score_stage(ctx, 1, true, b, ctx->desc_rev.as<PairDesc>(), st, &nl);
+        int rc = launch_score_stage(ctx, 1, b, ctx->desc_rev.as<PairDesc>(), st, &nl);
         if (rc != SDP_OK) return rc;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_REVERSE], st));
 
     // ---- a5 + a6 traceback, CIGAR runs, similarity filter
+    // wide pairs: rectangle DP that leaves four direction bits per cell, then the walk
+    if (n_wide) {
+        launch_fill_desc_tb(b, ctx->order_wide.as<uint32_t>(), n_wide, ctx->score.as<int32_t>(),
+                            ctx->ref_end.as<int32_t>(), ctx->rev_rows.as<int32_t>(), ctx->desc_wide.as<PairDesc>(), st);
+        ++nl;
+        int rc = launch_score_stage(ctx, 2, b, ctx->desc_wide.as<PairDesc>(), st, &nl);
+        if (rc != SDP_OK) return rc;
+        WalkParams wp{};
+        wp.b = b; wp.sc = ctx->sc; wp.desc = ctx->desc_wide.as<PairDesc>(); wp.count = n_wide;
+        wp.slots = ctx->slots[2]; wp.slot_of_n = ctx->d_slot_of_n;
+        wp.bits = ctx->wide_bits.as<uint32_t>(); wp.bits_off = ctx->wide_off.as<uint64_t>();
+        wp.ref_end = ctx->ref_end.as<int32_t>(); wp.tbW = ctx->tbW.as<int32_t>();
+        wp.ops_off = ctx->ops_off.as<uint64_t>(); wp.ops_rev = ctx->ops_rev.as<uint32_t>();
+        wp.ref_start = ctx->ref_start.as<int32_t>(); wp.read_start = ctx->read_start.as<int32_t>();
+        wp.read_end = ctx->read_end.as<int32_t>(); wp.pass = ctx->pass.as<uint8_t>();
+        wp.n_match = ctx->n_match.as<int32_t>(); wp.n_cols = ctx->n_cols.as<int32_t>();
+        wp.cigar_len = ctx->cigar_len.as<uint32_t>(); wp.err_flag = ctx->err_flag;
+        launch_walk(wp, st);
+        ++nl;
+    }
+    // everything else: one thread per pair, band of width min(2W+1, n+1)
     TraceParams tp{};
     tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
     tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
-    tp.rev_rows = ctx->rev_rows.as<int32_t>();
+    tp.rev_rows = nullptr;
     tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
     tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
     tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
@@ -419,10 +501,10 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
     for (int c = 0; c < TB_NCLASS; ++c) {
         tp.first = ctx->mb->tb_bounds[c];
-        const uint32_t end = (c + 1 < TB_NCLASS) ? ctx->mb->tb_bounds[c + 1] : (uint32_t)P;
-        tp.count = end - tp.first;
+        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
         if (tp.count) { launch_traceback(c, tp, st); ++nl; }
     }
+    (void)n_thin;
     CU(cudaGetLastError());
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
 

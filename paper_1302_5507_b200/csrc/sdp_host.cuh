@@ -25,6 +25,7 @@ void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint6
 
 // ---- score_inst.cu (compiled once per K range)
 void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t st);
+void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st);
 
 // ---- traceback.cu
 struct PostParams {
@@ -33,11 +34,15 @@ struct PostParams {
     const uint32_t* pn; const uint32_t* pm;      // per pair read / window length
     const int32_t* score; const int32_t* ref_end;
     int32_t* tbW;                // gap-content bound W per pair
-    uint32_t* keys_rev;          // bucket key of the reverse pass (SKIP when W == 0)
-    uint32_t* keys_tb;           // bucket key of the traceback pass
+    int32_t* tb_rows;            // rows the traceback may need: min(i_end, n + W), 0 when W == 0
+    uint32_t* keys_rev;          // bucket key of the reverse pass (wide pairs only, else SKIP)
+    uint32_t* keys_wide;         // bucket key of the traceback DP kernel (wide pairs only, else SKIP)
+    uint32_t* keys_tb;           // bucket key of the one-thread-per-pair traceback (everything else)
+    int wide_ok;                 // scoring fits the x8 tagged domain of trace_kernel.cuh
+    int wide_min_bw;             // bands wider than this take the wide path
     uint32_t* bits_words;        // direction-bit words the pair needs
     uint32_t* ops_cap;           // CIGAR run capacity the pair needs (2W + 1)
-    uint32_t* hist_rev; uint32_t* hist_tb;
+    uint32_t* hist_rev; uint32_t* hist_tb; uint32_t* hist_wide;
     unsigned long long* counters;   // [0] reverse cells, [1] traceback cells, [2] reverse pairs
 };
 void launch_post_forward(const PostParams& pp, cudaStream_t st);
@@ -56,6 +61,24 @@ struct TraceParams {
     int32_t* n_match; int32_t* n_cols; uint32_t* cigar_len;
     uint32_t* err_flag;
 };
+void launch_wide_regions(const uint32_t* order, uint32_t max_count, const uint32_t* count_dev, const uint32_t* pn,
+                         const int32_t* tb_rows, const uint16_t* slot_of_n, const SlotInfo* slots, uint32_t* words,
+                         cudaStream_t st);
+void launch_fill_desc_tb(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
+                         const int32_t* ref_end, const int32_t* rev_rows, PairDesc* desc, cudaStream_t st);
+struct WalkParams {
+    sdp_batch b;
+    Scoring sc;
+    const PairDesc* desc; uint32_t count;         // traceback-DP descriptors (wide order)
+    const SlotInfo* slots; const uint16_t* slot_of_n;
+    const uint32_t* bits; const uint64_t* bits_off;
+    const int32_t* ref_end; const int32_t* tbW;
+    const uint64_t* ops_off; uint32_t* ops_rev;
+    int32_t* ref_start; int32_t* read_start; int32_t* read_end; uint8_t* pass;
+    int32_t* n_match; int32_t* n_cols; uint32_t* cigar_len;
+    uint32_t* err_flag;
+};
+void launch_walk(const WalkParams& wp, cudaStream_t st);
 // band-width classes of the traceback kernel (local-memory row arrays)
 constexpr int TB_NCLASS = 4;
 constexpr int TB_CLASS_BW[TB_NCLASS] = {16, 64, 256, 1032};   // band <= min(2W+1, n+1) <= 1025

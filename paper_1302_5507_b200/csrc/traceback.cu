@@ -44,7 +44,7 @@ __global__ void k_post_forward(const PostParams pp)
 {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = p < pp.n_pairs;
-    uint32_t krev = SDP_KEY_SKIP, ktb = SDP_KEY_SKIP;
+    uint32_t krev = SDP_KEY_SKIP, ktb = SDP_KEY_SKIP, kwide = SDP_KEY_SKIP;
     unsigned long long c_rev = 0, c_tb = 0, n_rev = 0;
     if (valid) {
         const int n = (int)pp.pn[p];
@@ -54,28 +54,41 @@ __global__ void k_post_forward(const PostParams pp)
         W = min(W, n + i_end);
         pp.tbW[p] = W;
         uint32_t words = 0;
-        int bw = 1;
+        int bw = 1, rows = 0;
         if (W > 0) {
-            const int rows = min(i_end, n + W);
-            krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
+            rows = min(i_end, n + W);
             bw = min(2 * W + 1, n + 1);
-            words = (uint32_t)rows * (uint32_t)((bw + 7) / 8);
-            c_rev = (unsigned long long)n * rows; c_tb = (unsigned long long)bw * rows; n_rev = 1;
+        }
+        pp.tb_rows[p] = rows;
+        // wide pairs: the register-resident wavefront recomputes the whole rectangle rows x n
+        // (trace_kernel.cuh) when its x8 scaled values fit 16 bits; the reverse pass first trims
+        // the rectangle's rows. Narrow bands and everything else: one thread per pair.
+        const long long vmax = (long long)pp.sc.match * n + (long long)pp.sc.gap_extend * (n + rows) +
+                               3LL * pp.sc.gap_open + 8;
+        const bool wide = W > 0 && pp.wide_ok && bw > pp.wide_min_bw && vmax <= SDP_TB_MAX_VALUE;
+        if (wide) {
+            krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
+            kwide = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, (rows + 7) >> 3);
+            c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
+        } else {
+            if (W > 0) { words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows; }
+            ktb = (uint32_t)tb_class_of(bw) * 8192u + (uint32_t)min(bw, 8191);
         }
         pp.keys_rev[p] = krev;
+        pp.keys_wide[p] = kwide;
+        pp.keys_tb[p] = ktb;
         pp.bits_words[p] = words;
         pp.ops_cap[p] = 2u * (uint32_t)W + 3u;
-        ktb = (uint32_t)tb_class_of(bw) * 8192u + (uint32_t)min(bw, 8191);
-        pp.keys_tb[p] = ktb;
     }
     hist_add(pp.hist_rev, krev, krev != SDP_KEY_SKIP);
     hist_add(pp.hist_tb, ktb, ktb != SDP_KEY_SKIP);
+    hist_add(pp.hist_wide, kwide, kwide != SDP_KEY_SKIP);
     for (int o = 16; o > 0; o >>= 1) {
         c_rev += __shfl_down_sync(0xffffffffu, c_rev, o);
         c_tb += __shfl_down_sync(0xffffffffu, c_tb, o);
         n_rev += __shfl_down_sync(0xffffffffu, n_rev, o);
     }
-    if ((threadIdx.x & 31) == 0 && n_rev) {
+    if ((threadIdx.x & 31) == 0 && (c_tb | n_rev)) {
         atomicAdd(pp.counters + 0, c_rev); atomicAdd(pp.counters + 1, c_tb); atomicAdd(pp.counters + 2, n_rev);
     }
 }
@@ -154,7 +167,7 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
         emit(0, (uint32_t)n);
     } else {
         const int c = i_end - n;
-        const int s_lo = tp.rev_rows ? i_end - tp.rev_rows[p] : 0;
+        const int s_lo = 0;                               // thin pairs skip the reverse pass
         const int i_lo = max(0, max(s_lo, i_end - n - W));
         const bool banded = (2 * W + 1 < n + 1);
         const int bw = banded ? 2 * W + 1 : n + 1;
@@ -253,6 +266,137 @@ void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st)
         case 2: k_traceback<256><<<grid, 128, 0, st>>>(tp); break;
         default: k_traceback<1032><<<grid, 128, 0, st>>>(tp); break;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// wide pairs (trace_kernel.cuh). Sorted by (n, rows) into `order`; two neighbours of one read
+// length share the int16x2 lanes and one region of direction nibbles.
+__global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_count,
+                               const uint32_t* __restrict__ count_dev, const uint32_t* __restrict__ pn,
+                               const int32_t* __restrict__ tb_rows, const uint16_t* __restrict__ slot_of_n,
+                               const SlotInfo* __restrict__ slots, uint32_t* __restrict__ words)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= max_count || k >= *count_dev) return;       // the number of wide pairs is only known on the device
+    const uint32_t p = order[k];
+    const SlotInfo si = slots[slot_of_n[pn[p] - 1]];
+    const uint32_t local = k - si.first;
+    uint32_t w = 0;
+    if ((local & 1u) == 0) {
+        int rows = tb_rows[p];
+        if (local + 1 < si.count) rows = max(rows, tb_rows[order[k + 1]]);
+        w = (uint32_t)rows * (uint32_t)si.G * (uint32_t)((si.K + 3) / 4);
+    }
+    words[k] = w;
+}
+
+void launch_wide_regions(const uint32_t* order, uint32_t max_count, const uint32_t* count_dev, const uint32_t* pn,
+                         const int32_t* tb_rows, const uint16_t* slot_of_n, const SlotInfo* slots, uint32_t* words,
+                         cudaStream_t st)
+{
+    if (max_count)
+        k_wide_regions<<<(max_count + 255) / 256, 256, 0, st>>>(order, max_count, count_dev, pn, tb_rows, slot_of_n,
+                                                                 slots, words);
+}
+
+// descriptors of the traceback DP: rows (i_lo, i_end] with i_lo = i_end - R, R = rows the reverse
+// pass found the longest co-optimal alignment to span (at least 1, so that the DP has a row)
+__global__ void k_fill_desc_tb(const sdp_batch b, const uint32_t* __restrict__ order, uint32_t count,
+                               const int32_t* __restrict__ score, const int32_t* __restrict__ ref_end,
+                               const int32_t* __restrict__ rev_rows, PairDesc* __restrict__ desc)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    const uint32_t p = order[k];
+    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+    const int i_end = ref_end[p] + 1;
+    const int R = min(i_end, max(1, rev_rows[p]));
+    PairDesc d;
+    d.n = b.read_len[ri];
+    d.roff = b.read_off[ri];
+    d.woff = b.win_off[wi] + (uint64_t)(i_end - R);
+    d.m = (uint32_t)R;
+    d.pid = p; d.aux = score[p];
+    desc[k] = d;
+}
+
+void launch_fill_desc_tb(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
+                         const int32_t* ref_end, const int32_t* rev_rows, PairDesc* desc, cudaStream_t st)
+{
+    if (count) k_fill_desc_tb<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, score, ref_end, rev_rows, desc);
+}
+
+// the walk (R6) over the nibbles trace_kernel left: one thread per pair
+__global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
+{
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= wp.count) return;
+    const PairDesc d = wp.desc[k];
+    const uint32_t p = d.pid;
+    const int n = (int)d.n, R = (int)d.m;
+    const SlotInfo si = wp.slots[wp.slot_of_n[n - 1]];
+    const uint32_t local = k - si.first;
+    const int G = si.G, K = si.K, NW = (K + 3) / 4;
+    const int pad = G * K - n;
+    const uint32_t* region = wp.bits + wp.bits_off[k - (local & 1u)];
+    const uint32_t lane_shift = (local & 1u) * 16u;
+    const SeqReader RD{wp.b.reads_packed, wp.b.read_nmask, SDP_CODE_READ_N};
+    const SeqReader WN{wp.b.wins_packed, wp.b.win_nmask, SDP_CODE_WIN_N};
+    const uint32_t cap = 2u * (uint32_t)wp.tbW[p] + 3u;
+    uint32_t* ops = wp.ops_rev + wp.ops_off[p];
+
+    int n_match = 0, n_cols = 0;
+    uint32_t nops = 0;
+    int cur_op = -1; uint32_t cur_len = 0;
+    bool bad = false;
+    auto emit = [&](int op, uint32_t len) {
+        if (op == cur_op) { cur_len += len; return; }
+        if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
+        cur_op = op; cur_len = len;
+    };
+    int i = R, j = n, st = 0;                              // 0 = H, 1 = D, 2 = I
+    const int split = pad * (K - 1);                       // columns owned by the threads that skip one
+    while (j > 0) {
+        if (i == 0) { emit(1, (uint32_t)j); n_cols += j; j = 0; break; }   // row i_lo: all insertions
+        const int j0 = j - 1;
+        int g, kk;
+        if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
+        else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
+        const int w = kk >> 2;
+        const int cw = min(4, K - 4 * w);
+        const uint32_t word = __ldg(region + ((size_t)(i - 1) * G + g) * NW + w);
+        const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(cw - 1 - (kk & 3)))) & 15u;
+        if (st == 0) {
+            if ((f & 3u) == 3u) {
+                emit(0, 1u); ++n_cols;
+                n_match += (RD.at(d.roff + (uint64_t)j0) == WN.at(d.woff + (uint64_t)(i - 1)));
+                --i; --j;
+            } else if ((f & 3u) == 2u) st = 1;
+            else st = 2;
+        } else if (st == 1) {
+            emit(2, 1u); ++n_cols;
+            if (f & 4u) st = 0;
+            --i;
+        } else {
+            emit(1, 1u); ++n_cols;
+            if (f & 8u) st = 0;
+            --j;
+        }
+    }
+    emit(-2, 0u);
+    if (bad) { atomicOr(wp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
+    wp.ref_start[p] = wp.ref_end[p] + 1 - R + i;
+    wp.read_start[p] = 0;
+    wp.read_end[p] = n - 1;
+    wp.n_match[p] = n_match;
+    wp.n_cols[p] = n_cols;
+    wp.cigar_len[p] = nops;
+    wp.pass[p] = ((long long)n_match * 1000000LL >= wp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
+}
+
+void launch_walk(const WalkParams& wp, cudaStream_t st)
+{
+    if (wp.count) k_walk<<<(wp.count + 127) / 128, 128, 0, st>>>(wp);
 }
 
 // a7: copy each pair's runs (stored end -> start) into the dense buffer in alignment order
