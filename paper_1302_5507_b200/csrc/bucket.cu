@@ -176,6 +176,27 @@ __global__ void __launch_bounds__(1024) k_scan_tiles(const uint32_t* __restrict_
     if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
 }
 
+// 64-bit variant for the tile sums (1024 tile sums of up to 2^32 - 1 each do not fit 32 bits)
+__device__ __forceinline__ uint64_t block_exclusive_scan_1024_u64(uint64_t v, uint64_t* total)
+{
+    __shared__ uint64_t warp_sums64[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint64_t x = v;
+    for (int o = 1; o < 32; o <<= 1) { uint64_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) warp_sums64[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        uint64_t s = warp_sums64[lane];
+        for (int o = 1; o < 32; o <<= 1) { uint64_t y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+        warp_sums64[lane] = s;
+    }
+    __syncthreads();
+    const uint64_t base = w ? warp_sums64[w - 1] : 0ull;
+    if (total) *total = warp_sums64[31];
+    __syncthreads();
+    return base + x - v;
+}
+
 __global__ void __launch_bounds__(1024) k_scan_tile_sums(const uint32_t* __restrict__ tile_sums, uint32_t ntiles,
                                                          uint64_t* __restrict__ tile_base, uint64_t* __restrict__ total_out)
 {
@@ -184,9 +205,9 @@ __global__ void __launch_bounds__(1024) k_scan_tile_sums(const uint32_t* __restr
     __syncthreads();
     for (uint32_t start = 0; start < ntiles; start += 1024) {
         const uint32_t idx = start + threadIdx.x;
-        const uint32_t v = idx < ntiles ? tile_sums[idx] : 0u;
-        uint32_t total;
-        const uint32_t pre = block_exclusive_scan_1024(v, &total);
+        const uint64_t v = idx < ntiles ? (uint64_t)tile_sums[idx] : 0ull;
+        uint64_t total;
+        const uint64_t pre = block_exclusive_scan_1024_u64(v, &total);
         if (idx < ntiles) tile_base[idx] = carry + pre;
         __syncthreads();
         if (threadIdx.x == 0) carry += total;
