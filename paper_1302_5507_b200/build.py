@@ -42,7 +42,7 @@ def _deps_hash(extra: str) -> str:
 
 
 def _units():
-    units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []),
+    units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []), ("thin_kernel", "thin_kernel.cu", []),
              ("microbench", "microbench.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"score_r{r}", "score_inst.cu",

@@ -47,7 +47,7 @@ struct DevBuf {
 struct Mailbox {                    // pinned host memory the device results land in
     uint32_t task_prefix[3][SDP_NSLOTS + 1];   // forward, reverse, traceback DP
     uint32_t bin_total[4];                     // forward, reverse, thin traceback, wide traceback
-    uint32_t tb_bounds[TB_NCLASS + 1];
+    uint32_t tb_bounds[THIN_NW + TB_NCLASS + 1];   // narrow-band launches (one per W), then the generic band classes
     uint32_t err_flag;
     uint64_t totals[4];             // [0] thin direction-bit words, [1] run capacity, [2] CIGAR runs, [3] wide nibble words
     unsigned long long counters[4]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
@@ -64,7 +64,7 @@ struct sdp_ctx {
     ScoreConsts consts{};
     TraceConsts tconsts{};
     int wide_ok = 0;                 // scoring fits the x8 tagged domain of the traceback DP kernel
-    int wide_min_bw = 16;            // bands wider than this take the wide path (SDP_WIDE_MIN_BW overrides)
+    int no_thin = 0;                 // SDP_NO_THIN=1: keep W >= 1 pairs off the narrow-band kernel (debugging)
     char err[512] = {0};
     bool timing = false;
     sdp_stats stats{};
@@ -220,7 +220,8 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         // the diagonal increment is added with a 32-bit IMAD: it must be non-negative in both lanes,
         // and the match increment must stay an fp16 denormal bit pattern
         ctx->wide_ok = (qx >= 0 && qm < 1024 && sc8 * beta <= 32000) ? 1 : 0;
-        if (const char* v = getenv("SDP_WIDE_MIN_BW")) ctx->wide_min_bw = atoi(v);
+        if (const char* v = getenv("SDP_NO_THIN")) ctx->no_thin = atoi(v);
+        if (const char* v = getenv("SDP_NO_WIDE")) { if (atoi(v)) ctx->wide_ok = 0; }
     }
     choose_geometry(ctx);
 
@@ -414,7 +415,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     pp.tbW = ctx->tbW.as<int32_t>(); pp.tb_rows = ctx->tb_rows.as<int32_t>();
     pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
     pp.keys_wide = ctx->keys_wide.as<uint32_t>();
-    pp.wide_ok = ctx->wide_ok; pp.wide_min_bw = ctx->wide_min_bw;
+    pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin;
     pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
     pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
@@ -444,14 +445,13 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     CU(cudaMemcpyAsync(ctx->mb->task_prefix[2], ctx->task_prefix[2], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[1], ctx->bin_start[1] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[3], ctx->bin_start[3] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
-    for (int c = 0; c <= TB_NCLASS; ++c)
-        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * 8192, 4, cudaMemcpyDeviceToHost, st));
+    for (int c = 0; c <= THIN_NW + TB_NCLASS; ++c)
+        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * 4096, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->mb->counters, ctx->counters, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const uint32_t n_rev = ctx->mb->bin_total[1];
     const uint32_t n_wide = ctx->mb->bin_total[3];
-    const uint32_t n_thin = ctx->mb->tb_bounds[TB_NCLASS];
     EN(bits, (ctx->mb->totals[0] + 4) * 4);
     EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
     EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
@@ -488,7 +488,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         launch_walk(wp, st);
         ++nl;
     }
-    // everything else: one thread per pair, band of width min(2W+1, n+1)
+    // narrow bands (W <= 7): one thread per pair, band in registers; leftovers: generic band kernel
     TraceParams tp{};
     tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
     tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
@@ -499,12 +499,13 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
     tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
     tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    for (int c = 0; c < TB_NCLASS; ++c) {
+    for (int c = 0; c < THIN_NW + TB_NCLASS; ++c) {
         tp.first = ctx->mb->tb_bounds[c];
         tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
-        if (tp.count) { launch_traceback(c, tp, st); ++nl; }
+        if (!tp.count) continue;
+        if (c < THIN_NW) launch_thin(c, tp, st); else launch_traceback(c - THIN_NW, tp, st);
+        ++nl;
     }
-    (void)n_thin;
     CU(cudaGetLastError());
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
 

@@ -39,7 +39,7 @@ struct PostParams {
     uint32_t* keys_wide;         // bucket key of the traceback DP kernel (wide pairs only, else SKIP)
     uint32_t* keys_tb;           // bucket key of the one-thread-per-pair traceback (everything else)
     int wide_ok;                 // scoring fits the x8 tagged domain of trace_kernel.cuh
-    int wide_min_bw;             // bands wider than this take the wide path
+    int no_thin;                 // debugging: keep W >= 1 pairs off the narrow-band kernel
     uint32_t* bits_words;        // direction-bit words the pair needs
     uint32_t* ops_cap;           // CIGAR run capacity the pair needs (2W + 1)
     uint32_t* hist_rev; uint32_t* hist_tb; uint32_t* hist_wide;
@@ -83,6 +83,10 @@ void launch_walk(const WalkParams& wp, cudaStream_t st);
 constexpr int TB_NCLASS = 4;
 constexpr int TB_CLASS_BW[TB_NCLASS] = {16, 64, 256, 1032};   // band <= min(2W+1, n+1) <= 1025
 void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st);
+// narrow bands (thin_kernel.cu): one launch per gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
+constexpr int THIN_NW = 8;
+constexpr int THIN_MAXROWS = 336;
+void launch_thin(int W, const TraceParams& tp, cudaStream_t st);
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 

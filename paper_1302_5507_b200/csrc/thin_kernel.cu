@@ -1,0 +1,251 @@
+// thin_kernel.cu -- a5/a6 for pairs whose score leaves room for few gap bases: one thread per pair.
+//
+// The forward score S bounds the gap content of every co-optimal alignment,
+// W = floor((n*match - S - o) / e), so every co-optimal path lies in the
+// band |i - j - (i_end - n)| <= W of rows (i_end - n - W, i_end]. For W = 0 the alignment is
+// gapless: CIGAR nM, n_match by XOR + popcount over the 2-bit words. For 1 <= W <= 7 the band
+// (2W+1 <= 15 columns) is recomputed with the paper's recurrences in the same
+// x8 tagged integer domain as trace_kernel.cuh -- scalar int32 here, band cells in registers, the
+// row loop fully unrolled over the band -- and leaves four direction bits per cell in a per-thread
+// (hardware-interleaved, hence coalesced) local-memory array; the walk of PAPER.md:353 /
+// DESIGN.md R6 then reads them back. Nothing of this uses the reverse pass.
+#include "sdp_host.cuh"
+
+namespace sdp {
+
+namespace {
+
+constexpr int TNEG = -(1 << 28);                  // "minus infinity", a multiple of 8
+
+// 16 consecutive 2-bit bases starting at base position pos; words outside [0, nwords) read as 0
+__device__ __forceinline__ uint32_t bases16(const uint32_t* __restrict__ packed, long long pos, long long nwords) {
+    const long long w = pos >> 4;
+    const uint32_t sh = ((uint32_t)pos & 15u) * 2u;
+    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(packed + w) : 0u;
+    const uint32_t hi = (sh != 0u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(packed + w + 1) : 0u;
+    return __funnelshift_r(lo, hi, sh);
+}
+// 16 consecutive mask bits starting at bit position pos, spread to the even bit positions
+__device__ __forceinline__ uint32_t nbits16_spread(const uint32_t* __restrict__ bits, long long pos, long long nwords) {
+    if (bits == nullptr) return 0u;
+    const long long w = pos >> 5;
+    const uint32_t sh = (uint32_t)pos & 31u;
+    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(bits + w) : 0u;
+    const uint32_t hi = (sh > 16u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(bits + w + 1) : 0u;
+    uint32_t x = __funnelshift_r(lo, hi, sh) & 0xFFFFu;
+    x = (x | (x << 8)) & 0x00FF00FFu;
+    x = (x | (x << 4)) & 0x0F0F0F0Fu;
+    x = (x | (x << 2)) & 0x33333333u;
+    x = (x | (x << 1)) & 0x55555555u;
+    return x;
+}
+// even bit 2k set iff base k of a and of b are equal (N never equal)
+__device__ __forceinline__ uint32_t eq16(uint32_t a, uint32_t b, uint32_t nmask_spread) {
+    const uint32_t x = a ^ b;
+    return ~(x | (x >> 1) | nmask_spread) & 0x55555555u;
+}
+
+__device__ __forceinline__ int base_at(const uint32_t* __restrict__ packed, const uint32_t* __restrict__ nmask,
+                                       uint64_t pos, int ncode) {
+    int c = (int)((__ldg(packed + (pos >> 4)) >> (2u * ((uint32_t)pos & 15u))) & 3u);
+    if (nmask != nullptr && ((__ldg(nmask + (pos >> 5)) >> ((uint32_t)pos & 31u)) & 1u)) c = ncode;
+    return c;
+}
+
+}  // namespace
+
+struct ThinConsts {
+    int negOe;      // 8 * (-o) + 1
+    int negOf;      // 8 * (-o) + 6
+    int qm, qx;     // 8 * (2e + match) + 7, 8 * (2e + mismatch) + 7
+    int e8;         // 8 * e
+};
+
+// W_ = gap-content bound of every pair of the launch (0 = gapless). MAXROWS bounds the rows of the
+// band (n + W); pairs beyond it are classified onto the other paths by k_post_forward.
+template <int W_, int MAXROWS>
+__global__ void __launch_bounds__(128) k_thin(const TraceParams tp, const ThinConsts tc)
+{
+    constexpr int BW = 2 * W_ + 1;                 // band columns
+    constexpr int WPR = (BW + 7) / 8;              // 32-bit words of direction nibbles per row
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= tp.count) return;
+    const uint32_t p = tp.order[tp.first + k];
+    const sdp_batch& b = tp.b;
+    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+    const int n = (int)b.read_len[ri];
+    const uint64_t roff = b.read_off[ri], woff = b.win_off[wi];
+    const int i_end = tp.ref_end[p] + 1;
+    const long long rwords = (long long)((b.reads_bases + 15) / 16), wwords = (long long)((b.wins_bases + 15) / 16);
+    const long long rnwords = (long long)((b.reads_bases + 31) / 32), wnwords = (long long)((b.wins_bases + 31) / 32);
+    uint32_t* ops = tp.ops_rev + tp.ops_off[p];
+    constexpr uint32_t cap = 2u * (uint32_t)W_ + 3u;
+
+    int n_match = 0, n_cols = 0, ref_start = 0;
+    uint32_t nops = 0;
+    int cur_op = -1; uint32_t cur_len = 0;
+    bool bad = false;
+    auto emit = [&](int op, uint32_t len) {
+        if (op == cur_op) { cur_len += len; return; }
+        if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
+        cur_op = op; cur_len = len;
+    };
+
+    if constexpr (W_ == 0) {
+        // gapless: every co-optimal alignment is ungapped, so the CIGAR is nM
+        ref_start = i_end - n;
+        if (ref_start < 0) { bad = true; ref_start = 0; }
+        for (int j0 = 0; j0 < n; j0 += 16) {
+            const uint32_t r = bases16(b.reads_packed, (long long)roff + j0, rwords);
+            const uint32_t t = bases16(b.wins_packed, (long long)woff + ref_start + j0, wwords);
+            const uint32_t nm = nbits16_spread(b.read_nmask, (long long)roff + j0, rnwords) |
+                                nbits16_spread(b.win_nmask, (long long)woff + ref_start + j0, wnwords);
+            uint32_t eq = eq16(r, t, nm);
+            if (n - j0 < 16) eq &= (1u << (2 * (n - j0))) - 1u;
+            n_match += __popc(eq);
+        }
+        n_cols = n;
+        emit(0, (uint32_t)n);
+    } else {
+        const int c = i_end - n;
+        const int i_lo = max(0, c - W_);
+        const int R = i_end - i_lo;
+        uint32_t lbits[MAXROWS * WPR];
+        int Hc[BW + 1], Fc[BW + 1];
+        {   // row i_lo of the restricted problem: M(i_lo, 0) = 0, M(i_lo, j) = -(o + e j) (drift form: -o)
+            const int jb0 = i_lo - c - W_;
+#pragma unroll
+            for (int jj = 0; jj <= BW; ++jj) {
+                const int j = jj + jb0;
+                Hc[jj] = (jj == BW || j < 0 || j > n) ? TNEG : (j == 0 ? 0 : tc.negOe - 1);
+                Fc[jj] = TNEG + 2;
+            }
+        }
+        // sliding 32-base buffers of the read (bases and spread N bits), refilled every 16 rows
+        long long q0 = (long long)(i_lo + 1 - c - W_) - 1;            // read position of segment bit 0 at row i_lo+1
+        uint64_t rbuf = (uint64_t)bases16(b.reads_packed, (long long)roff + q0, rwords) |
+                        ((uint64_t)bases16(b.reads_packed, (long long)roff + q0 + 16, rwords) << 32);
+        uint64_t rnbuf = 0;
+        if (b.read_nmask != nullptr)
+            rnbuf = (uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0, rnwords) |
+                    ((uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0 + 16, rnwords) << 32);
+        int roffs = 0;                                                // bases consumed from the buffer
+        uint32_t tw = 0, twn = 0;
+        int finH = TNEG;
+
+        auto row = [&](const int ir, auto check_tag) {
+            constexpr bool CHECK = decltype(check_tag)::value;
+            const int i = i_lo + ir;
+            const int jb = i - c - W_;
+            const uint64_t tpos = woff + (uint64_t)(i - 1);
+            if (ir == 1 || (tpos & 15u) == 0) tw = __ldg(b.wins_packed + (tpos >> 4));
+            const uint32_t t = (tw >> (2u * ((uint32_t)tpos & 15u))) & 3u;
+            uint32_t nm = 0;
+            if (b.win_nmask != nullptr) {
+                if (ir == 1 || (tpos & 31u) == 0) twn = __ldg(b.win_nmask + (tpos >> 5));
+                if ((twn >> ((uint32_t)tpos & 31u)) & 1u) nm = 0x55555555u;
+            }
+            if (roffs == 16) {
+                q0 += 16; roffs = 0;
+                rbuf = (rbuf >> 32) | ((uint64_t)bases16(b.reads_packed, (long long)roff + q0 + 16, rwords) << 32);
+                if (b.read_nmask != nullptr)
+                    rnbuf = (rnbuf >> 32) | ((uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0 + 16, rnwords) << 32);
+            }
+            const uint32_t seg = (uint32_t)(rbuf >> (2 * roffs));
+            nm |= (uint32_t)(rnbuf >> (2 * roffs));
+            ++roffs;
+            const uint32_t eqw = eq16(seg, t * 0x55555555u, nm);
+
+            int Hl = TNEG, El = TNEG;
+            uint32_t acc[WPR];
+#pragma unroll
+            for (int w = 0; w < WPR; ++w) acc[w] = 0u;
+#pragma unroll
+            for (int jj = 0; jj < BW; ++jj) {
+                int Ft = __viaddmax_s32(Hc[jj + 1], tc.negOf, Fc[jj + 1]);
+                int Et = __viaddmax_s32(Hl, tc.negOe, El);
+                const int q = ((eqw >> (2 * jj)) & 1u) ? tc.qm : tc.qx;
+                int Ht = __vimax3_s32(Hc[jj] + q, Ft, Et);
+                if (CHECK) {
+                    const int j = jb + jj;
+                    if (j < 1 || j > n) { Ht = (j == 0) ? tc.e8 * ir : TNEG; Ft = TNEG + 2; Et = TNEG; }
+                }
+                const int Hn = Ht & ~7, Fn = Ft & ~4, En = Et & ~1;
+                const uint32_t nib = (uint32_t)(((Ht & 3) | (Ft & 4)) + 8 * (Et - En));
+                acc[jj >> 3] |= nib << (4 * (jj & 7));
+                Hc[jj] = Hn; Fc[jj] = Fn; Hl = Hn; El = En;
+                if (CHECK) { if (jb + jj == n) finH = Hn; }
+            }
+#pragma unroll
+            for (int w = 0; w < WPR; ++w) lbits[(ir - 1) * WPR + w] = acc[w];
+        };
+
+        // rows whose band touches column 0 or column n+1 take the checked variant
+        const int ir_a = min(R, max(0, c + W_ + 1 - i_lo - 1));        // last row with jb < 1
+        const int ir_b = max(ir_a, min(R, c - W_ + n - i_lo));         // last row with jb + BW - 1 <= n
+        int ir = 1;
+        for (; ir <= ir_a; ++ir) row(ir, std::true_type{});
+        for (; ir <= ir_b; ++ir) row(ir, std::false_type{});
+        for (; ir <= R; ++ir) row(ir, std::true_type{});
+        // the band DP must end on the forward score: H'(R, n) = 8 (S + e (R + n))
+        if ((finH >> 3) - (tc.e8 >> 3) * (R + n) != tp.score[p]) bad = true;
+
+        // walk back from (i_end, n)
+        int i = i_end, j = n, st = 0;                                  // 0 = H, 1 = D, 2 = I
+        while (j > 0) {
+            if (i == i_lo) { emit(1, (uint32_t)j); n_cols += j; j = 0; break; }
+            const int jj = j - (i - c - W_);
+            if (jj < 0 || jj >= BW) { bad = true; break; }
+            const uint32_t f = (lbits[(i - i_lo - 1) * WPR + (jj >> 3)] >> (4 * (jj & 7))) & 15u;
+            if (st == 0) {
+                if ((f & 3u) == 3u) {
+                    emit(0, 1u); ++n_cols;
+                    n_match += (base_at(b.reads_packed, b.read_nmask, roff + (uint64_t)(j - 1), SDP_CODE_READ_N) ==
+                                base_at(b.wins_packed, b.win_nmask, woff + (uint64_t)(i - 1), SDP_CODE_WIN_N));
+                    --i; --j;
+                } else if ((f & 3u) == 2u) st = 1;
+                else st = 2;
+            } else if (st == 1) {
+                emit(2, 1u); ++n_cols;
+                if (f & 4u) st = 0;
+                --i;
+            } else {
+                emit(1, 1u); ++n_cols;
+                if (f & 8u) st = 0;
+                --j;
+            }
+        }
+        ref_start = i;
+    }
+    emit(-2, 0u);                                          // flush the last run
+    if (bad) { atomicOr(tp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
+    tp.ref_start[p] = ref_start;
+    tp.read_start[p] = 0;
+    tp.read_end[p] = n - 1;
+    tp.n_match[p] = n_match;
+    tp.n_cols[p] = n_cols;
+    tp.cigar_len[p] = nops;
+    tp.pass[p] = ((long long)n_match * 1000000LL >= tp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
+}
+
+void launch_thin(int W, const TraceParams& tp, cudaStream_t st)
+{
+    if (tp.count == 0) return;
+    ThinConsts tc;
+    const int o = tp.sc.gap_open, e = tp.sc.gap_extend;
+    tc.negOe = -8 * o + 1; tc.negOf = -8 * o + 6;
+    tc.qm = 8 * (2 * e + tp.sc.match) + 7; tc.qx = 8 * (2 * e + tp.sc.mismatch) + 7; tc.e8 = 8 * e;
+    const uint32_t grid = (tp.count + 127) / 128;
+    switch (W) {
+        case 0: k_thin<0, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 1: k_thin<1, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 2: k_thin<2, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 3: k_thin<3, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 4: k_thin<4, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 5: k_thin<5, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        case 6: k_thin<6, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+        default: k_thin<7, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+    }
+}
+
+}  // namespace sdp

@@ -31,6 +31,7 @@ __device__ __forceinline__ int tb_class_of(int bw) {
     static_assert(TB_NCLASS == 4, "update tb_class_of");
     return bw > 256 ? 3 : (bw > 64 ? 2 : (bw > 16 ? 1 : 0));
 }
+static_assert((THIN_NW + TB_NCLASS) * 4096 <= SDP_NBINS, "thin keys must fit the bucket-sort key space");
 
 __device__ __forceinline__ void hist_add(uint32_t* hist, uint32_t key, bool valid) {
     const uint32_t active = __ballot_sync(0xffffffffu, valid);
@@ -60,19 +61,24 @@ __global__ void k_post_forward(const PostParams pp)
             bw = min(2 * W + 1, n + 1);
         }
         pp.tb_rows[p] = rows;
-        // wide pairs: the register-resident wavefront recomputes the whole rectangle rows x n
-        // (trace_kernel.cuh) when its x8 scaled values fit 16 bits; the reverse pass first trims
-        // the rectangle's rows. Narrow bands and everything else: one thread per pair.
+        // Three paths. Narrow: W <= 7 and a real band -> one thread per pair,
+        // band in registers (thin_kernel.cu). Wide: the register-resident wavefront recomputes the
+        // whole rectangle rows x n (trace_kernel.cuh) when its x8 scaled values fit 16 bits; the
+        // reverse pass first trims the rectangle's rows. Anything else: the generic band kernel.
         const long long vmax = (long long)pp.sc.match * n + (long long)pp.sc.gap_extend * (n + rows) +
                                3LL * pp.sc.gap_open + 8;
-        const bool wide = W > 0 && pp.wide_ok && bw > pp.wide_min_bw && vmax <= SDP_TB_MAX_VALUE;
-        if (wide) {
+        const bool narrow = W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && !pp.no_thin);
+        const bool wide = !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
+        if (narrow) {
+            ktb = (uint32_t)W * 4096u + (uint32_t)min(4095, W ? rows : n);
+            c_tb = (unsigned long long)bw * rows;
+        } else if (wide) {
             krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
             kwide = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, (rows + 7) >> 3);
             c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
         } else {
-            if (W > 0) { words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows; }
-            ktb = (uint32_t)tb_class_of(bw) * 8192u + (uint32_t)min(bw, 8191);
+            words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows;
+            ktb = (uint32_t)(THIN_NW + tb_class_of(bw)) * 4096u + (uint32_t)min(bw, 4095);
         }
         pp.keys_rev[p] = krev;
         pp.keys_wide[p] = kwide;
