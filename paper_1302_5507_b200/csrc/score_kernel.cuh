@@ -14,16 +14,21 @@
 //    s - g at step s (anti-diagonal wavefront); H and E of the chunk's last column cross to the
 //    right neighbour with one warp shuffle each per row.
 //  * drift form: stored values are H + e*(i+j) + beta, so gap extension needs no add:
-//        E' = max(H'(i,j-1) - o, E'(i,j-1))          1 VIADDMNMX.S16x2   (on the row's serial chain)
-//        F' = max(H'(i-1,j) - o, F'(i-1,j))          1 VIADDMNMX.S16x2   (off the chain)
-//        t  = max(H'(i-1,j-1) + (2e+mismatch), F')   1 VIADDMNMX.S16x2   (off the chain)
-//        H' = max3(H'(i-1,j-1) + q, t, E')           1 VIMNMX3.S16x2     (on the chain)
-//    where q = (2e+match) when the bases are equal and a large negative number otherwise. q comes
-//    from the otherwise idle FMA pipe: base codes are fp16 values, d = r - t (HADD2),
-//    q = fma(d, -d, C) (HFMA2) with C the fp16 DENORMAL whose bit pattern is the integer 2e+match;
-//    d == 0 gives exactly C, d != 0 gives a negative half whose bit pattern read as int16 is below
-//    -15000. The add H' + q is a 32-bit IMAD (no carry crosses the lanes because every stored
-//    value is in [0, 16000]). Four ALU-pipe instructions per two cells.
+//        E' = max(H'(i,j-1) - o, E'(i,j-1))          VIADDMNMX.S16x2   (on the row's serial chain)
+//        F' = max(H'(i-1,j) - o, F'(i-1,j))          VIADDMNMX.S16x2   (off the chain)
+//        u  = max(H'(i-1,j-1) + q, F')               VIADDMNMX.S16x2   (off the chain)
+//        H' = max(u, E')                             VIMNMX.S16x2      (on the chain)
+//    with q = 2e + delta(T[i], R[j]) EXACT: 2e+match or 2e+mismatch. Four ALU-pipe instructions per
+//    two cells. q comes from the FMA pipe, which runs beside the ALU pipe (measured: DESIGN.md
+//    "Pipes"): base codes are fp16 values at least 1 apart, d = t - r (HADD2),
+//    g = sat(1 - d*d) (HFMA2.SAT: 1.0 iff the bases are equal, else 0.0), q = g*Cd + Cy (HFMA2) with
+//    Cd, Cy the fp16 DENORMALS whose bit patterns are the integers (match - mismatch) and
+//    (2e + mismatch): the result's bit pattern IS the integer q. This needs 2e + mismatch >= 0
+//    (EXACT variant). Otherwise (general variant) q = Cf - d*d with Cf the denormal 2e+match: d == 0
+//    gives exactly Cf, d != 0 a negative half whose bits read as int16 are below -15000, and the
+//    mismatch candidate costs a fifth instruction t = max(H'(i-1,j-1) + (2e+mismatch), F').
+//    No integer multiply-add and no register move is wanted in the loop: IMAD and IMAD.MOV issue at
+//    a quarter of the HFMA2 rate on sm_100a (measured) and starve the FMA pipe.
 //  * window rows: the 2-bit window bases of both lanes are expanded once per chunk of rows into
 //    a per-group shared-memory ring of 16-bit PRMT selectors; a row then costs one LDS.U16 and one
 //    PRMT to obtain the fp16 codes of both lanes (instead of two address computations, two global
@@ -35,28 +40,39 @@
 
 namespace sdp {
 
-// fp16 code bytes: value byte T[c] for c = A,C,G,T, read-N (4), window-N (5). A base code is the
-// half whose two bytes are (T[c]^0x80, T[c]) on the read side and (T[c], T[c]) on the window side,
-// i.e. exact negatives of each other; all six magnitudes differ by >= 0.125 and are <= 1.94.
-#define SDP_TBL_LO 0xBFBEBDBCu      // PRMT source a: bytes 0..3 = A C G T
-#define SDP_TBL_HI 0x0000BBBAu      // PRMT source b: byte 4 = read N, byte 5 = window N
+// fp16 codes: the half whose two bytes both equal B[c], for c = A,C,G,T, read-N (4), window-N (5):
+// 0x3C3C = 1.059, 0x4040 = 2.125, 0x4242 = 3.129, 0x4444 = 4.266, 0x4545 = 5.270, 0x4646 = 6.273.
+// Any two differ by more than 1 and every difference is exact in fp16, so d*d >= 1 unless the
+// bases are equal. Read-N and window-N have different codes: N never matches, not even N.
+#define SDP_TBL_LO 0x4442403Cu      // PRMT source a: bytes 0..3 = A C G T
+#define SDP_TBL_HI 0x00004645u      // PRMT source b: byte 4 = read N, byte 5 = window N
 
 __device__ __forceinline__ uint32_t read_code_half(uint32_t c) {      // c in 0..4
-    const uint32_t t = (c < 4u) ? (0xBCu + c) : 0xBAu;
-    return ((t ^ 0x80u) << 8) | t;
+    const uint32_t t = __byte_perm(SDP_TBL_LO, SDP_TBL_HI, c);
+    return (t & 0xFFu) * 0x0101u;
 }
 
-__device__ __forceinline__ uint32_t hadd2_u(uint32_t a, uint32_t b) {
-    uint32_t d; asm("add.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d;
+__device__ __forceinline__ uint32_t hsub2_u(uint32_t a, uint32_t b) {
+    uint32_t d; asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d;
 }
-// fma(d, -d, c) per fp16 lane; non-ftz so the denormal addend survives
+// c - d*d per fp16 lane; non-ftz so a denormal addend survives
 __device__ __forceinline__ uint32_t hfma2_negsq(uint32_t d, uint32_t c) {
     uint32_t r;
     asm("{.reg .b32 nd; neg.f16x2 nd, %1; fma.rn.f16x2 %0, %1, nd, %2;}" : "=r"(r) : "r"(d), "r"(c));
     return r;
 }
-__device__ __forceinline__ uint32_t imad_add(uint32_t one, uint32_t a, uint32_t b) {
-    uint32_t r; asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(one), "r"(a), "r"(b)); return r;
+// sat(1 - d*d) per fp16 lane: 1.0 when d == 0, 0.0 when |d| >= 1
+__device__ __forceinline__ uint32_t hfma2_is_zero(uint32_t d) {
+    uint32_t r;
+    asm("{.reg .b32 nd, on; neg.f16x2 nd, %1; mov.b32 on, 0x3C003C00; fma.rn.sat.f16x2 %0, %1, nd, on;}"
+        : "=r"(r) : "r"(d));
+    return r;
+}
+__device__ __forceinline__ uint32_t hfma2_u(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r; asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c)); return r;
+}
+__device__ __forceinline__ uint32_t add_s16x2(uint32_t a, uint32_t b) {
+    uint32_t r; asm("add.s16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b)); return r;
 }
 // max per int16 lane plus, per lane, whether a >= b. Same PTX as CUDA's __vibmax_s16x2 but with an
 // early-clobber output: the header's "=r" lets the result share a's register, which turns the
@@ -183,12 +199,20 @@ __device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingG
     }
 }
 
+// Rows per iteration of the steady-state loop (even). ptxas pays ~45 register moves per loop
+// iteration to bring the loop-carried H/F registers back to their entry assignment, and a move
+// (IMAD.MOV) costs as much FMA-pipe time as two HFMA2: unrolling amortises them.
+#ifndef SDP_ROWS_UNROLL
+#define SDP_ROWS_UNROLL 8
+#endif
+
 // resident CTAs per SM the register budget is sized for: 128 registers up to K = 21, 168 above
 #ifndef SDP_SCORE_MIN_CTAS
 #define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)
 #endif
 
-template <int K, bool REV, bool PAD>
+// EXACT: 2e + mismatch >= 0, the four-instruction recurrence; otherwise the general five-instruction one
+template <int K, bool REV, bool PAD, bool EXACT>
 __global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))
 score_kernel(const ScoreParams P)
 {
@@ -261,7 +285,7 @@ score_kernel(const ScoreParams P)
         if (in_group) fill_ring_rows<REV>(P, rg, ring_w, g, G, s0, dA.woff, mA, dB.woff, mB);
     };
 
-    const uint32_t one = P.c.one, negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, e2 = P.c.e2;
+    const uint32_t negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, Cd = P.c.Cd, e2 = P.c.e2;
     const uint32_t notfirst = is_first ? 0u : 0xFFFFFFFFu;
     // boundary column 0 as seen by the group's first thread: H'(i,0) = beta + e*i (forward, free
     // start) or beta - o (reverse, start anchored: a leading deletion of i bases costs o + e*i)
@@ -289,28 +313,27 @@ score_kernel(const ScoreParams P)
         fv = __vadd2(fv, fstep);
         hin = (hin & notfirst) | fv;
         ein = ein & notfirst;
-        // negated fp16 codes of the window bases of row i, both lanes
+        // fp16 codes of the window bases of row i, both lanes
         const uint32_t nt = __byte_perm(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
 
         uint32_t Hl = hin, E = ein;
         uint32_t Hsk = hin, Esk = ein;                    // outputs if the last column is skipped
-        uint32_t t1;
-        Hn[0] = imad_add(one, hdiag, hfma2_negsq(hadd2_u(rh[0], nt), Cf));
-        F[0] = __viaddmax_s16x2(Hs[0], negO, F[0]);
-        t1 = __viaddmax_s16x2(hdiag, cmis, F[0]);
+        // u[k] = max(H'(i-1,k-1) + q, F'(i,k)): everything of column k that does not wait for the chain
+        auto off_chain = [&](const int k, const uint32_t hd) -> uint32_t {
+            const uint32_t d = hsub2_u(nt, rh[k]);
+            F[k] = __viaddmax_s16x2(Hs[k], negO, F[k]);
+            if (EXACT) return __viaddmax_s16x2(hd, hfma2_u(hfma2_is_zero(d), Cd, cmis), F[k]);
+            const uint32_t t = __viaddmax_s16x2(hd, cmis, F[k]);
+            return __viaddmax_s16x2(hd, hfma2_negsq(d, Cf), t);
+        };
+        Hn[0] = off_chain(0, hdiag);
         hdiag = hin;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            uint32_t t1_n = 0u;
-            if (k + 1 < K) {                              // off-chain work of column k+1
-                Hn[k + 1] = imad_add(one, Hs[k], hfma2_negsq(hadd2_u(rh[k + 1], nt), Cf));
-                F[k + 1] = __viaddmax_s16x2(Hs[k + 1], negO, F[k + 1]);
-                t1_n = __viaddmax_s16x2(Hs[k], cmis, F[k + 1]);
-            }
+            if (k + 1 < K) Hn[k + 1] = off_chain(k + 1, Hs[k]);
             E = __viaddmax_s16x2(Hl, negO, E);
-            Hl = __vimax3_s16x2(Hn[k], t1, E);
+            Hl = __vmaxs2(Hn[k], E);
             Hn[k] = Hl;
-            t1 = t1_n;
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }
         if (PAD) { hout = blend(skipmask, Hsk, Hl); eout = blend(skipmask, Esk, E); }
@@ -357,12 +380,16 @@ score_kernel(const ScoreParams P)
         for (; s <= min(send, G - 1); ++s, ++rp) row_step1(s - g, rp, std::true_type{});
         const int fe = min(send, fast_end);
 #pragma unroll 1
-        for (; s + 1 <= fe; s += 2, rp += 2) {
+        for (; s + SDP_ROWS_UNROLL - 1 <= fe; s += SDP_ROWS_UNROLL, rp += SDP_ROWS_UNROLL) {
             uint32_t H2[K];
-            row_step(s - g, rp, std::false_type{}, H, H2);
-            row_step(s + 1 - g, rp + 1, std::false_type{}, H2, H);
+#pragma unroll
+            for (int r = 0; r < SDP_ROWS_UNROLL; r += 2) {
+                row_step(s + r - g, rp + r, std::false_type{}, H, H2);
+                row_step(s + r + 1 - g, rp + r + 1, std::false_type{}, H2, H);
+            }
         }
-        if (s <= fe) { row_step1(s - g, rp, std::false_type{}); ++s; ++rp; }
+#pragma unroll 1
+        for (; s <= fe; ++s, ++rp) row_step1(s - g, rp, std::false_type{});
 #pragma unroll 1
         for (; s <= send; ++s, ++rp) row_step1(s - g, rp, std::true_type{});
     }
@@ -384,16 +411,19 @@ score_kernel(const ScoreParams P)
 }
 
 template <int K>
-static void launch_score_K(bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
+static void launch_score_K(bool pad, bool rev, bool exact, const ScoreParams& p, cudaStream_t st) {
     const uint32_t ntasks = p.task_end - p.task_begin;
     if (ntasks == 0) return;
     const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
-    if (rev) {
-        if (pad) score_kernel<K, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-        else     score_kernel<K, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+    if (!exact) {                                         // general scoring: the padded variant serves every length
+        if (rev) score_kernel<K, true, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        else     score_kernel<K, false, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+    } else if (rev) {
+        if (pad) score_kernel<K, true, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        else     score_kernel<K, true, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
     } else {
-        if (pad) score_kernel<K, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-        else     score_kernel<K, false, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        if (pad) score_kernel<K, false, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        else     score_kernel<K, false, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
     }
 }
 

@@ -144,12 +144,16 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
 void choose_geometry(sdp_ctx* c) {
     struct Ent { uint16_t n, G, K, pad; };
     Ent ents[SDP_NSLOTS];
+    int force_g = 0;                                  // SDP_FORCE_G: tuning experiments only
+    if (const char* v = getenv("SDP_FORCE_G")) force_g = atoi(v);
     for (int n = 1; n <= SDP_NSLOTS; ++n) {
         double best = -1; int bG = 32, bK = (n + 31) / 32;
         for (int G = 1; G <= 32; ++G) {
             int K = (n + G - 1) / G;
             if (K > SDP_MAX_K) continue;
             if (G * K - n >= G) continue;
+            if (force_g && G != force_g && (n + force_g - 1) / force_g <= SDP_MAX_K &&
+                force_g * ((n + force_g - 1) / force_g) - n < force_g) continue;
             double ppw = 2.0 * (32 / G);
             double rows = (double)n + 300.0 + G - 1;
             double thr = ppw / (rows * (4.0 * K + 11.0 + (G * K != n ? 4.0 : 0.0)));
@@ -196,10 +200,12 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     ctx->user_sc = *s;
     ctx->sc = Scoring{s->match, s->mismatch, s->gap_open, s->gap_extend, llround(s->min_similarity * 1e6)};
     const int o = s->gap_open, e = s->gap_extend, beta = 3 * o + 8;
-    ctx->consts.one = 1u;
+    ctx->consts.exact = (2 * e + s->mismatch >= 0) ? 1u : 0u;
+    if (const char* v = getenv("SDP_NO_EXACT")) { if (atoi(v)) ctx->consts.exact = 0u; }
     ctx->consts.negO = sdp_pack2(-o);
     ctx->consts.cmis = sdp_pack2(2 * e + s->mismatch);
     ctx->consts.Cf = sdp_pack2(2 * e + s->match);
+    ctx->consts.Cd = sdp_pack2(s->match - s->mismatch);
     ctx->consts.e2 = sdp_pack2(e);
     ctx->consts.beta2 = sdp_pack2(beta);
     ctx->consts.betaMinusO2 = sdp_pack2(beta - o);

@@ -19,7 +19,7 @@
 #define SDP_ERRF_RANGE   4u     // int16 range rule or SDP_MAX_READ_LEN broken
 #define SDP_ERRF_TRACE   8u     // traceback left its band or overflowed its run buffer (internal)
 
-// fp16 code of base c (0..3 = ACGT, 4 = read N, 5 = window N): 1.0 + 0.25*c, exact in fp16
+// code index of the two N kinds (0..3 = ACGT); fp16 values in score_kernel.cuh
 #define SDP_CODE_READ_N 4u
 #define SDP_CODE_WIN_N 5u
 
@@ -44,10 +44,11 @@ struct SlotInfo {
 };
 
 struct ScoreConsts {
-    uint32_t one;      // 1, opaque to the compiler (keeps the 32-bit add on the FMA pipe as IMAD)
+    uint32_t exact;    // 2e + mismatch >= 0: the exact-delta (four-instruction) score kernels apply
     uint32_t negO;     // packed (-o, -o)
     uint32_t cmis;     // packed (2e + mismatch)
     uint32_t Cf;       // packed fp16 bit pattern == integer (2e + match), a denormal
+    uint32_t Cd;       // packed fp16 bit pattern == integer (match - mismatch), a denormal
     uint32_t e2;       // packed (e, e)
     uint32_t beta2;    // packed (beta, beta)
     uint32_t betaMinusO2;

@@ -134,7 +134,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         uint32_t acc = 0u;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const uint32_t sel = hfma2_negsq(hadd2_u(rh[k], nt), Cf);
+            const uint32_t sel = hfma2_negsq(hsub2_u(nt, rh[k]), Cf);
             const uint32_t dq = __vmaxs2(sel, qx);
             const uint32_t dg = imad_u(one, hd, dq);
             hd = Hs[k];

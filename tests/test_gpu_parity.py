@@ -176,6 +176,20 @@ def test_other_scorings(sc):
         c.destroy()
 
 
+def test_general_score_kernel_with_default_scoring(monkeypatch):
+    # SDP_NO_EXACT=1 (read by sdp_create) sends the default scoring through the general five-instruction
+    # score kernels that scorings with 2*extend + mismatch < 0 use; results must not change
+    monkeypatch.setenv("SDP_NO_EXACT", "1")
+    c = make_ctx(DEFAULT)
+    try:
+        parity.check_batch(c, W.make_config(2, n_pairs=1500, ref_bases=500_000), DEFAULT, "general kernels cfg2",
+                           host_path=False)
+        parity.check_batch(c, W.make_config(5, n_pairs=3000, ref_bases=500_000), DEFAULT, "general kernels cfg5",
+                           host_path=False)
+    finally:
+        c.destroy()
+
+
 def test_mixed_window_lengths_in_one_warp(ctx):
     # same read length, window lengths from 1 to 900 in one batch: lanes of a warp finish at
     # different rows (the masked tail loop of the score kernel)
