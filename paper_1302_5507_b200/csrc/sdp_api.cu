@@ -74,6 +74,8 @@ struct sdp_ctx {
     uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr, *d_slot_of_n = nullptr;
     Mailbox* mb = nullptr;
     cudaStream_t own_stream = nullptr;
+    cudaStream_t side_stream = nullptr;   // narrow-band traceback runs here, beside the wide path on the caller's stream
+    cudaEvent_t side_done = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     // fixed-size device buffers
     uint32_t* hist[4] = {};          // forward, reverse, thin traceback, wide traceback
@@ -244,10 +246,12 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaMallocHost(&ctx->mb, sizeof(Mailbox)));
         memset(ctx->mb, 0, sizeof(Mailbox));
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
         for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
         for (int i = 0; i < 4; ++i) {
             CU(cudaMalloc(&ctx->hist[i], (SDP_NBINS + 1) * 4));
-            CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 1) * 4));
+            CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 4 + SDP_BIN_SCRATCH) * 4));
         }
         for (int i = 0; i < 3; ++i) {
             CU(cudaMalloc(&ctx->slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
@@ -285,6 +289,8 @@ void sdp_destroy(sdp_ctx* ctx)
     cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K); cudaFree(ctx->d_slot_of_n);
     if (ctx->mb) cudaFreeHost(ctx->mb);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
+    if (ctx->side_done) cudaEventDestroy(ctx->side_done);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
 }
@@ -392,7 +398,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
                         ctx->hist[0], ctx->err_flag, ctx->counters + 3, st);
     launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0], st);
-    nl += 4;
+    nl += 5;
     CU(cudaMemcpyAsync(ctx->mb->task_prefix[0], ctx->task_prefix[0], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[0], ctx->bin_start[0] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
@@ -431,7 +437,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
                      nullptr, nullptr, nullptr, nullptr, nullptr, st);
     launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2], st);
-    nl += 9;
+    nl += 12;
     // one region of direction nibbles per two wide pairs that share the int16x2 lanes (every slot of
     // order_wide beyond the wide pairs reads as a zero-size region)
     CU(cudaMemsetAsync(ctx->wide_words.p, 0, P * 4, st));
@@ -462,6 +468,30 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
     EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
     EN(wide_bits, (ctx->mb->totals[3] + 4) * 4);
+
+    // ---- a5 + a6, narrow bands (W <= 7: one thread per pair, band in registers) and the generic band kernel.
+    // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on a
+    // side stream beside it (the stream synchronisation above has completed everything they read).
+    cudaStream_t ss = ctx->side_stream;
+    TraceParams tp{};
+    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
+    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
+    tp.rev_rows = nullptr;
+    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
+    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
+    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
+    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
+    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
+    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
+    if (launch_thin_all(ctx->mb->tb_bounds, tp, ss)) ++nl;
+    for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
+        tp.first = ctx->mb->tb_bounds[c];
+        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
+        if (!tp.count) continue;
+        launch_traceback(c - THIN_NW, tp, ss);
+        ++nl;
+    }
+    CU(cudaEventRecord(ctx->side_done, ss));
 
     // ---- a4 reverse pass over the pairs whose score admits a gap
     launch_fill_desc_rev(b, ctx->order_rev.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
@@ -494,24 +524,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         launch_walk(wp, st);
         ++nl;
     }
-    // narrow bands (W <= 7): one thread per pair, band in registers; leftovers: generic band kernel
-    TraceParams tp{};
-    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
-    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
-    tp.rev_rows = nullptr;
-    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
-    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
-    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
-    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
-    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
-    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    for (int c = 0; c < THIN_NW + TB_NCLASS; ++c) {
-        tp.first = ctx->mb->tb_bounds[c];
-        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
-        if (!tp.count) continue;
-        if (c < THIN_NW) launch_thin(c, tp, st); else launch_traceback(c - THIN_NW, tp, st);
-        ++nl;
-    }
+    CU(cudaStreamWaitEvent(st, ctx->side_done, 0));
     CU(cudaGetLastError());
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
 

@@ -86,7 +86,7 @@ void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st);
 // narrow bands (thin_kernel.cu): one launch per gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
 constexpr int THIN_NW = 8;
 constexpr int THIN_MAXROWS = 336;
-void launch_thin(int W, const TraceParams& tp, cudaStream_t st);
+bool launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st);   // false: nothing to do
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 

@@ -9,6 +9,7 @@
 #define SDP_SCORE_THREADS (32 * SDP_WARPS_PER_CTA)
 #define SDP_MAX_K 32            // columns of the read one thread keeps in registers
 #define SDP_NBINS 65536         // bucket-sort key space: (n-1) * 64 + min(63, rows >> 6)
+#define SDP_BIN_SCRATCH 60      // words behind bin_start[SDP_NBINS] the bin scan may use
 #define SDP_NSLOTS 1024         // one slot per read length 1..SDP_MAX_READ_LEN
 #define SDP_RING_WORDS 1792     // shared-memory words per warp for the window-row selector rings
 #define SDP_KEY_SKIP 0xFFFFFFFFu

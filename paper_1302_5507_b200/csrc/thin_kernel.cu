@@ -64,13 +64,13 @@ struct ThinConsts {
 // W_ = gap-content bound of every pair of the launch (0 = gapless). MAXROWS bounds the rows of the
 // band (n + W); pairs beyond it are classified onto the other paths by k_post_forward.
 template <int W_, int MAXROWS>
-__global__ void __launch_bounds__(128) k_thin(const TraceParams tp, const ThinConsts tc)
+__device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConsts& tc, const uint32_t first,
+                                          const uint32_t count, const uint32_t k)
 {
     constexpr int BW = 2 * W_ + 1;                 // band columns
     constexpr int WPR = (BW + 7) / 8;              // 32-bit words of direction nibbles per row
-    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= tp.count) return;
-    const uint32_t p = tp.order[tp.first + k];
+    if (k >= count) return;
+    const uint32_t p = tp.order[first + k];
     const sdp_batch& b = tp.b;
     const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
     const int n = (int)b.read_len[ri];
@@ -228,24 +228,48 @@ __global__ void __launch_bounds__(128) k_thin(const TraceParams tp, const ThinCo
     tp.pass[p] = ((long long)n_match * 1000000LL >= tp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
 }
 
-void launch_thin(int W, const TraceParams& tp, cudaStream_t st)
+// All gap bounds W = 0..THIN_NW-1 in ONE launch: block b serves class w with
+// r.block_start[w] <= b < r.block_start[w+1] (seven small launches in a row left the GPU mostly idle).
+struct ThinRanges { uint32_t first[THIN_NW], count[THIN_NW], block_start[THIN_NW + 1]; };
+
+__global__ void __launch_bounds__(128) k_thin_all(const TraceParams tp, const ThinConsts tc, const ThinRanges r)
 {
-    if (tp.count == 0) return;
+    int w = 0;
+#pragma unroll
+    for (int c = 1; c < THIN_NW; ++c) w += (blockIdx.x >= r.block_start[c]) ? 1 : 0;
+    const uint32_t k = (blockIdx.x - r.block_start[w]) * blockDim.x + threadIdx.x;
+    switch (w) {                                           // block-uniform
+        case 0: thin_body<0, THIN_MAXROWS>(tp, tc, r.first[0], r.count[0], k); break;
+        case 1: thin_body<1, THIN_MAXROWS>(tp, tc, r.first[1], r.count[1], k); break;
+        case 2: thin_body<2, THIN_MAXROWS>(tp, tc, r.first[2], r.count[2], k); break;
+        case 3: thin_body<3, THIN_MAXROWS>(tp, tc, r.first[3], r.count[3], k); break;
+        case 4: thin_body<4, THIN_MAXROWS>(tp, tc, r.first[4], r.count[4], k); break;
+        case 5: thin_body<5, THIN_MAXROWS>(tp, tc, r.first[5], r.count[5], k); break;
+        case 6: thin_body<6, THIN_MAXROWS>(tp, tc, r.first[6], r.count[6], k); break;
+        default: thin_body<7, THIN_MAXROWS>(tp, tc, r.first[7], r.count[7], k); break;
+    }
+}
+
+// bounds[w] .. bounds[w+1]: range of tp.order that holds the pairs with gap bound w
+bool launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st)
+{
+    static_assert(THIN_NW == 8, "update k_thin_all");
     ThinConsts tc;
     const int o = tp.sc.gap_open, e = tp.sc.gap_extend;
     tc.negOe = -8 * o + 1; tc.negOf = -8 * o + 6;
     tc.qm = 8 * (2 * e + tp.sc.match) + 7; tc.qx = 8 * (2 * e + tp.sc.mismatch) + 7; tc.e8 = 8 * e;
-    const uint32_t grid = (tp.count + 127) / 128;
-    switch (W) {
-        case 0: k_thin<0, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 1: k_thin<1, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 2: k_thin<2, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 3: k_thin<3, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 4: k_thin<4, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 5: k_thin<5, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        case 6: k_thin<6, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
-        default: k_thin<7, THIN_MAXROWS><<<grid, 128, 0, st>>>(tp, tc); break;
+    ThinRanges r;
+    uint32_t blocks = 0;
+    // heaviest classes first, so that the long-running blocks do not form the tail of the launch
+    for (int w = 0; w < THIN_NW; ++w) {
+        r.first[w] = bounds[w]; r.count[w] = bounds[w + 1] - bounds[w];
+        r.block_start[w] = blocks;
+        blocks += (r.count[w] + 127) / 128;
     }
+    r.block_start[THIN_NW] = blocks;
+    if (blocks == 0) return false;
+    k_thin_all<<<blocks, 128, 0, st>>>(tp, tc, r);
+    return true;
 }
 
 }  // namespace sdp
