@@ -291,6 +291,10 @@ def main():
     sm_max = float(peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     peak = sms * sm_max * 1e6 * DPX_RATE * 2.0 / INSTR_PER_2_CELLS / 1e9
+    try:        # issue-rate microbenchmark of this very GPU, reported beside the constant the peak uses
+        dpx_live = S.sdp_measure_dpx_rate(local)
+    except Exception as ex:  # noqa: BLE001
+        dpx_live = {"error": str(ex)}
     fwd = cells / (statistics.mean(fwd_ms) * 1e-3) / 1e9 if fwd_ms and statistics.mean(fwd_ms) > 0 else None
     traffic = None
     try:
@@ -305,7 +309,7 @@ def main():
                             f"instr/clk/SM (measured, profiles/) x 2 cells / {INSTR_PER_2_CELLS:.0f} instr",
                 "achieved_how": "sum n*m of the batch / mean CUDA-event time of the forward-kernel launches per step, "
                                 "events recorded by libsdp on the launching stream inside the timed steps",
-                "whole_path_frac": value / world / peak}
+                "whole_path_frac": value / world / peak, "dpx_rate_measured_now": dpx_live}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

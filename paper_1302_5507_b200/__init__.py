@@ -4,9 +4,9 @@ The product is the C-ABI library ``libsdp.so`` (``include/sdp.h``) built from ``
 package is its thin Python binding plus the seeded input generators. There is no CPU fallback:
 every entry point raises if the CUDA library is missing.
 """
-__all__ = ["workloads"]
+__all__ = ["workloads", "shard"]
 
-from . import workloads  # noqa: E402,F401
+from . import shard, workloads  # noqa: E402,F401
 from .binding import (  # noqa: E402,F401
     Context,
     DeviceBatch,
