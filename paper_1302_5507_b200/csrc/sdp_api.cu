@@ -216,18 +216,18 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         const int sc8 = SDP_TB_SCALE;
         const int qm = sc8 * (2 * e + s->match) + 7, qx = sc8 * (2 * e + s->mismatch) + 7;
         TraceConsts& t = ctx->tconsts;
-        t.one = 1u; t.c16 = 16u; t.c8 = 8u; t.cm1 = 0xFFFFFFFFu; t.m4 = 0x00040004u;
+        t.m4 = 0x00040004u;
         t.negO_e = sdp_pack2(-sc8 * o + 1);
         t.negO_f = sdp_pack2(-sc8 * o + 6);
         t.qx = sdp_pack2(qx);
-        t.Cf = sdp_pack2(qm);
+        t.Cd8 = sdp_pack2(sc8 * (s->match - s->mismatch));
         t.e2 = sdp_pack2(sc8 * e);
         t.beta2 = sdp_pack2(sc8 * beta);
         t.betaMinusO2 = sdp_pack2(sc8 * (beta - o));
         t.e = e; t.beta = beta;
         // the diagonal increment is added with a 32-bit IMAD: it must be non-negative in both lanes,
         // and the match increment must stay an fp16 denormal bit pattern
-        ctx->wide_ok = (qx >= 0 && qm < 1024 && sc8 * beta <= 32000) ? 1 : 0;
+        ctx->wide_ok = (qx >= 0 && qm < 2048 && sc8 * beta <= 32000) ? 1 : 0;
         if (const char* v = getenv("SDP_NO_THIN")) ctx->no_thin = atoi(v);
         if (const char* v = getenv("SDP_NO_WIDE")) { if (atoi(v)) ctx->wide_ok = 0; }
     }
@@ -458,7 +458,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[1], ctx->bin_start[1] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->bin_total[3], ctx->bin_start[3] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
     for (int c = 0; c <= THIN_NW + TB_NCLASS; ++c)
-        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * 4096, 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * TB_KEY_STRIDE, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->mb->counters, ctx->counters, 4 * 8, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
@@ -483,7 +483,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
     tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
     tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    if (launch_thin_all(ctx->mb->tb_bounds, tp, ss)) ++nl;
+    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss);
     for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
         tp.first = ctx->mb->tb_bounds[c];
         tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;

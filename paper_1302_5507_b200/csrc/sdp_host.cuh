@@ -83,10 +83,12 @@ void launch_walk(const WalkParams& wp, cudaStream_t st);
 constexpr int TB_NCLASS = 4;
 constexpr int TB_CLASS_BW[TB_NCLASS] = {16, 64, 256, 1032};   // band <= min(2W+1, n+1) <= 1025
 void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st);
-// narrow bands (thin_kernel.cu): one launch per gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
-constexpr int THIN_NW = 8;
+// narrow bands (thin_kernel.cu): gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
+constexpr int THIN_NW = 24;
+constexpr int THIN_SPLIT = 8;             // classes below / from here on run in two launches (register budgets differ)
+constexpr uint32_t TB_KEY_STRIDE = 2048;  // traceback bucket key = class * TB_KEY_STRIDE + rows (rows, n < 2048)
 constexpr int THIN_MAXROWS = 336;
-bool launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st);   // false: nothing to do
+int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st);   // returns kernels launched
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 

@@ -79,12 +79,11 @@ struct ScoreParams {
 #define SDP_TB_SCALE 8
 #define SDP_TB_MAX_VALUE 4090   // largest unscaled drift-form value: 8 * 4090 + 7 <= 32767
 struct TraceConsts {
-    uint32_t one, c16, c8, cm1;    // 1, 16, 8, -1: opaque multipliers that keep adds/shifts on the FMA pipe
     uint32_t m4;                   // 0x00040004, opaque so that the tag select stays one LOP3
     uint32_t negO_e;               // 8 * (-o) + 1 : "I opened here" candidate (tag bit 0)
     uint32_t negO_f;               // 8 * (-o) + 6 : "D opened here" candidate (tag bit 2); D extended carries tag 2
     uint32_t qx;                   // 8 * (2e + mismatch) + 7 : diagonal increment of a mismatch, tag 7
-    uint32_t Cf;                   // fp16 denormal whose bits are 8 * (2e + match) + 7
+    uint32_t Cd8;                  // fp16 denormal whose bits are 8 * (match - mismatch)
     uint32_t e2, beta2, betaMinusO2;   // 8e, 8 beta, 8 (beta - o)
     int32_t  e, beta;              // unscaled
 };

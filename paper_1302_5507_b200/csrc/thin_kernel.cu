@@ -121,14 +121,16 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
                 Fc[jj] = TNEG + 2;
             }
         }
-        // sliding 32-base buffers of the read (bases and spread N bits), refilled every 16 rows
+        // sliding buffer of the read: NSEG + 1 words of 16 bases (and their spread N bits) starting at read
+        // position q0; row ir looks at the BW bases from position q0 + roffs on. Refilled every 16 rows.
+        constexpr int NSEG = (BW + 15) / 16;
         long long q0 = (long long)(i_lo + 1 - c - W_) - 1;            // read position of segment bit 0 at row i_lo+1
-        uint64_t rbuf = (uint64_t)bases16(b.reads_packed, (long long)roff + q0, rwords) |
-                        ((uint64_t)bases16(b.reads_packed, (long long)roff + q0 + 16, rwords) << 32);
-        uint64_t rnbuf = 0;
-        if (b.read_nmask != nullptr)
-            rnbuf = (uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0, rnwords) |
-                    ((uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0 + 16, rnwords) << 32);
+        uint32_t rw[NSEG + 1], rnw[NSEG + 1];
+#pragma unroll
+        for (int sgm = 0; sgm <= NSEG; ++sgm) {
+            rw[sgm] = bases16(b.reads_packed, (long long)roff + q0 + 16 * sgm, rwords);
+            rnw[sgm] = nbits16_spread(b.read_nmask, (long long)roff + q0 + 16 * sgm, rnwords);
+        }
         int roffs = 0;                                                // bases consumed from the buffer
         uint32_t tw = 0, twn = 0;
         int finH = TNEG;
@@ -147,14 +149,17 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
             }
             if (roffs == 16) {
                 q0 += 16; roffs = 0;
-                rbuf = (rbuf >> 32) | ((uint64_t)bases16(b.reads_packed, (long long)roff + q0 + 16, rwords) << 32);
-                if (b.read_nmask != nullptr)
-                    rnbuf = (rnbuf >> 32) | ((uint64_t)nbits16_spread(b.read_nmask, (long long)roff + q0 + 16, rnwords) << 32);
+#pragma unroll
+                for (int sgm = 0; sgm < NSEG; ++sgm) { rw[sgm] = rw[sgm + 1]; rnw[sgm] = rnw[sgm + 1]; }
+                rw[NSEG] = bases16(b.reads_packed, (long long)roff + q0 + 16 * NSEG, rwords);
+                rnw[NSEG] = nbits16_spread(b.read_nmask, (long long)roff + q0 + 16 * NSEG, rnwords);
             }
-            const uint32_t seg = (uint32_t)(rbuf >> (2 * roffs));
-            nm |= (uint32_t)(rnbuf >> (2 * roffs));
+            uint32_t eqw[NSEG];
+#pragma unroll
+            for (int sgm = 0; sgm < NSEG; ++sgm)
+                eqw[sgm] = eq16(__funnelshift_r(rw[sgm], rw[sgm + 1], 2 * roffs), t * 0x55555555u,
+                                nm | __funnelshift_r(rnw[sgm], rnw[sgm + 1], 2 * roffs));
             ++roffs;
-            const uint32_t eqw = eq16(seg, t * 0x55555555u, nm);
 
             int Hl = TNEG, El = TNEG;
             uint32_t acc[WPR];
@@ -164,7 +169,7 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
             for (int jj = 0; jj < BW; ++jj) {
                 int Ft = __viaddmax_s32(Hc[jj + 1], tc.negOf, Fc[jj + 1]);
                 int Et = __viaddmax_s32(Hl, tc.negOe, El);
-                const int q = ((eqw >> (2 * jj)) & 1u) ? tc.qm : tc.qx;
+                const int q = ((eqw[jj >> 4] >> (2 * (jj & 15))) & 1u) ? tc.qm : tc.qx;
                 int Ht = __vimax3_s32(Hc[jj] + q, Ft, Et);
                 if (CHECK) {
                     const int j = jb + jj;
@@ -228,48 +233,50 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
     tp.pass[p] = ((long long)n_match * 1000000LL >= tp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
 }
 
-// All gap bounds W = 0..THIN_NW-1 in ONE launch: block b serves class w with
-// r.block_start[w] <= b < r.block_start[w+1] (seven small launches in a row left the GPU mostly idle).
+// Gap bounds LO..HI-1 in ONE launch: block b serves class w with
+// r.block_start[w] <= b < r.block_start[w+1] (one small launch per class left the GPU mostly idle).
 struct ThinRanges { uint32_t first[THIN_NW], count[THIN_NW], block_start[THIN_NW + 1]; };
 
-__global__ void __launch_bounds__(128) k_thin_all(const TraceParams tp, const ThinConsts tc, const ThinRanges r)
+template <int W_, int HI>
+__device__ __forceinline__ void thin_dispatch(const int w, const TraceParams& tp, const ThinConsts& tc,
+                                              const ThinRanges& r, const uint32_t k)
 {
-    int w = 0;
+    if (w == W_) thin_body<W_, THIN_MAXROWS>(tp, tc, r.first[W_], r.count[W_], k);
+    else if constexpr (W_ + 1 < HI) thin_dispatch<W_ + 1, HI>(w, tp, tc, r, k);
+}
+
+template <int LO, int HI>
+__global__ void __launch_bounds__(128) k_thin_range(const TraceParams tp, const ThinConsts tc, const ThinRanges r)
+{
+    const uint32_t b = blockIdx.x + r.block_start[LO];
+    int w = LO;
 #pragma unroll
-    for (int c = 1; c < THIN_NW; ++c) w += (blockIdx.x >= r.block_start[c]) ? 1 : 0;
-    const uint32_t k = (blockIdx.x - r.block_start[w]) * blockDim.x + threadIdx.x;
-    switch (w) {                                           // block-uniform
-        case 0: thin_body<0, THIN_MAXROWS>(tp, tc, r.first[0], r.count[0], k); break;
-        case 1: thin_body<1, THIN_MAXROWS>(tp, tc, r.first[1], r.count[1], k); break;
-        case 2: thin_body<2, THIN_MAXROWS>(tp, tc, r.first[2], r.count[2], k); break;
-        case 3: thin_body<3, THIN_MAXROWS>(tp, tc, r.first[3], r.count[3], k); break;
-        case 4: thin_body<4, THIN_MAXROWS>(tp, tc, r.first[4], r.count[4], k); break;
-        case 5: thin_body<5, THIN_MAXROWS>(tp, tc, r.first[5], r.count[5], k); break;
-        case 6: thin_body<6, THIN_MAXROWS>(tp, tc, r.first[6], r.count[6], k); break;
-        default: thin_body<7, THIN_MAXROWS>(tp, tc, r.first[7], r.count[7], k); break;
-    }
+    for (int c = LO + 1; c < HI; ++c) w += (b >= r.block_start[c]) ? 1 : 0;
+    const uint32_t k = (b - r.block_start[w]) * blockDim.x + threadIdx.x;
+    thin_dispatch<LO, HI>(w, tp, tc, r, k);                // w is block-uniform
 }
 
 // bounds[w] .. bounds[w+1]: range of tp.order that holds the pairs with gap bound w
-bool launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st)
+int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st)
 {
-    static_assert(THIN_NW == 8, "update k_thin_all");
     ThinConsts tc;
     const int o = tp.sc.gap_open, e = tp.sc.gap_extend;
     tc.negOe = -8 * o + 1; tc.negOf = -8 * o + 6;
     tc.qm = 8 * (2 * e + tp.sc.match) + 7; tc.qx = 8 * (2 * e + tp.sc.mismatch) + 7; tc.e8 = 8 * e;
     ThinRanges r;
     uint32_t blocks = 0;
-    // heaviest classes first, so that the long-running blocks do not form the tail of the launch
     for (int w = 0; w < THIN_NW; ++w) {
         r.first[w] = bounds[w]; r.count[w] = bounds[w + 1] - bounds[w];
         r.block_start[w] = blocks;
         blocks += (r.count[w] + 127) / 128;
     }
     r.block_start[THIN_NW] = blocks;
-    if (blocks == 0) return false;
-    k_thin_all<<<blocks, 128, 0, st>>>(tp, tc, r);
-    return true;
+    int launched = 0;
+    const uint32_t lo_blocks = r.block_start[THIN_SPLIT], hi_blocks = blocks - lo_blocks;
+    // the wide bands first: their blocks run longest
+    if (hi_blocks) { k_thin_range<THIN_SPLIT, THIN_NW><<<hi_blocks, 128, 0, st>>>(tp, tc, r); ++launched; }
+    if (lo_blocks) { k_thin_range<0, THIN_SPLIT><<<lo_blocks, 128, 0, st>>>(tp, tc, r); ++launched; }
+    return launched;
 }
 
 }  // namespace sdp

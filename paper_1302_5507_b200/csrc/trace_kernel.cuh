@@ -16,20 +16,24 @@
 // I extended 0) and (b) the winner's tag survives in the low bits of the result:
 //     Et = max(Hc(i,j-1) - 8o + 1, Ec(i,j-1))             VIADDMNMX   tag bit 0 = opened
 //     Ft = max(Hc(i-1,j) - 8o + 6, Fc(i-1,j) [= 8v+2])    VIADDMNMX   tag bit 2 = opened
-//     q  = max(fp16 selector, 8(2e+mismatch)+7)           VIMNMX      8(2e+match)+7 when bases are equal
-//     Ht = max3(Hc(i-1,j-1) + q, Ft, Et)                  IMAD + VIMNMX3
+//     u  = max(Hc(i-1,j-1) + q8, Ft)                      VIADDMNMX   q8 = 8(2e+delta)+7, exact (fp16 pipe,
+//     Ht = max(u, Et)                                     VIMNMX           as in score_kernel.cuh)
 //     Ec = Et & ~1, Fc = Ft & ~4, Hc = Ht & ~7            3 LOP3      clean values for the next cell
-//     nibble = ((Ht & ~4 | Ft & 4) - Hc) + 8 (Et - Ec)    1 LOP3 + IMADs (FMA pipe)
+//     v  = Ht & ~4 | Ft & 4                               1 LOP3
 // Eight ALU-pipe instructions per two cells (two pairs share the int16x2 lanes) against four in
-// the score kernel. Nibbles are packed four cells per 16-bit lane and stored row by row:
+// the score kernel. The nibble (v - Hc) + 8 (Et - Ec) and its packing run on the FMA pipe without
+// any IMAD (an IMAD costs two HFMA2 slots on sm_100a): two VIADD.16x2 subtractions, then fp16
+// FMAs on the small integers as DENORMALS (t = eb*8 + nib, byte = t0*16 + t1: exact below 2048),
+// and one PRMT per four cells joins two bytes. Nibbles are left-aligned, four cells per 16-bit
+// lane (cell kk of a word in bits 4*(3 - kk)), and stored row by row:
 //     word((i, g, w)) = region + ((i-1) * G + g) * ceil(K/4) + w,   low half = first pair of the two.
 #pragma once
 #include "score_kernel.cuh"
 
 namespace sdp {
 
-__device__ __forceinline__ uint32_t imad_u(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t r; asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c)); return r;
+__device__ __forceinline__ uint32_t sub_s16x2(uint32_t a, uint32_t b) {
+    return __vsub2(a, b);
 }
 // bitwise (mask ? b : a) in one LOP3 (mask kept in a register: a LOP3 takes one immediate at most)
 __device__ __forceinline__ uint32_t lop3_select(uint32_t a, uint32_t b, uint32_t mask) {
@@ -102,8 +106,9 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     const uint32_t rowstride = (uint32_t)(G * NW);
     uint32_t* wp = T.bits + (st_ok ? T.bits_off[first + 2 * q] : 0ull) + (uint32_t)(g * NW);
 
-    const uint32_t one = T.c.one, c16 = T.c.c16, c8 = T.c.c8, cm1 = T.c.cm1, m4 = T.c.m4;
-    const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, Cf = T.c.Cf, e2 = T.c.e2;
+    const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8;
+    const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, e2 = T.c.e2;
+    constexpr uint32_t H2_8 = 0x48004800u, H2_16 = 0x4C004C00u;        // fp16 8.0 and 16.0, both lanes
     const uint32_t notfirst = is_first ? 0u : 0xFFFFFFFFu;
     uint32_t fv = is_first ? T.c.beta2 : 0u;              // 8 H'(i,0) = 8 (beta + e i): free start
     const uint32_t fstep = is_first ? e2 : 0u;
@@ -131,28 +136,31 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         uint32_t Hsk = hin, Esk = ein;
         uint32_t hd = hdiag;
         hdiag = hin;
-        uint32_t acc = 0u;
+        uint32_t b0 = 0u, b1 = 0u, t0 = 0u;              // high byte, low byte of the current word; first nibble of a byte
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const uint32_t sel = hfma2_negsq(hsub2_u(nt, rh[k]), Cf);
-            const uint32_t dq = __vmaxs2(sel, qx);
-            const uint32_t dg = imad_u(one, hd, dq);
-            hd = Hs[k];
+            const uint32_t q8 = hfma2_u(hfma2_is_zero(hsub2_u(nt, rh[k])), Cd8, qx);
             const uint32_t Ft = __viaddmax_s16x2(Hs[k], negOf, F[k]);
             F[k] = Ft & 0xFFFBFFFBu;
+            const uint32_t u = __viaddmax_s16x2(hd, q8, Ft);
+            hd = Hs[k];
             const uint32_t Et = __viaddmax_s16x2(Hl, negOe, E);
             E = Et & 0xFFFEFFFEu;
-            const uint32_t Ht = __vimax3_s16x2(dg, Ft, Et);
+            const uint32_t Ht = __vmaxs2(u, Et);
             Hl = Ht & 0xFFF8FFF8u;
             Hn[k] = Hl;
             const uint32_t v = lop3_select(Ht, Ft, m4);
-            const uint32_t nib = imad_u(Hl, cm1, v);      // v - Hc: bits 2..0
-            const uint32_t eb = imad_u(E, cm1, Et);       // Et - Ec: 0 or 1
-            acc = imad_u(acc, c16, nib);
-            acc = imad_u(eb, c8, acc);
+            const uint32_t nib = sub_s16x2(v, Hl);        // bits 2..0
+            const uint32_t eb = sub_s16x2(Et, E);         // 0 or 1
+            const uint32_t t = hfma2_u(eb, H2_8, nib);    // nib + 8 eb as fp16 denormals: exact
+            if ((k & 1) == 0) t0 = t;
+            if ((k & 1) == 1 || k == K - 1) {
+                const uint32_t byte = (k & 1) ? hfma2_u(t0, H2_16, t) : hfma2_u(t0, H2_16, 0u);
+                if ((k & 3) < 2) b0 = byte; else b1 = byte;
+            }
             if ((k & 3) == 3 || k == K - 1) {
-                if (do_store) wp[k >> 2] = acc;
-                acc = 0u;
+                if ((k & 3) < 2) b1 = 0u;
+                if (do_store) wp[k >> 2] = __byte_perm(b1, b0, 0x6240);
             }
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }

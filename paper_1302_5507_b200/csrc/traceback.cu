@@ -31,7 +31,7 @@ __device__ __forceinline__ int tb_class_of(int bw) {
     static_assert(TB_NCLASS == 4, "update tb_class_of");
     return bw > 256 ? 3 : (bw > 64 ? 2 : (bw > 16 ? 1 : 0));
 }
-static_assert((THIN_NW + TB_NCLASS) * 4096 <= SDP_NBINS, "thin keys must fit the bucket-sort key space");
+static_assert((THIN_NW + TB_NCLASS) * TB_KEY_STRIDE <= SDP_NBINS && SDP_MAX_READ_LEN < TB_KEY_STRIDE, "thin keys must fit the bucket-sort key space");
 
 __device__ __forceinline__ void hist_add(uint32_t* hist, uint32_t key, bool valid) {
     const uint32_t active = __ballot_sync(0xffffffffu, valid);
@@ -70,7 +70,7 @@ __global__ void k_post_forward(const PostParams pp)
         const bool narrow = W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && !pp.no_thin);
         const bool wide = !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
         if (narrow) {
-            ktb = (uint32_t)W * 4096u + (uint32_t)min(4095, W ? rows : n);
+            ktb = (uint32_t)W * TB_KEY_STRIDE + (uint32_t)min((int)TB_KEY_STRIDE - 1, W ? rows : n);
             c_tb = (unsigned long long)bw * rows;
         } else if (wide) {
             krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
@@ -78,7 +78,7 @@ __global__ void k_post_forward(const PostParams pp)
             c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
         } else {
             words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows;
-            ktb = (uint32_t)(THIN_NW + tb_class_of(bw)) * 4096u + (uint32_t)min(bw, 4095);
+            ktb = (uint32_t)(THIN_NW + tb_class_of(bw)) * TB_KEY_STRIDE + (uint32_t)min(bw, (int)TB_KEY_STRIDE - 1);
         }
         pp.keys_rev[p] = krev;
         pp.keys_wide[p] = kwide;
@@ -369,9 +369,8 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
         else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
         const int w = kk >> 2;
-        const int cw = min(4, K - 4 * w);
         const uint32_t word = __ldg(region + ((size_t)(i - 1) * G + g) * NW + w);
-        const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(cw - 1 - (kk & 3)))) & 15u;
+        const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u;
         if (st == 0) {
             if ((f & 3u) == 3u) {
                 emit(0, 1u); ++n_cols;
