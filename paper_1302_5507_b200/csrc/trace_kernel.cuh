@@ -22,19 +22,18 @@
 //     v  = Ht & ~4 | Ft & 4                               1 LOP3
 // Eight ALU-pipe instructions per two cells (two pairs share the int16x2 lanes) against four in
 // the score kernel. The nibble (v - Hc) + 8 (Et - Ec) and its packing run on the FMA pipe without
-// any IMAD (an IMAD costs two HFMA2 slots on sm_100a): two VIADD.16x2 subtractions, then fp16
+// any IMAD (an IMAD costs two HFMA2 slots on sm_100a; a packed subtraction costs a LOP3 and two
+// VIADD.16x2, so the tags are masked out with two more LOP3 instead): fp16
 // FMAs on the small integers as DENORMALS (t = eb*8 + nib, byte = t0*16 + t1: exact below 2048),
 // and one PRMT per four cells joins two bytes. Nibbles are left-aligned, four cells per 16-bit
 // lane (cell kk of a word in bits 4*(3 - kk)), and stored row by row:
-//     word((i, g, w)) = region + ((i-1) * G + g) * ceil(K/4) + w,   low half = first pair of the two.
+//     word((i, w, lane)) = task region + ((i-1) * ceil(K/4) + w) * 32 + lane,   low half = first pair of the two
+// (one region per warp task: a warp-wide store writes one 128-byte line).
 #pragma once
 #include "score_kernel.cuh"
 
 namespace sdp {
 
-__device__ __forceinline__ uint32_t sub_s16x2(uint32_t a, uint32_t b) {
-    return __vsub2(a, b);
-}
 // bitwise (mask ? b : a) in one LOP3 (mask kept in a register: a LOP3 takes one immediate at most)
 __device__ __forceinline__ uint32_t lop3_select(uint32_t a, uint32_t b, uint32_t mask) {
     uint32_t r; asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(r) : "r"(a), "r"(b), "r"(mask)); return r;
@@ -103,8 +102,8 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
 
     const bool st_ok = hasA;                              // hasB implies hasA
-    const uint32_t rowstride = (uint32_t)(G * NW);
-    uint32_t* wp = T.bits + (st_ok ? T.bits_off[first + 2 * q] : 0ull) + (uint32_t)(g * NW);
+    constexpr uint32_t rowstride = 32u * NW;              // word (row, w, lane): a warp-wide store is one 128-byte line
+    uint32_t* wp = T.bits + T.bits_off[first] + (uint32_t)lane;
 
     const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8;
     const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, e2 = T.c.e2;
@@ -150,8 +149,8 @@ trace_kernel(const ScoreParams P, const TraceDP T)
             Hl = Ht & 0xFFF8FFF8u;
             Hn[k] = Hl;
             const uint32_t v = lop3_select(Ht, Ft, m4);
-            const uint32_t nib = sub_s16x2(v, Hl);        // bits 2..0
-            const uint32_t eb = sub_s16x2(Et, E);         // 0 or 1
+            const uint32_t nib = v & 0x00070007u;         // bits 2..0
+            const uint32_t eb = Et & 0x00010001u;         // 0 or 1
             const uint32_t t = hfma2_u(eb, H2_8, nib);    // nib + 8 eb as fp16 denormals: exact
             if ((k & 1) == 0) t0 = t;
             if ((k & 1) == 1 || k == K - 1) {
@@ -160,7 +159,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
             }
             if ((k & 3) == 3 || k == K - 1) {
                 if ((k & 3) < 2) b1 = 0u;
-                if (do_store) wp[k >> 2] = __byte_perm(b1, b0, 0x6240);
+                if (do_store) wp[(k >> 2) * 32] = __byte_perm(b1, b0, 0x6240);
             }
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }

@@ -275,8 +275,8 @@ void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st)
 }
 
 // ---------------------------------------------------------------------------------------------
-// wide pairs (trace_kernel.cuh). Sorted by (n, rows) into `order`; two neighbours of one read
-// length share the int16x2 lanes and one region of direction nibbles.
+// wide pairs (trace_kernel.cuh). Sorted by (n, rows) into `order`; the pairs of one warp task share
+// one region of direction nibbles, laid out so that a warp's store of one word per lane is contiguous.
 __global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_count,
                                const uint32_t* __restrict__ count_dev, const uint32_t* __restrict__ pn,
                                const int32_t* __restrict__ tb_rows, const uint16_t* __restrict__ slot_of_n,
@@ -287,11 +287,12 @@ __global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_
     const uint32_t p = order[k];
     const SlotInfo si = slots[slot_of_n[pn[p] - 1]];
     const uint32_t local = k - si.first;
+    const uint32_t ppw = 2u * (32u / si.G);               // pairs per warp task
     uint32_t w = 0;
-    if ((local & 1u) == 0) {
-        int rows = tb_rows[p];
-        if (local + 1 < si.count) rows = max(rows, tb_rows[order[k + 1]]);
-        w = (uint32_t)rows * (uint32_t)si.G * (uint32_t)((si.K + 3) / 4);
+    if (local % ppw == 0) {                               // first pair of a task owns the task's region
+        int rows = 0;
+        for (uint32_t t = 0; t < ppw && local + t < si.count; ++t) rows = max(rows, tb_rows[order[k + t]]);
+        w = (uint32_t)rows * 32u * (uint32_t)((si.K + 3) / 4);
     }
     words[k] = w;
 }
@@ -344,7 +345,10 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
     const uint32_t local = k - si.first;
     const int G = si.G, K = si.K, NW = (K + 3) / 4;
     const int pad = G * K - n;
-    const uint32_t* region = wp.bits + wp.bits_off[k - (local & 1u)];
+    const uint32_t ppw = 2u * (32u / (uint32_t)G);
+    const uint32_t in_task = local % ppw;
+    const uint32_t* region = wp.bits + wp.bits_off[k - in_task];
+    const uint32_t lane0 = (in_task >> 1) * (uint32_t)G;  // lane of the group's first thread
     const uint32_t lane_shift = (local & 1u) * 16u;
     const SeqReader RD{wp.b.reads_packed, wp.b.read_nmask, SDP_CODE_READ_N};
     const SeqReader WN{wp.b.wins_packed, wp.b.win_nmask, SDP_CODE_WIN_N};
@@ -369,7 +373,7 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
         else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
         const int w = kk >> 2;
-        const uint32_t word = __ldg(region + ((size_t)(i - 1) * G + g) * NW + w);
+        const uint32_t word = __ldg(region + ((size_t)(i - 1) * NW + w) * 32u + lane0 + (uint32_t)g);
         const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u;
         if (st == 0) {
             if ((f & 3u) == 3u) {
