@@ -3,7 +3,7 @@
 // The forward score S bounds the gap content of every co-optimal alignment,
 // W = floor((n*match - S - o) / e), so every co-optimal path lies in the
 // band |i - j - (i_end - n)| <= W of rows (i_end - n - W, i_end]. For W = 0 the alignment is
-// gapless: CIGAR nM, n_match by XOR + popcount over the 2-bit words. For 1 <= W <= 7 the band
+// gapless: CIGAR nM, n_match from the score alone. For 1 <= W <= 7 the band
 // (2W+1 <= 15 columns) is recomputed with the paper's recurrences in the same
 // x8 tagged integer domain as trace_kernel.cuh -- scalar int32 here, band cells in registers, the
 // row loop fully unrolled over the band -- and leaves four direction bits per cell in a per-thread
@@ -85,9 +85,14 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
     uint32_t nops = 0;
     int cur_op = -1; uint32_t cur_len = 0;
     bool bad = false;
+    int gap_runs = 0, gap_bases = 0;
     auto emit = [&](int op, uint32_t len) {
         if (op == cur_op) { cur_len += len; return; }
-        if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
+        if (cur_op >= 0) {
+            if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true;
+            ++nops;
+            if (cur_op > 0) { ++gap_runs; gap_bases += (int)cur_len; }
+        }
         cur_op = op; cur_len = len;
     };
 
@@ -95,15 +100,6 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
         // gapless: every co-optimal alignment is ungapped, so the CIGAR is nM
         ref_start = i_end - n;
         if (ref_start < 0) { bad = true; ref_start = 0; }
-        for (int j0 = 0; j0 < n; j0 += 16) {
-            const uint32_t r = bases16(b.reads_packed, (long long)roff + j0, rwords);
-            const uint32_t t = bases16(b.wins_packed, (long long)woff + ref_start + j0, wwords);
-            const uint32_t nm = nbits16_spread(b.read_nmask, (long long)roff + j0, rnwords) |
-                                nbits16_spread(b.win_nmask, (long long)woff + ref_start + j0, wnwords);
-            uint32_t eq = eq16(r, t, nm);
-            if (n - j0 < 16) eq &= (1u << (2 * (n - j0))) - 1u;
-            n_match += __popc(eq);
-        }
         n_cols = n;
         emit(0, (uint32_t)n);
     } else {
@@ -205,8 +201,6 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
             if (st == 0) {
                 if ((f & 3u) == 3u) {
                     emit(0, 1u); ++n_cols;
-                    n_match += (base_at(b.reads_packed, b.read_nmask, roff + (uint64_t)(j - 1), SDP_CODE_READ_N) ==
-                                base_at(b.wins_packed, b.win_nmask, woff + (uint64_t)(i - 1), SDP_CODE_WIN_N));
                     --i; --j;
                 } else if ((f & 3u) == 2u) st = 1;
                 else st = 2;
@@ -223,6 +217,15 @@ __device__ __forceinline__ void thin_body(const TraceParams& tp, const ThinConst
         ref_start = i;
     }
     emit(-2, 0u);                                          // flush the last run
+    {   // The path scores exactly S = match*n_match + mismatch*(M columns - n_match) - sum over gap runs of
+        // (o + e*len), so n_match follows from the score without touching the sequences again
+        // (N columns score mismatch and are not matches, consistently). A remainder means the walk is wrong.
+        const int num = tp.score[p] + tp.sc.gap_open * gap_runs + tp.sc.gap_extend * gap_bases -
+                        tp.sc.mismatch * (n_cols - gap_bases);
+        const int den = tp.sc.match - tp.sc.mismatch;
+        n_match = num / den;
+        if (num < 0 || n_match * den != num || n_match > n_cols - gap_bases) bad = true;
+    }
     if (bad) { atomicOr(tp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
     tp.ref_start[p] = ref_start;
     tp.read_start[p] = 0;

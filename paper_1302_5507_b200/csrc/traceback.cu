@@ -350,8 +350,6 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
     const uint32_t* region = wp.bits + wp.bits_off[k - in_task];
     const uint32_t lane0 = (in_task >> 1) * (uint32_t)G;  // lane of the group's first thread
     const uint32_t lane_shift = (local & 1u) * 16u;
-    const SeqReader RD{wp.b.reads_packed, wp.b.read_nmask, SDP_CODE_READ_N};
-    const SeqReader WN{wp.b.wins_packed, wp.b.win_nmask, SDP_CODE_WIN_N};
     const uint32_t cap = 2u * (uint32_t)wp.tbW[p] + 3u;
     uint32_t* ops = wp.ops_rev + wp.ops_off[p];
 
@@ -359,9 +357,14 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
     uint32_t nops = 0;
     int cur_op = -1; uint32_t cur_len = 0;
     bool bad = false;
+    int gap_runs = 0, gap_bases = 0;
     auto emit = [&](int op, uint32_t len) {
         if (op == cur_op) { cur_len += len; return; }
-        if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
+        if (cur_op >= 0) {
+            if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true;
+            ++nops;
+            if (cur_op > 0) { ++gap_runs; gap_bases += (int)cur_len; }
+        }
         cur_op = op; cur_len = len;
     };
     int i = R, j = n, st = 0;                              // 0 = H, 1 = D, 2 = I
@@ -378,7 +381,6 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (st == 0) {
             if ((f & 3u) == 3u) {
                 emit(0, 1u); ++n_cols;
-                n_match += (RD.at(d.roff + (uint64_t)j0) == WN.at(d.woff + (uint64_t)(i - 1)));
                 --i; --j;
             } else if ((f & 3u) == 2u) st = 1;
             else st = 2;
@@ -393,6 +395,13 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         }
     }
     emit(-2, 0u);
+    {   // n_match from the score (see thin_kernel.cu): S = match*n_match + mismatch*(M columns - n_match) - gap costs
+        const int num = d.aux + wp.sc.gap_open * gap_runs + wp.sc.gap_extend * gap_bases -
+                        wp.sc.mismatch * (n_cols - gap_bases);
+        const int den = wp.sc.match - wp.sc.mismatch;
+        n_match = num / den;
+        if (num < 0 || n_match * den != num || n_match > n_cols - gap_bases) bad = true;
+    }
     if (bad) { atomicOr(wp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
     wp.ref_start[p] = wp.ref_end[p] + 1 - R + i;
     wp.read_start[p] = 0;
