@@ -143,7 +143,8 @@ __global__ void __launch_bounds__(1024) k_tasks(const uint32_t* __restrict__ bin
                                                 const uint16_t* __restrict__ slot_n,
                                                 const uint16_t* __restrict__ slot_G,
                                                 const uint16_t* __restrict__ slot_K,
-                                                SlotInfo* __restrict__ slots, uint32_t* __restrict__ task_prefix)
+                                                SlotInfo* __restrict__ slots, uint32_t* __restrict__ task_prefix,
+                                                uint32_t* __restrict__ host_prefix, uint32_t* __restrict__ host_total)
 {
     const int t = threadIdx.x;
     const uint32_t n = slot_n[t];
@@ -157,7 +158,8 @@ __global__ void __launch_bounds__(1024) k_tasks(const uint32_t* __restrict__ bin
     SlotInfo si; si.first = first; si.count = count; si.n = n; si.G = (uint16_t)G; si.K = slot_K[t];
     slots[t] = si;
     task_prefix[t] = pre;
-    if (t == 0) task_prefix[SDP_NSLOTS] = total;
+    host_prefix[t] = pre;                                 // pinned host mailbox: the host sizes the launches from it
+    if (t == 0) { task_prefix[SDP_NSLOTS] = total; host_prefix[SDP_NSLOTS] = total; *host_total = bin_start[SDP_NBINS]; }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -253,6 +255,26 @@ void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint6
 }
 
 // ---------------------------------------------------------------------------------------------
+// everything else the host needs after the post-forward bookkeeping, written straight into the pinned
+// mailbox by one small kernel (instead of some twenty 4-byte copies)
+__global__ void k_mailbox(const uint32_t* __restrict__ tb_bin_start, uint32_t stride, uint32_t nbounds,
+                          const uint64_t* __restrict__ totals, const unsigned long long* __restrict__ counters,
+                          uint32_t* __restrict__ host_bounds, uint64_t* __restrict__ host_totals,
+                          unsigned long long* __restrict__ host_counters)
+{
+    const uint32_t t = threadIdx.x;
+    if (t < nbounds) host_bounds[t] = tb_bin_start[(size_t)t * stride];
+    if (t < 4) { host_totals[t] = totals[t]; host_counters[t] = counters[t]; }
+}
+
+void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbounds, const uint64_t* totals,
+                    const unsigned long long* counters, uint32_t* host_bounds, uint64_t* host_totals,
+                    unsigned long long* host_counters, cudaStream_t st)
+{
+    k_mailbox<<<1, 64, 0, st>>>(tb_bin_start, stride, nbounds, totals, counters, host_bounds, host_totals, host_counters);
+}
+
+// ---------------------------------------------------------------------------------------------
 // host wrappers
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st)
@@ -268,13 +290,13 @@ void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t 
 
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
-                      SlotInfo* slots, uint32_t* task_prefix, cudaStream_t st)
+                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st)
 {
     uint32_t* tile_sums = bin_start + SDP_NBINS + 4;        // scratch behind the total (SDP_BIN_SCRATCH words)
     k_scan_bins_tiles<<<BIN_TILES, 1024, 0, st>>>(hist, bin_start, tile_sums);
     k_scan_bins_finish<<<BIN_TILES, 1024, 0, st>>>(hist, bin_start, tile_sums);
     k_scatter<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist, order);
-    if (slots) k_tasks<<<1, 1024, 0, st>>>(bin_start, slot_n, slot_G, slot_K, slots, task_prefix);
+    if (slots) k_tasks<<<1, 1024, 0, st>>>(bin_start, slot_n, slot_G, slot_K, slots, task_prefix, host_prefix, host_total);
 }
 
 void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st)

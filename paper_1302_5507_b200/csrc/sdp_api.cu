@@ -397,11 +397,10 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
                         ctx->hist[0], ctx->err_flag, ctx->counters + 3, st);
     launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0], st);
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0],
+                     ctx->mb->task_prefix[0], &ctx->mb->bin_total[0], st);
     nl += 5;
-    CU(cudaMemcpyAsync(ctx->mb->task_prefix[0], ctx->task_prefix[0], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(&ctx->mb->bin_total[0], ctx->bin_start[0] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     if (ctx->mb->err_flag & SDP_ERRF_INDEX)
         return fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)");
@@ -432,11 +431,13 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
     launch_sort_tail(ctx->keys_rev.as<uint32_t>(), P, ctx->hist[1], ctx->bin_start[1], ctx->order_rev.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1], st);
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1],
+                     ctx->mb->task_prefix[1], &ctx->mb->bin_total[1], st);
     launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
-                     nullptr, nullptr, nullptr, nullptr, nullptr, st);
+                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, st);
     launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2], st);
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2],
+                     ctx->mb->task_prefix[2], &ctx->mb->bin_total[3], st);
     nl += 12;
     // one region of direction nibbles per two wide pairs that share the int16x2 lanes (every slot of
     // order_wide beyond the wide pairs reads as a zero-size region)
@@ -453,14 +454,9 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     exclusive_scan_u32_u64(ctx->ops_cap.as<uint32_t>(), P, ctx->ops_off.as<uint64_t>(), ctx->totals + 1,
                            ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
                            ctx->scan_tile_base.as<uint64_t>(), st, &nl);
-    CU(cudaMemcpyAsync(ctx->mb->task_prefix[1], ctx->task_prefix[1], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(ctx->mb->task_prefix[2], ctx->task_prefix[2], (SDP_NSLOTS + 1) * 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(&ctx->mb->bin_total[1], ctx->bin_start[1] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(&ctx->mb->bin_total[3], ctx->bin_start[3] + SDP_NBINS, 4, cudaMemcpyDeviceToHost, st));
-    for (int c = 0; c <= THIN_NW + TB_NCLASS; ++c)
-        CU(cudaMemcpyAsync(&ctx->mb->tb_bounds[c], ctx->bin_start[2] + (size_t)c * TB_KEY_STRIDE, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(ctx->mb->totals, ctx->totals, 4 * 8, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(ctx->mb->counters, ctx->counters, 4 * 8, cudaMemcpyDeviceToHost, st));
+    launch_mailbox(ctx->bin_start[2], TB_KEY_STRIDE, THIN_NW + TB_NCLASS + 1, ctx->totals, ctx->counters,
+                   ctx->mb->tb_bounds, ctx->mb->totals, ctx->mb->counters, st);
+    ++nl;
     CU(cudaStreamSynchronize(st));
     const uint32_t n_rev = ctx->mb->bin_total[1];
     const uint32_t n_wide = ctx->mb->bin_total[3];

@@ -17,7 +17,10 @@ void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t 
 // scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
-                      SlotInfo* slots, uint32_t* task_prefix, cudaStream_t st);
+                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st);
+void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbounds, const uint64_t* totals,
+                    const unsigned long long* counters, uint32_t* host_bounds, uint64_t* host_totals,
+                    unsigned long long* host_counters, cudaStream_t st);
 void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st);
 void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev,
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
