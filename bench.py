@@ -279,9 +279,47 @@ def main():
             dt = float(t.item())
         P = batch.n_pairs
         d2h = P * (4 * 7 + 1 + 8 + 4) + int(res.n_cigar_ops) * 4
-        e2e = {"value": cells_all * args.steps / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "ms_per_step": dt / args.steps * 1e3,
-               "timer": "host wall clock around sdp_align_batch_host (it synchronises internally)"}
+        single_ms = dt / args.steps * 1e3
+        # Same call, two contexts driven by two host threads (separate contexts are independent, sdp.h):
+        # the H2D/D2H copies of one batch overlap the kernels of the other, as a caller streaming batches would.
+        pipe_ms = None
+        if args.steps >= 2:
+            ctx2 = S.Context(device=local)
+            ctx2.align_batch_host_raw(cb)
+            ctx2.align_batch_host_raw(cb)
+            ctxs, errs = (ctx, ctx2), []
+
+            def worker(j):
+                try:
+                    for _ in range(j, args.steps, 2):
+                        ctxs[j].align_batch_host_raw(cb)
+                except Exception as ex:  # noqa: BLE001
+                    errs.append(ex)
+
+            barrier()
+            ths = [threading.Thread(target=worker, args=(j,)) for j in range(2)]
+            t0 = time.perf_counter()
+            for th in ths:
+                th.start()
+            for th in ths:
+                th.join()
+            torch.cuda.synchronize(dev)
+            dtp = time.perf_counter() - t0
+            ctx2.destroy()
+            if errs:
+                raise errs[0]
+            if world > 1:
+                t = torch.tensor([dtp], dtype=torch.float64, device=dev)
+                torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+                dtp = float(t.item())
+            pipe_ms = dtp / args.steps * 1e3
+        best_ms = min(single_ms, pipe_ms) if pipe_ms else single_ms
+        e2e = {"value": cells_all / (best_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": best_ms, "ms_per_step_one_context": single_ms,
+               "ms_per_step_two_contexts": pipe_ms,
+               "timer": "host wall clock around K calls of sdp_align_batch_host (pinned host inputs, every result array "
+                        "copied back to pinned host memory inside the call); value = the better of one context called "
+                        "back to back and two contexts on two host threads"}
 
     if rank != 0:
         return
