@@ -52,6 +52,14 @@ __device__ __forceinline__ uint32_t read_code_half(uint32_t c) {      // c in 0.
     return (t & 0xFFu) * 0x0101u;
 }
 
+// value the optimiser cannot see through (keeps masks from being turned back into predicates + SEL)
+__device__ __forceinline__ uint32_t opaque_u32(uint32_t x) {
+    uint32_t r; asm("mov.b32 %0, %1;" : "=r"(r) : "r"(x)); return r;
+}
+// PRMT without the selector masking __byte_perm adds (every selector nibble here is <= 5)
+__device__ __forceinline__ uint32_t prmt_raw(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t r; asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel)); return r;
+}
 __device__ __forceinline__ uint32_t hsub2_u(uint32_t a, uint32_t b) {
     uint32_t d; asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d;
 }
@@ -286,7 +294,7 @@ score_kernel(const ScoreParams P)
     };
 
     const uint32_t negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, Cd = P.c.Cd, e2 = P.c.e2;
-    const uint32_t notfirst = is_first ? 0u : 0xFFFFFFFFu;
+    const uint32_t notfirst = opaque_u32(is_first ? 0u : 0xFFFFFFFFu);   // a mask, not a predicate: one LOP3 per use
     // boundary column 0 as seen by the group's first thread: H'(i,0) = beta + e*i (forward, free
     // start) or beta - o (reverse, start anchored: a leading deletion of i bases costs o + e*i)
     uint32_t fv = is_first ? (REV ? P.c.betaMinusO2 : P.c.beta2) : 0u;
@@ -314,7 +322,7 @@ score_kernel(const ScoreParams P)
         hin = (hin & notfirst) | fv;
         ein = ein & notfirst;
         // fp16 codes of the window bases of row i, both lanes
-        const uint32_t nt = __byte_perm(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
+        const uint32_t nt = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
 
         uint32_t Hl = hin, E = ein;
         uint32_t Hsk = hin, Esk = ein;                    // outputs if the last column is skipped

@@ -108,7 +108,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8;
     const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, e2 = T.c.e2;
     constexpr uint32_t H2_8 = 0x48004800u, H2_16 = 0x4C004C00u;        // fp16 8.0 and 16.0, both lanes
-    const uint32_t notfirst = is_first ? 0u : 0xFFFFFFFFu;
+    const uint32_t notfirst = opaque_u32(is_first ? 0u : 0xFFFFFFFFu);   // a mask, not a predicate: one LOP3 per use
     uint32_t fv = is_first ? T.c.beta2 : 0u;              // 8 H'(i,0) = 8 (beta + e i): free start
     const uint32_t fstep = is_first ? e2 : 0u;
     uint32_t hout = h_row0, eout = 0u;
@@ -127,7 +127,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         fv = __vadd2(fv, fstep);
         hin = (hin & notfirst) | fv;
         ein = ein & notfirst;
-        const uint32_t nt = __byte_perm(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
+        const uint32_t nt = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
         // (thread g runs G-1-g rows past Mmin inside the steady-state loop: always test the row)
         const bool do_store = st_ok && i <= Rpp;
 
