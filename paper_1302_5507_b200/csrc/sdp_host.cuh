@@ -91,7 +91,7 @@ constexpr int THIN_NW = 24;
 constexpr int THIN_SPLIT = 8;             // classes below / from here on run in two launches (register budgets differ)
 constexpr uint32_t TB_KEY_STRIDE = 2048;  // traceback bucket key = class * TB_KEY_STRIDE + rows (rows, n < 2048)
 constexpr int THIN_MAXROWS = 336;
-int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st);   // returns kernels launched
+int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st, cudaStream_t st_hi);   // returns kernels launched
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 

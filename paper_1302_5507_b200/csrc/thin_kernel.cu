@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(128) k_thin_range(const TraceParams tp, const 
 }
 
 // bounds[w] .. bounds[w+1]: range of tp.order that holds the pairs with gap bound w
-int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st)
+int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st, cudaStream_t st_hi)
 {
     ThinConsts tc;
     const int o = tp.sc.gap_open, e = tp.sc.gap_extend;
@@ -276,8 +276,8 @@ int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t 
     r.block_start[THIN_NW] = blocks;
     int launched = 0;
     const uint32_t lo_blocks = r.block_start[THIN_SPLIT], hi_blocks = blocks - lo_blocks;
-    // the wide bands first: their blocks run longest
-    if (hi_blocks) { k_thin_range<THIN_SPLIT, THIN_NW><<<hi_blocks, 128, 0, st>>>(tp, tc, r); ++launched; }
+    // the wider bands on their own stream: few blocks that run long
+    if (hi_blocks) { k_thin_range<THIN_SPLIT, THIN_NW><<<hi_blocks, 128, 0, st_hi>>>(tp, tc, r); ++launched; }
     if (lo_blocks) { k_thin_range<0, THIN_SPLIT><<<lo_blocks, 128, 0, st>>>(tp, tc, r); ++launched; }
     return launched;
 }
