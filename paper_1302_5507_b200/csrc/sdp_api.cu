@@ -53,6 +53,8 @@ struct Mailbox {                    // pinned host memory the device results lan
     unsigned long long counters[4]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
 };
 
+constexpr int SDP_FAN_STREAMS = 4;
+
 enum { EV_START, EV_BUCKET, EV_FORWARD, EV_REVERSE, EV_TRACE, EV_END, EV_COUNT };
 
 }  // namespace
@@ -76,6 +78,8 @@ struct sdp_ctx {
     cudaStream_t own_stream = nullptr;
     cudaStream_t side_stream = nullptr;   // narrow-band traceback runs here, beside the wide path on the caller's stream
     cudaEvent_t side_done = nullptr;
+    cudaStream_t fan_stream[SDP_FAN_STREAMS] = {};   // [0] unused: the caller's stream takes that turn
+    cudaEvent_t fan_fork = nullptr, fan_join[SDP_FAN_STREAMS] = {};
     cudaStream_t side_stream2 = nullptr;  // the wider narrow bands (W >= THIN_SPLIT): few, long-running blocks
     cudaEvent_t side_done2 = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
@@ -251,6 +255,11 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
         CU(cudaStreamCreateWithFlags(&ctx->side_stream2, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->fan_fork, cudaEventDisableTiming));
+        for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
+            CU(cudaStreamCreateWithFlags(&ctx->fan_stream[k], cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&ctx->fan_join[k], cudaEventDisableTiming));
+        }
         CU(cudaEventCreateWithFlags(&ctx->side_done2, cudaEventDisableTiming));
         for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
         for (int i = 0; i < 4; ++i) {
@@ -296,6 +305,11 @@ void sdp_destroy(sdp_ctx* ctx)
     if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
     if (ctx->side_done) cudaEventDestroy(ctx->side_done);
     if (ctx->side_stream2) cudaStreamDestroy(ctx->side_stream2);
+    if (ctx->fan_fork) cudaEventDestroy(ctx->fan_fork);
+    for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
+        if (ctx->fan_stream[k]) cudaStreamDestroy(ctx->fan_stream[k]);
+        if (ctx->fan_join[k]) cudaEventDestroy(ctx->fan_join[k]);
+    }
     if (ctx->side_done2) cudaEventDestroy(ctx->side_done2);
     for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
@@ -338,15 +352,37 @@ static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const
     sp.c = ctx->consts;
     sp.score = ctx->score.as<int32_t>(); sp.ref_end = ctx->ref_end.as<int32_t>();
     sp.rev_rows = ctx->rev_rows.as<int32_t>(); sp.err_flag = ctx->err_flag;
+    // One launch per column-count class in use. With several classes (mixed read lengths) the launches go
+    // round-robin over the caller's stream and SDP_FAN_STREAMS - 1 helper streams, forked from and joined
+    // back into the caller's stream with events, so that one class's tail overlaps the next class's start.
+    int classes = 0;
     for (int cls = 2; cls <= 2 * SDP_MAX_K + 1; ++cls) {
+        const uint32_t s0 = ctx->cls_begin[cls], s1 = ctx->cls_begin[cls + 1];
+        if (s1 > s0 && tp[s1] > tp[s0]) ++classes;
+    }
+    const bool fan = classes > 1;
+    if (fan) {
+        CU(cudaEventRecord(ctx->fan_fork, st));
+        for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_stream[k], ctx->fan_fork, 0));
+    }
+    int turn = 0;
+    for (int cls = 2 * SDP_MAX_K + 1; cls >= 2; --cls) {                 // largest K (longest reads) first
         const uint32_t s0 = ctx->cls_begin[cls], s1 = ctx->cls_begin[cls + 1];
         if (s1 <= s0) continue;
         const uint32_t t0 = tp[s0], t1 = tp[s1];
         if (t1 <= t0) continue;
         sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
-        if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, st);
-        else launch_score(cls >> 1, (cls & 1) != 0, rev, sp, st);
+        cudaStream_t ls = (fan && (turn % SDP_FAN_STREAMS)) ? ctx->fan_stream[turn % SDP_FAN_STREAMS] : st;
+        ++turn;
+        if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, ls);
+        else launch_score(cls >> 1, (cls & 1) != 0, rev, sp, ls);
         ++*nlaunch;
+    }
+    if (fan) {
+        for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
+            CU(cudaEventRecord(ctx->fan_join[k], ctx->fan_stream[k]));
+            CU(cudaStreamWaitEvent(st, ctx->fan_join[k], 0));
+        }
     }
     CU(cudaGetLastError());
     return SDP_OK;
