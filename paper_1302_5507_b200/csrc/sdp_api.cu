@@ -145,10 +145,10 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
         if (rc_ != SDP_OK) return rc_;                         \
     } while (0)
 
-// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model
-// (DESIGN.md "Score kernel"): a warp runs 2*floor(32/G) pairs for (m + G - 1) steps; a step is
-// bound by the ALU pipe at 2 cycles per instruction: 4 per column, ~11 per row, 4 more when the
-// read length is not G*K (padded variant).
+// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model fitted to
+// measurements on B200: a warp runs 2*floor(32/G) pairs for (m + G - 1) steps;
+// a step costs 4 ALU slots per column plus ~17 of row bookkeeping, ~2.5 more when the read length is not
+// G*K (padded variant), and 12 % more beyond K = 25, where the register budget gets tight.
 void choose_geometry(sdp_ctx* c) {
     struct Ent { uint16_t n, G, K, pad; };
     Ent ents[SDP_NSLOTS];
@@ -164,7 +164,7 @@ void choose_geometry(sdp_ctx* c) {
                 force_g * ((n + force_g - 1) / force_g) - n < force_g) continue;
             double ppw = 2.0 * (32 / G);
             double rows = (double)n + 300.0 + G - 1;
-            double thr = ppw / (rows * (4.0 * K + 11.0 + (G * K != n ? 4.0 : 0.0)));
+            double thr = ppw / (rows * (4.0 * K + 17.0 + (G * K != n ? 2.5 : 0.0)) * (K > 25 ? 1.12 : 1.0));
             if (thr > best) { best = thr; bG = G; bK = K; }
         }
         ents[n - 1] = Ent{(uint16_t)n, (uint16_t)bG, (uint16_t)bK, (uint16_t)(bG * bK != n ? 1 : 0)};

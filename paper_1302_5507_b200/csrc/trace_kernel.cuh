@@ -27,8 +27,10 @@
 // FMAs on the small integers as DENORMALS (t = eb*8 + nib, byte = t0*16 + t1: exact below 2048),
 // and one PRMT per four cells joins two bytes. Nibbles are left-aligned, four cells per 16-bit
 // lane (cell kk of a word in bits 4*(3 - kk)), and stored row by row:
-//     word((i, w, lane)) = task region + ((i-1) * ceil(K/4) + w) * 32 + lane,   low half = first pair of the two
-// (one region per warp task: a warp-wide store writes one 128-byte line).
+//     word((i, w, lane)) = task region + ((s-1) * ceil(K/4) + w) * 32 + lane,   low half = first pair of the two,
+// where s = i + g is the STEP at which thread g of its group works on row i: the threads of a warp are on
+// different rows at any one time (anti-diagonal wavefront), so only a step-major layout makes a warp-wide
+// store one 128-byte line. One region of (rows + G - 1) steps per warp task.
 #pragma once
 #include "score_kernel.cuh"
 
@@ -102,7 +104,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
 
     const bool st_ok = hasA;                              // hasB implies hasA
-    constexpr uint32_t rowstride = 32u * NW;              // word (row, w, lane): a warp-wide store is one 128-byte line
+    constexpr uint32_t rowstride = 32u * NW;              // word (step, w, lane): a warp-wide store is one 128-byte line
     uint32_t* wp = T.bits + T.bits_off[first] + (uint32_t)lane;
 
     const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8;
@@ -122,6 +124,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         if (SLOW && i < 1) {
 #pragma unroll
             for (int k = 0; k < K; ++k) Hn[k] = Hs[k];
+            wp += rowstride;                              // wp follows the STEP, not the row (see the layout above)
             return;
         }
         fv = __vadd2(fv, fstep);

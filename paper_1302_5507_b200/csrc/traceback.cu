@@ -292,7 +292,7 @@ __global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_
     if (local % ppw == 0) {                               // first pair of a task owns the task's region
         int rows = 0;
         for (uint32_t t = 0; t < ppw && local + t < si.count; ++t) rows = max(rows, tb_rows[order[k + t]]);
-        w = (uint32_t)rows * 32u * (uint32_t)((si.K + 3) / 4);
+        w = (uint32_t)(rows + si.G - 1) * 32u * (uint32_t)((si.K + 3) / 4);   // one line set per wavefront step
     }
     words[k] = w;
 }
@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
         else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
         const int w = kk >> 2;
-        const uint32_t word = __ldg(region + ((size_t)(i - 1) * NW + w) * 32u + lane0 + (uint32_t)g);
+        const uint32_t word = __ldg(region + ((size_t)(i - 1 + g) * NW + w) * 32u + lane0 + (uint32_t)g);   // step i + g
         const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u;
         if (st == 0) {
             if ((f & 3u) == 3u) {
