@@ -122,6 +122,38 @@ def test_long_reads(ctx):
     parity.check_batch(ctx, b, DEFAULT, "long reads")
 
 
+def test_band_widths(ctx):
+    # gap bounds W from 0 to ~40 (narrow-band kernels up to W = 23, wide path beyond), reads up to the row limit
+    # of the narrow-band kernels (n + W around 336), indels near both read ends, N on both sides, short windows
+    rng = random.Random(21)
+    reads, wins = [], []
+    for rep in range(1800):
+        n = rng.choice([30, 47, 64, 100, 101, 150, 200, 250, 299, 300, 310, 320, 330, 336])
+        m = n + rng.choice([0, 3, 40, 300])
+        T = [rng.choice("ACGT") for _ in range(m)]
+        if rng.random() < 0.2:
+            a = rng.randrange(m)
+            for k in range(a, min(m, a + rng.randint(1, 12))):
+                T[k] = "N"
+        s = rng.randint(0, m - n)
+        R = T[s:s + n]
+        for _ in range(rng.randint(0, 20)):                       # each substitution widens W by 2
+            R[rng.randrange(n)] = rng.choice("ACGT")
+        for _ in range(rng.randint(0, 2)):
+            k = rng.choice([rng.randint(0, 6), rng.randint(max(0, n - 7), n - 1), rng.randrange(n)])
+            L = rng.randint(1, 12)
+            if rng.random() < 0.5:
+                R = R[:k] + [rng.choice("ACGT") for _ in range(L)] + R[k:]
+            else:
+                R = R[:k] + R[k + L:]
+        R = (R + [rng.choice("ACGT") for _ in range(n)])[:n]
+        R = [c if c != "N" else rng.choice("ACGTN") for c in R]
+        reads.append("".join(R))
+        wins.append("".join(T))
+    b = W.batch_from_strings(wins, reads)
+    parity.check_batch(ctx, b, DEFAULT, "band widths")
+
+
 def test_n_bases_both_sides(ctx):
     rng = random.Random(13)
     reads, wins = [], []
