@@ -134,6 +134,29 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
  * back; `out` then holds pinned HOST pointers owned by the ctx. */
 int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* batch, sdp_result* out);
 
+/*
+ * Step-3 shape ("enumerates candidate regions to be aligned to the whole read using dynamic
+ * programming"; up to a ceiling of candidate regions per read): after sdp_align_batch
+ * has aligned a pair list in which a read appears with several candidate windows, pick per read the best
+ * candidate. The paper does not say how the winner is chosen; the rule here (R16):
+ * highest score; among equal scores the lowest window index; among equal windows the lowest pair index.
+ * DEVICE pointers owned by the ctx, one entry per read of the batch, valid until the next call on the ctx.
+ */
+typedef struct sdp_read_best {
+    const uint32_t* best_pair;      /* index into the pair list, SDP_NO_PAIR if the read is in no pair      */
+    const int32_t*  best_score;     /* score of best_pair (undefined when SDP_NO_PAIR)                      */
+    const int32_t*  second_score;   /* best score among the read's OTHER pairs, INT32_MIN if it has none    */
+    const uint32_t* n_candidates;   /* pairs of the batch that name the read                                */
+    uint32_t        n_reads;
+} sdp_read_best;
+#define SDP_NO_PAIR 0xFFFFFFFFu
+
+/* `batch` (DEVICE pointers) and `result` must be the arguments / output of the last successful
+ * sdp_align_batch on this ctx (sdp_align_batch_host results are host pointers: not accepted). Enqueued on
+ * `cuda_stream`, returns after completion. SDP_EINVAL for null arguments or a result of another batch. */
+int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* result, void* cuda_stream,
+                      sdp_read_best* out);
+
 /* Counters of the last align call on this ctx. */
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);
 

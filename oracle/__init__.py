@@ -9,6 +9,7 @@ from .oracle import (  # noqa: F401
     OracleBatchResult,
     align_pair,
     align_batch,
+    best_per_read,
     build,
     decode_cigar,
 )

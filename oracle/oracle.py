@@ -194,3 +194,31 @@ def align_batch(reads_packed, read_off, read_len, wins_packed, win_off, win_len,
         lib.oracle_batch_free(h)
     r.threads = int(used.value)
     return r
+
+
+def best_per_read(pairs: np.ndarray, score: np.ndarray, n_reads: int) -> dict:
+    """Per-read choice among its candidate windows (TEST INFRASTRUCTURE, R16).
+
+    The paper enumerates up to a ceiling of candidate regions per read and aligns the whole read to each
+     but does not say how the winner is picked. Rule taken: highest score, then
+    lowest window index, then lowest pair index. Written as the definition: one pass over the pairs in
+    order, replacing the incumbent only when strictly better; `second_score` is the best score among the
+    read's other pairs. Plain Python loop on purpose.
+    """
+    NO_PAIR, INT_MIN = 0xFFFFFFFF, -(2 ** 31)
+    best_pair = np.full(n_reads, NO_PAIR, dtype=np.uint32)
+    best_score = np.full(n_reads, INT_MIN, dtype=np.int32)
+    second = np.full(n_reads, INT_MIN, dtype=np.int32)
+    ncand = np.zeros(n_reads, dtype=np.uint32)
+    best_win = [0] * n_reads
+    for p in range(pairs.shape[0]):
+        r, w, s = int(pairs[p, 0]), int(pairs[p, 1]), int(score[p])
+        ncand[r] += 1
+        if best_pair[r] == NO_PAIR:
+            best_pair[r], best_score[r], best_win[r] = p, s, w
+        elif s > best_score[r] or (s == best_score[r] and w < best_win[r]):
+            second[r] = max(int(second[r]), int(best_score[r]))       # the old incumbent becomes an "other" pair
+            best_pair[r], best_score[r], best_win[r] = p, s, w
+        else:
+            second[r] = max(int(second[r]), s)
+    return dict(best_pair=best_pair, best_score=best_score, second_score=second, n_candidates=ncand)

@@ -11,6 +11,7 @@ from .binding import (  # noqa: E402,F401
     Context,
     DeviceBatch,
     HostResult,
+    SDP_NO_PAIR,
     SdpError,
     load_library,
     sdp_measure_dpx_rate,

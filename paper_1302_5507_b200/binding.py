@@ -21,7 +21,7 @@ SDP_MAX_READ_LEN = 1024
 SDP_MAX_CELL_VALUE = 16000
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
-           "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version"]
+           "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read"]
 
 
 class SdpError(RuntimeError):
@@ -49,6 +49,14 @@ class sdp_result(ctypes.Structure):
                 ("n_match", ctypes.c_void_p), ("n_cols", ctypes.c_void_p), ("cigar_off", ctypes.c_void_p),
                 ("cigar_len", ctypes.c_void_p), ("cigar_ops", ctypes.c_void_p), ("n_cigar_ops", ctypes.c_uint64),
                 ("n_pairs", ctypes.c_uint64)]
+
+
+class sdp_read_best(ctypes.Structure):
+    _fields_ = [("best_pair", ctypes.c_void_p), ("best_score", ctypes.c_void_p), ("second_score", ctypes.c_void_p),
+                ("n_candidates", ctypes.c_void_p), ("n_reads", ctypes.c_uint32)]
+
+
+SDP_NO_PAIR = 0xFFFFFFFF
 
 
 class sdp_stats(ctypes.Structure):
@@ -82,6 +90,9 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
                                     ctypes.POINTER(sdp_result)]
     lib.sdp_align_batch_host.restype = ctypes.c_int
     lib.sdp_align_batch_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result)]
+    lib.sdp_best_per_read.restype = ctypes.c_int
+    lib.sdp_best_per_read.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result),
+                                      ctypes.c_void_p, ctypes.POINTER(sdp_read_best)]
     lib.sdp_get_stats.restype = ctypes.c_int
     lib.sdp_get_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_stats)]
     lib.sdp_set_timing.restype = ctypes.c_int
@@ -277,6 +288,26 @@ class Context:
                           down(res.n_match, P, np.int32), down(res.n_cols, P, np.int32),
                           down(res.cigar_off, P, np.uint64), down(res.cigar_len, P, np.uint32),
                           down(res.cigar_ops, n_ops, np.uint32))
+
+    def best_per_read(self, dbatch: DeviceBatch, res: sdp_result, stream=None) -> dict:
+        """sdp_best_per_read on the result of the last align_batch; returns host numpy arrays."""
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        rb = sdp_read_best()
+        self._check(self._lib.sdp_best_per_read(self._h, ctypes.byref(dbatch.c), ctypes.byref(res),
+                                                ctypes.c_void_p(stream.cuda_stream), ctypes.byref(rb)))
+        cudart, R = _cudart(), int(rb.n_reads)
+
+        def down(ptr, dtype):
+            out = np.zeros(R, dtype=dtype)
+            if R and int(cudart.cudaMemcpy(ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(ptr),
+                                           ctypes.c_size_t(out.nbytes), 2)) != 0:
+                raise SdpError(SDP_ECUDA, "cudaMemcpy D2H failed")
+            return out
+
+        return dict(best_pair=down(rb.best_pair, np.uint32), best_score=down(rb.best_score, np.int32),
+                    second_score=down(rb.second_score, np.int32), n_candidates=down(rb.n_candidates, np.uint32))
 
     # -- host path
     def align_batch_host(self, batch) -> HostResult:

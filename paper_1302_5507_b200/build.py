@@ -43,7 +43,7 @@ def _deps_hash(extra: str) -> str:
 
 def _units():
     units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []), ("thin_kernel", "thin_kernel.cu", []),
-             ("microbench", "microbench.cu", [])]
+             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"score_r{r}", "score_inst.cu",
                       [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_K_FN=launch_score_r{r}",
@@ -73,8 +73,16 @@ def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -
         return obj
 
     jobs = jobs or min(12, (os.cpu_count() or 4))
+    units = _units()
+    only = os.environ.get("SDP_BUILD_UNITS")          # development: recompile just these units, reuse the other objects
+    if only:
+        names = set(only.split(","))
+        todo = [u for u in units if u[0] in names or not os.path.exists(os.path.join(OBJ, u[0] + ".o"))]
+    else:
+        todo = units
     with ThreadPoolExecutor(max_workers=jobs) as ex:
-        objs = list(ex.map(compile_one, _units()))
+        list(ex.map(compile_one, todo))
+    objs = [os.path.join(OBJ, u[0] + ".o") for u in units]
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs]
     r = subprocess.run(cmd, capture_output=True, text=True)
@@ -82,7 +90,7 @@ def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, LIB)
     with open(stamp, "w") as f:
-        f.write(want)
+        f.write(want if not only else "partial build")
     return LIB
 
 

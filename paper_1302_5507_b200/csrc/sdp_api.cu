@@ -100,6 +100,10 @@ struct sdp_ctx {
     // sdp_align_batch_host: device copies of the inputs and pinned host copies of the outputs
     DevBuf in_reads, in_read_off, in_read_len, in_read_nmask, in_wins, in_win_off, in_win_len, in_win_nmask, in_pairs;
     DevBuf h_out;                    // one pinned slab, carved per call
+    // sdp_best_per_read
+    DevBuf rb_key, rb_pair, rb_score, rb_second, rb_ncand;
+    const uint32_t* last_pairs = nullptr;   // pair list of the last successful align call (to match results to it)
+    uint64_t last_n_pairs = 0;
 };
 
 namespace {
@@ -293,7 +297,8 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->bits, &ctx->ops_rev, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
                       &ctx->in_win_nmask, &ctx->in_pairs, &ctx->tb_rows, &ctx->keys_wide, &ctx->order_wide,
-                      &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits};
+                      &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits,
+                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
     for (int i = 0; i < 4; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
@@ -427,6 +432,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (P == 0) {
         EN(cigar_ops, 16);
         ctx->stats = stats;
+        ctx->last_pairs = b.pairs; ctx->last_n_pairs = 0;
         finish(0);
         return SDP_OK;
     }
@@ -600,7 +606,32 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         cudaEventElapsedTime(&stats.ms_compact, ctx->ev[EV_TRACE], ctx->ev[EV_END]);
     }
     ctx->stats = stats;
+    ctx->last_pairs = b.pairs; ctx->last_n_pairs = P;
     finish(ctx->mb->totals[2]);
+    return SDP_OK;
+}
+
+int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* result, void* cuda_stream,
+                      sdp_read_best* out)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!batch || !result || !out) return fail(ctx, SDP_EINVAL, "null batch, result or output");
+    if (result->score != ctx->score.as<int32_t>() || result->n_pairs != batch->n_pairs ||
+        batch->pairs != ctx->last_pairs || batch->n_pairs != ctx->last_n_pairs)
+        return fail(ctx, SDP_EINVAL, "result does not belong to the last sdp_align_batch of this ctx on this batch");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->device));
+    const size_t R = batch->n_reads ? batch->n_reads : 1;
+    EN(rb_key, R * 8); EN(rb_pair, R * 4); EN(rb_score, R * 4); EN(rb_second, R * 4); EN(rb_ncand, R * 4);
+    launch_best_per_read(batch->n_pairs, batch->n_reads, batch->pairs, result->score,
+                         ctx->rb_key.as<unsigned long long>(), ctx->rb_pair.as<uint32_t>(), ctx->rb_score.as<int32_t>(),
+                         ctx->rb_second.as<int32_t>(), ctx->rb_ncand.as<uint32_t>(), st);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    out->best_pair = ctx->rb_pair.as<uint32_t>(); out->best_score = ctx->rb_score.as<int32_t>();
+    out->second_score = ctx->rb_second.as<int32_t>(); out->n_candidates = ctx->rb_ncand.as<uint32_t>();
+    out->n_reads = batch->n_reads;
     return SDP_OK;
 }
 

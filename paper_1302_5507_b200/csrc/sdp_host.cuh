@@ -95,6 +95,11 @@ int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t 
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 
+// ---- best_read.cu
+void launch_best_per_read(uint64_t n_pairs, uint32_t n_reads, const uint32_t* pairs, const int32_t* score,
+                          unsigned long long* key, uint32_t* best_pair, int32_t* best_score, int32_t* second,
+                          uint32_t* ncand, cudaStream_t st);
+
 // ---- microbench.cu
 int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz);
 

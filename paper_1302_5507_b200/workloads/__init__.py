@@ -267,3 +267,35 @@ def make_config(cfg: int, n_pairs: Optional[int] = None, ref_bases: Optional[int
                  wins_out if P.private_windows else ref_packed, win_off, win_len, pairs,
                  None, None if P.private_windows else ref_nmask,
                  name=f"cfg{cfg}", meta=dict(cfg=cfg, n_pairs=n_pairs, ref_bases=ref_bases, seed=seed))
+
+
+def make_step3(n_reads: int, max_candidates: int = 30, ref_bases: Optional[int] = None,
+               seed: Optional[int] = None) -> Batch:
+    """Step-3 shape: each read against up to ``max_candidates`` candidate windows.
+
+    Reads and their true windows come from the config-2 generator (100 bp reads, 500 bp windows cut from
+    the seeded reference). Every read gets c ~ U{1..max_candidates} candidates: its true window, up to two
+    windows shifted by +-U{20..150} bases (overlapping the true locus, so scores tie or nearly tie), and
+    uniformly placed decoys. Windows are views into the packed reference; the pair list is grouped by read
+    with the candidates of a read in random order. No alignment arithmetic here.
+    """
+    base = make_config(2, n_pairs=n_reads, ref_bases=ref_bases, seed=seed)
+    rng = np.random.default_rng(SEED_BASE + 77 if seed is None else int(seed) + 77)
+    ref_len = int(base.wins_packed.shape[0]) * 16 - 64
+    m = int(base.win_len[0])
+    ncand = rng.integers(1, max_candidates + 1, size=n_reads)
+    total = int(ncand.sum())
+    read_idx = np.repeat(np.arange(n_reads, dtype=np.uint32), ncand)
+    first = np.concatenate([[0], np.cumsum(ncand)[:-1]])
+    slot = np.arange(total) - np.repeat(first, ncand)            # 0 = true window, 1..2 = shifted, rest decoys
+    true_off = base.win_off[read_idx].astype(np.int64)
+    shift = rng.integers(20, 151, size=total) * rng.choice([-1, 1], size=total)
+    decoy = rng.integers(0, max(1, ref_len - m), size=total)
+    off = np.where(slot == 0, true_off, np.where(slot <= 2, true_off + shift, decoy))
+    off = np.clip(off, 0, max(0, ref_len - m)).astype(np.uint64)
+    order = np.lexsort((rng.random(total), read_idx))            # shuffle inside each read's group
+    win_off = np.ascontiguousarray(off[order])
+    pairs = np.ascontiguousarray(np.stack([read_idx[order], np.arange(total, dtype=np.uint32)], axis=1))
+    return Batch(base.reads_packed, base.read_off, base.read_len, base.wins_packed, win_off,
+                 np.full(total, m, dtype=np.uint32), pairs, base.read_nmask, base.win_nmask,
+                 f"step3[{n_reads} reads x <= {max_candidates}]", dict(base.meta))
