@@ -157,6 +157,12 @@ typedef struct sdp_read_best {
 int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* result, void* cuda_stream,
                       sdp_read_best* out);
 
+/* Candidate screening for the step-3 shape: with score-only on (1), sdp_align_batch / sdp_align_batch_host stop
+ * after the forward score pass (a1-a3): `score` and `ref_end` are as always, `ref_start` and `read_end` are -1,
+ * `read_start`, `n_match`, `n_cols`, `pass`, `cigar_len`, `cigar_off` are 0 and n_cigar_ops is 0. A caller scores every
+ * candidate this way, picks winners with sdp_best_per_read and aligns only those with score-only off (0, default). */
+int sdp_set_score_only(sdp_ctx* ctx, int enabled);
+
 /* Counters of the last align call on this ctx. */
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);
 

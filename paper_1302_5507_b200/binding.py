@@ -21,7 +21,8 @@ SDP_MAX_READ_LEN = 1024
 SDP_MAX_CELL_VALUE = 16000
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
-           "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read"]
+           "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
+           "sdp_set_score_only"]
 
 
 class SdpError(RuntimeError):
@@ -93,6 +94,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_best_per_read.restype = ctypes.c_int
     lib.sdp_best_per_read.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result),
                                       ctypes.c_void_p, ctypes.POINTER(sdp_read_best)]
+    lib.sdp_set_score_only.restype = ctypes.c_int
+    lib.sdp_set_score_only.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_get_stats.restype = ctypes.c_int
     lib.sdp_get_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_stats)]
     lib.sdp_set_timing.restype = ctypes.c_int
@@ -220,6 +223,9 @@ class Context:
 
     def set_timing(self, enabled: bool):
         self._lib.sdp_set_timing(self._h, int(bool(enabled)))
+
+    def set_score_only(self, enabled: bool):
+        self._lib.sdp_set_score_only(self._h, int(bool(enabled)))
 
     def stats(self) -> dict:
         s = sdp_stats()

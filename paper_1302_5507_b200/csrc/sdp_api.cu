@@ -69,6 +69,7 @@ struct sdp_ctx {
     int no_thin = 0;                 // SDP_NO_THIN=1: keep W >= 1 pairs off the narrow-band kernel (debugging)
     char err[512] = {0};
     bool timing = false;
+    bool score_only = false;         // sdp_set_score_only: stop after the forward pass
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
     uint32_t cls_begin[2 * SDP_MAX_K + 3];   // first slot of class c = 2K + padded; [c+1] ends it
@@ -327,6 +328,13 @@ int sdp_set_timing(sdp_ctx* ctx, int enabled)
     return SDP_OK;
 }
 
+int sdp_set_score_only(sdp_ctx* ctx, int enabled)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->score_only = enabled != 0;
+    return SDP_OK;
+}
+
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out)
 {
     if (!ctx || !out) return SDP_EINVAL;
@@ -466,6 +474,34 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         stats.forward_launches = nl - before;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_FORWARD], st));
+
+    if (ctx->score_only) {
+        // candidate screening (step-3 shape): score and ref_end only; everything the traceback would fill reads
+        // as "no alignment" (ref_start -1, no CIGAR, pass 0)
+        EN(cigar_ops, 16);
+        CU(cudaMemsetAsync(ctx->ref_start.p, 0xFF, P * 4, st));
+        CU(cudaMemsetAsync(ctx->read_start.p, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->read_end.p, 0xFF, P * 4, st));
+        CU(cudaMemsetAsync(ctx->pass.p, 0, P, st));
+        CU(cudaMemsetAsync(ctx->n_match.p, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->n_cols.p, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->cigar_off.p, 0, P * 8, st));
+        CU(cudaMemsetAsync(ctx->cigar_len.p, 0, P * 4, st));
+        CU(cudaMemcpyAsync(ctx->mb->counters + 3, ctx->counters + 3, 8, cudaMemcpyDeviceToHost, st));
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
+        CU(cudaStreamSynchronize(st));
+        stats.cells_forward = ctx->mb->counters[3];
+        stats.kernel_launches = nl;
+        if (ctx->timing) {
+            cudaEventElapsedTime(&stats.ms_total, ctx->ev[EV_START], ctx->ev[EV_END]);
+            cudaEventElapsedTime(&stats.ms_bucket, ctx->ev[EV_START], ctx->ev[EV_BUCKET]);
+            cudaEventElapsedTime(&stats.ms_forward, ctx->ev[EV_BUCKET], ctx->ev[EV_FORWARD]);
+        }
+        ctx->stats = stats;
+        ctx->last_pairs = b.pairs; ctx->last_n_pairs = P;
+        finish(0);
+        return SDP_OK;
+    }
 
     // ---- gap bound W, keys of the two later stages, scratch sizes
     PostParams pp{};

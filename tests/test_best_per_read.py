@@ -86,3 +86,32 @@ def test_gpu_best_per_read_rejects_foreign_result():
         ctx.align_batch(d2)
         with pytest.raises(SdpError):
             ctx.best_per_read(d1, r1)
+
+
+@pytest.mark.gpu
+def test_gpu_screen_then_align_winners():
+    # the step-3 flow: score every candidate (forward pass only), choose per read, align only the winners
+    from paper_1302_5507_b200 import Context
+    sc = OracleScoring()
+    b = W.make_step3(400, max_candidates=30, ref_bases=1_000_000)
+    full = oracle.align_batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len, b.pairs, sc,
+                              threads=4)
+    exp_best = oracle.best_per_read(b.pairs, full.score, len(b.read_len))
+    with Context(device=0) as ctx:
+        ctx.set_score_only(True)
+        db = ctx.upload(b)
+        res = ctx.align_batch(db)
+        scr = ctx.fetch(res)
+        assert np.array_equal(scr.score, full.score) and np.array_equal(scr.ref_end, full.ref_end)
+        assert not scr.cigar_len.any() and not scr.passed.any() and (scr.ref_start == -1).all() and len(scr.cigar_ops) == 0
+        best = ctx.best_per_read(db, res)
+        for k in exp_best:
+            assert np.array_equal(exp_best[k].astype(np.int64), best[k].astype(np.int64)), k
+        ctx.set_score_only(False)
+        winners = b.subset(best["best_pair"].astype(np.int64))
+        got = ctx.fetch(ctx.align_batch(ctx.upload(winners)))
+    w = best["best_pair"].astype(np.int64)
+    for f in ("score", "ref_start", "ref_end", "n_match", "n_cols", "passed", "cigar_len"):
+        assert np.array_equal(np.asarray(getattr(full, f))[w].astype(np.int64), getattr(got, f).astype(np.int64)), f
+    for i, p in enumerate(w):
+        assert full.cigar(int(p)) == got.cigar(i)
