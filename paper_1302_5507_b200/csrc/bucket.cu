@@ -50,18 +50,6 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
     if ((threadIdx.x & 31) == 0 && my_cells) atomicAdd(cells, my_cells);
 }
 
-// histogram of precomputed keys (stages after the forward pass)
-__global__ void k_hist(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ hist)
-{
-    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint32_t key = p < n ? keys[p] : SDP_KEY_SKIP;
-    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
-    if (key != SDP_KEY_SKIP) {
-        const uint32_t peers = __match_any_sync(active, key);
-        if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t block_exclusive_scan_1024(uint32_t v, uint32_t* total)
 {
@@ -281,11 +269,6 @@ void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, 
 {
     const uint32_t grid = (uint32_t)((b.n_pairs + 255) / 256);
     k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells);
-}
-
-void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t st)
-{
-    k_hist<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist);
 }
 
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,

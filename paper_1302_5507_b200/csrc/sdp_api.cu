@@ -95,9 +95,10 @@ struct sdp_ctx {
     // per-pair device buffers (grow only)
     DevBuf keys, pn, pm, order, desc, order_rev, desc_rev, order_tb, keys_rev, keys_tb, tbW, rev_rows,
         tb_rows, keys_wide, order_wide, desc_wide, wide_words, wide_off, wide_bits,
-        bits_words, ops_cap, bits_off, ops_off, scan_local, scan_tiles, scan_tile_base,
+        bits_words, ops_cap, bits_off, ops_off,
         score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len,
         bits, ops_rev, cigar_ops;
+    DevBuf scan_local[3], scan_tiles[3], scan_tile_base[3];   // one set per concurrent scan
     // sdp_align_batch_host: device copies of the inputs and pinned host copies of the outputs
     DevBuf in_reads, in_read_off, in_read_len, in_read_nmask, in_wins, in_win_off, in_win_len, in_win_nmask, in_pairs;
     DevBuf h_out;                    // one pinned slab, carved per call
@@ -292,8 +293,9 @@ void sdp_destroy(sdp_ctx* ctx)
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->order_rev, &ctx->desc_rev,
                       &ctx->order_tb, &ctx->keys_rev, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
-                      &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local, &ctx->scan_tiles,
-                      &ctx->scan_tile_base, &ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start,
+                      &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local[0], &ctx->scan_local[1], &ctx->scan_local[2],
+                      &ctx->scan_tiles[0], &ctx->scan_tiles[1], &ctx->scan_tiles[2], &ctx->scan_tile_base[0],
+                      &ctx->scan_tile_base[1], &ctx->scan_tile_base[2], &ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start,
                       &ctx->read_end, &ctx->pass, &ctx->n_match, &ctx->n_cols, &ctx->cigar_off, &ctx->cigar_len,
                       &ctx->bits, &ctx->ops_rev, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
@@ -425,7 +427,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     EN(tb_rows, Pp * 4); EN(keys_wide, Pp * 4); EN(order_wide, Pp * 4); EN(desc_wide, Pp * sizeof(PairDesc));
     EN(wide_words, Pp * 4); EN(wide_off, Pp * 8);
     EN(bits_words, Pp * 4); EN(ops_cap, Pp * 4); EN(bits_off, Pp * 8); EN(ops_off, Pp * 8);
-    EN(scan_local, Pp * 4); EN(scan_tiles, (Pp / 4096 + 2) * 4); EN(scan_tile_base, (Pp / 4096 + 2) * 8);
+    for (int k = 0; k < 3; ++k) { EN(scan_local[k], Pp * 4); EN(scan_tiles[k], (Pp / 4096 + 2) * 4); EN(scan_tile_base[k], (Pp / 4096 + 2) * 8); }
     EN(score, Pp * 4); EN(ref_start, Pp * 4); EN(ref_end, Pp * 4); EN(read_start, Pp * 4); EN(read_end, Pp * 4);
     EN(pass, Pp); EN(n_match, Pp * 4); EN(n_cols, Pp * 4); EN(cigar_off, Pp * 8); EN(cigar_len, Pp * 4);
 
@@ -514,30 +516,39 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
     pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
+    // The three bucket sorts and the three scratch-offset scans are short, latency-bound launch chains that
+    // depend only on k_post_forward: they fan out over the helper streams and join before the mailbox kernel.
+    cudaStream_t f1 = ctx->fan_stream[1], f2 = ctx->fan_stream[2], f3 = ctx->fan_stream[3];
+    CU(cudaEventRecord(ctx->fan_fork, st));
+    for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_stream[k], ctx->fan_fork, 0));
     launch_sort_tail(ctx->keys_rev.as<uint32_t>(), P, ctx->hist[1], ctx->bin_start[1], ctx->order_rev.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1],
-                     ctx->mb->task_prefix[1], &ctx->mb->bin_total[1], st);
+                     ctx->mb->task_prefix[1], &ctx->mb->bin_total[1], f1);
     launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
-                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, st);
+                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, f2);
     launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2],
                      ctx->mb->task_prefix[2], &ctx->mb->bin_total[3], st);
     nl += 12;
-    // one region of direction nibbles per two wide pairs that share the int16x2 lanes (every slot of
-    // order_wide beyond the wide pairs reads as a zero-size region)
+    // one region of direction nibbles per warp task of wide pairs (every slot of order_wide beyond the wide
+    // pairs reads as a zero-size region)
     CU(cudaMemsetAsync(ctx->wide_words.p, 0, P * 4, st));
     launch_wide_regions(ctx->order_wide.as<uint32_t>(), (uint32_t)P, ctx->bin_start[3] + SDP_NBINS, ctx->pn.as<uint32_t>(),
                         ctx->tb_rows.as<int32_t>(), ctx->d_slot_of_n, ctx->slots[2], ctx->wide_words.as<uint32_t>(), st);
     ++nl;
     exclusive_scan_u32_u64(ctx->wide_words.as<uint32_t>(), P, ctx->wide_off.as<uint64_t>(), ctx->totals + 3,
-                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
-                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
+                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
     exclusive_scan_u32_u64(ctx->bits_words.as<uint32_t>(), P, ctx->bits_off.as<uint64_t>(), ctx->totals + 0,
-                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
-                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+                           ctx->scan_local[1].as<uint32_t>(), ctx->scan_tiles[1].as<uint32_t>(),
+                           ctx->scan_tile_base[1].as<uint64_t>(), f2, &nl);
     exclusive_scan_u32_u64(ctx->ops_cap.as<uint32_t>(), P, ctx->ops_off.as<uint64_t>(), ctx->totals + 1,
-                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
-                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+                           ctx->scan_local[2].as<uint32_t>(), ctx->scan_tiles[2].as<uint32_t>(),
+                           ctx->scan_tile_base[2].as<uint64_t>(), f3, &nl);
+    for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
+        CU(cudaEventRecord(ctx->fan_join[k], ctx->fan_stream[k]));
+        CU(cudaStreamWaitEvent(st, ctx->fan_join[k], 0));
+    }
     launch_mailbox(ctx->bin_start[2], TB_KEY_STRIDE, THIN_NW + TB_NCLASS + 1, ctx->totals, ctx->counters,
                    ctx->mb->tb_bounds, ctx->mb->totals, ctx->mb->counters, st);
     ++nl;
@@ -612,8 +623,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     // ---- a7 compaction in caller pair order
     exclusive_scan_u32_u64(ctx->cigar_len.as<uint32_t>(), P, ctx->cigar_off.as<uint64_t>(), ctx->totals + 2,
-                           ctx->scan_local.as<uint32_t>(), ctx->scan_tiles.as<uint32_t>(),
-                           ctx->scan_tile_base.as<uint64_t>(), st, &nl);
+                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
+                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
     launch_compact(P, ctx->ops_off.as<uint64_t>(), ctx->ops_rev.as<uint32_t>(), ctx->cigar_len.as<uint32_t>(),
                    ctx->cigar_off.as<uint64_t>(), ctx->cigar_ops.as<uint32_t>(), st);
     ++nl;
@@ -622,9 +633,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
-    if ((ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE)) && getenv("SDP_DEBUG_NOFAIL"))
-        fprintf(stderr, "[sdp] internal flags 0x%x ignored (SDP_DEBUG_NOFAIL)\n", ctx->mb->err_flag);
-    else if (ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
+    if (ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
         return fail(ctx, SDP_ECUDA, "internal consistency check failed (flags 0x%x): reverse pass or traceback "
                     "disagrees with the forward score", ctx->mb->err_flag);
 
@@ -683,8 +692,6 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
     CU(cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->own_stream;
     sdp_batch d = *hb;
-    auto words16 = [](uint64_t bases) { return (size_t)(((bases + 15) / 16 + 3) / 4 * 4); };
-    auto words32 = [](uint64_t bases) { return (size_t)(((bases + 31) / 32 + 3) / 4 * 4); };
     struct Cp { DevBuf* buf; const void* src; size_t bytes; const void** dst; };
     // the caller's buffers are only guaranteed readable to the end of the last word in use
     const size_t rb = (size_t)((hb->reads_bases + 15) / 16) * 4, wb = (size_t)((hb->wins_bases + 15) / 16) * 4;
@@ -700,7 +707,6 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
         {&ctx->in_win_nmask, hb->win_nmask, wnb, (const void**)&d.win_nmask},
         {&ctx->in_pairs, hb->pairs, (size_t)P * 8, (const void**)&d.pairs},
     };
-    (void)words16; (void)words32;
     for (Cp& c : cps) {
         if (!c.src) { *c.dst = nullptr; continue; }
         int rc = ensure(ctx, *c.buf, c.bytes + 64);

@@ -13,7 +13,6 @@ struct Scoring {
 // ---- bucket.cu
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st);
-void launch_hist(const uint32_t* keys, uint64_t n, uint32_t* hist, cudaStream_t st);
 // scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
