@@ -228,7 +228,7 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         const int sc8 = SDP_TB_SCALE;
         const int qm = sc8 * (2 * e + s->match) + 7, qx = sc8 * (2 * e + s->mismatch) + 7;
         TraceConsts& t = ctx->tconsts;
-        t.m4 = 0x00040004u;
+        t.m4 = 0x00040004u; t.cm1 = 0xFFFFFFFFu;
         t.negO_e = sdp_pack2(-sc8 * o + 1);
         t.negO_f = sdp_pack2(-sc8 * o + 6);
         t.qx = sdp_pack2(qx);

@@ -79,6 +79,7 @@ struct ScoreParams {
 #define SDP_TB_SCALE 8
 #define SDP_TB_MAX_VALUE 4090   // largest unscaled drift-form value: 8 * 4090 + 7 <= 32767
 struct TraceConsts {
+    uint32_t cm1;                  // 0xFFFFFFFF (-1), opaque multiplier: subtractions as IMAD on the FMA pipe
     uint32_t m4;                   // 0x00040004, opaque so that the tag select stays one LOP3
     uint32_t negO_e;               // 8 * (-o) + 1 : "I opened here" candidate (tag bit 0)
     uint32_t negO_f;               // 8 * (-o) + 6 : "D opened here" candidate (tag bit 2); D extended carries tag 2

@@ -37,6 +37,9 @@
 namespace sdp {
 
 // bitwise (mask ? b : a) in one LOP3 (mask kept in a register: a LOP3 takes one immediate at most)
+__device__ __forceinline__ uint32_t imad_u(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r; asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c)); return r;
+}
 __device__ __forceinline__ uint32_t lop3_select(uint32_t a, uint32_t b, uint32_t mask) {
     uint32_t r; asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(r) : "r"(a), "r"(b), "r"(mask)); return r;
 }
@@ -107,7 +110,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     constexpr uint32_t rowstride = 32u * NW;              // word (step, w, lane): a warp-wide store is one 128-byte line
     uint32_t* wp = T.bits + T.bits_off[first] + (uint32_t)lane;
 
-    const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8;
+    const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8, cm1 = T.c.cm1;
     const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, e2 = T.c.e2;
     constexpr uint32_t H2_8 = 0x48004800u, H2_16 = 0x4C004C00u;        // fp16 8.0 and 16.0, both lanes
     const uint32_t notfirst = opaque_u32(is_first ? 0u : 0xFFFFFFFFu);   // a mask, not a predicate: one LOP3 per use
@@ -152,8 +155,10 @@ trace_kernel(const ScoreParams P, const TraceDP T)
             Hl = Ht & 0xFFF8FFF8u;
             Hn[k] = Hl;
             const uint32_t v = lop3_select(Ht, Ft, m4);
-            const uint32_t nib = v & 0x00070007u;         // bits 2..0
-            const uint32_t eb = Et & 0x00010001u;         // 0 or 1
+            // v - Hc and Et - Ec as 32-bit IMADs (no borrow crosses the lanes: Hc <= v, Ec <= Et per lane). An IMAD
+            // costs two FMA-pipe slots, but the ALU pipe is this kernel's bottleneck and the FMA pipe has room.
+            const uint32_t nib = imad_u(Hl, cm1, v);      // bits 2..0
+            const uint32_t eb = imad_u(E, cm1, Et);       // 0 or 1
             const uint32_t t = hfma2_u(eb, H2_8, nib);    // nib + 8 eb as fp16 denormals: exact
             if ((k & 1) == 0) t0 = t;
             if ((k & 1) == 1 || k == K - 1) {
