@@ -21,9 +21,9 @@
 //     Ec = Et & ~1, Fc = Ft & ~4, Hc = Ht & ~7            3 LOP3      clean values for the next cell
 //     v  = Ht & ~4 | Ft & 4                               1 LOP3
 // Eight ALU-pipe instructions per two cells (two pairs share the int16x2 lanes) against four in
-// the score kernel. The nibble (v - Hc) + 8 (Et - Ec) and its packing run on the FMA pipe without
-// any IMAD (an IMAD costs two HFMA2 slots on sm_100a; a packed subtraction costs a LOP3 and two
-// VIADD.16x2, so the tags are masked out with two more LOP3 instead): fp16
+// the score kernel. The nibble (v - Hc) + 8 (Et - Ec) and its packing run on the FMA pipe: the two
+// subtractions are 32-bit IMADs (an IMAD costs two HFMA2 slots on sm_100a, but masking the tags out with
+// two more LOP3 instead loads the ALU pipe, which is this kernel's bottleneck: measured 6 % slower), then fp16
 // FMAs on the small integers as DENORMALS (t = eb*8 + nib, byte = t0*16 + t1: exact below 2048),
 // and one PRMT per four cells joins two bytes. Nibbles are left-aligned, four cells per 16-bit
 // lane (cell kk of a word in bits 4*(3 - kk)), and stored row by row:
