@@ -258,9 +258,11 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaMallocHost(&ctx->mb, sizeof(Mailbox)));
         memset(ctx->mb, 0, sizeof(Mailbox));
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
-        CU(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+        int prio_lo = 0, prio_hi = 0;                 // narrow-band work fills the gaps of the (critical) wide path
+        CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+        CU(cudaStreamCreateWithPriority(&ctx->side_stream, cudaStreamNonBlocking, prio_lo));
         CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
-        CU(cudaStreamCreateWithFlags(&ctx->side_stream2, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithPriority(&ctx->side_stream2, cudaStreamNonBlocking, prio_lo));
         CU(cudaEventCreateWithFlags(&ctx->fan_fork, cudaEventDisableTiming));
         for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
             CU(cudaStreamCreateWithFlags(&ctx->fan_stream[k], cudaStreamNonBlocking));
@@ -560,31 +562,6 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
     EN(wide_bits, (ctx->mb->totals[3] + 4) * 4);
 
-    // ---- a5 + a6, narrow bands (W <= 7: one thread per pair, band in registers) and the generic band kernel.
-    // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on a
-    // side stream beside it (the stream synchronisation above has completed everything they read).
-    cudaStream_t ss = ctx->side_stream;
-    TraceParams tp{};
-    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
-    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
-    tp.rev_rows = nullptr;
-    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
-    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
-    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
-    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
-    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
-    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream2);
-    CU(cudaEventRecord(ctx->side_done2, ctx->side_stream2));
-    for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
-        tp.first = ctx->mb->tb_bounds[c];
-        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
-        if (!tp.count) continue;
-        launch_traceback(c - THIN_NW, tp, ss);
-        ++nl;
-    }
-    CU(cudaEventRecord(ctx->side_done, ss));
-
     // ---- a4 reverse pass over the pairs whose score admits a gap
     launch_fill_desc_rev(b, ctx->order_rev.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
                          ctx->tbW.as<int32_t>(), ctx->desc_rev.as<PairDesc>(), st);
@@ -616,6 +593,31 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         launch_walk(wp, st);
         ++nl;
     }
+    // ---- a5 + a6, narrow bands (W <= 7: one thread per pair, band in registers) and the generic band kernel.
+    // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on a
+    // side stream beside it (the stream synchronisation above has completed everything they read).
+    cudaStream_t ss = ctx->side_stream;
+    TraceParams tp{};
+    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
+    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
+    tp.rev_rows = nullptr;
+    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
+    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
+    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
+    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
+    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
+    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
+    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream2);
+    CU(cudaEventRecord(ctx->side_done2, ctx->side_stream2));
+    for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
+        tp.first = ctx->mb->tb_bounds[c];
+        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
+        if (!tp.count) continue;
+        launch_traceback(c - THIN_NW, tp, ss);
+        ++nl;
+    }
+    CU(cudaEventRecord(ctx->side_done, ss));
+
     CU(cudaStreamWaitEvent(st, ctx->side_done, 0));
     CU(cudaStreamWaitEvent(st, ctx->side_done2, 0));
     CU(cudaGetLastError());
