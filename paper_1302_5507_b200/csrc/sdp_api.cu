@@ -509,7 +509,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     // ---- gap bound W, keys of the two later stages, scratch sizes
     PostParams pp{};
-    pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
+    pp.b = b; pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
     pp.score = ctx->score.as<int32_t>(); pp.ref_end = ctx->ref_end.as<int32_t>();
     pp.tbW = ctx->tbW.as<int32_t>(); pp.tb_rows = ctx->tb_rows.as<int32_t>();
     pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();

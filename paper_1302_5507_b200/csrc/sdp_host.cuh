@@ -31,6 +31,7 @@ void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaS
 
 // ---- traceback.cu
 struct PostParams {
+    sdp_batch b;                 // sequences, for the ungapped shortcut
     uint64_t n_pairs;
     Scoring sc;
     const uint32_t* pn; const uint32_t* pm;      // per pair read / window length

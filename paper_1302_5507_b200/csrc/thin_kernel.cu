@@ -10,40 +10,13 @@
 // (hardware-interleaved, hence coalesced) local-memory array; the walk of PAPER.md:353 /
 // DESIGN.md R6 then reads them back. Nothing of this uses the reverse pass.
 #include "sdp_host.cuh"
+#include "seq_bits.cuh"
 
 namespace sdp {
 
 namespace {
 
 constexpr int TNEG = -(1 << 28);                  // "minus infinity", a multiple of 8
-
-// 16 consecutive 2-bit bases starting at base position pos; words outside [0, nwords) read as 0
-__device__ __forceinline__ uint32_t bases16(const uint32_t* __restrict__ packed, long long pos, long long nwords) {
-    const long long w = pos >> 4;
-    const uint32_t sh = ((uint32_t)pos & 15u) * 2u;
-    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(packed + w) : 0u;
-    const uint32_t hi = (sh != 0u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(packed + w + 1) : 0u;
-    return __funnelshift_r(lo, hi, sh);
-}
-// 16 consecutive mask bits starting at bit position pos, spread to the even bit positions
-__device__ __forceinline__ uint32_t nbits16_spread(const uint32_t* __restrict__ bits, long long pos, long long nwords) {
-    if (bits == nullptr) return 0u;
-    const long long w = pos >> 5;
-    const uint32_t sh = (uint32_t)pos & 31u;
-    const uint32_t lo = (w >= 0 && w < nwords) ? __ldg(bits + w) : 0u;
-    const uint32_t hi = (sh > 16u && w + 1 >= 0 && w + 1 < nwords) ? __ldg(bits + w + 1) : 0u;
-    uint32_t x = __funnelshift_r(lo, hi, sh) & 0xFFFFu;
-    x = (x | (x << 8)) & 0x00FF00FFu;
-    x = (x | (x << 4)) & 0x0F0F0F0Fu;
-    x = (x | (x << 2)) & 0x33333333u;
-    x = (x | (x << 1)) & 0x55555555u;
-    return x;
-}
-// even bit 2k set iff base k of a and of b are equal (N never equal)
-__device__ __forceinline__ uint32_t eq16(uint32_t a, uint32_t b, uint32_t nmask_spread) {
-    const uint32_t x = a ^ b;
-    return ~(x | (x >> 1) | nmask_spread) & 0x55555555u;
-}
 
 __device__ __forceinline__ int base_at(const uint32_t* __restrict__ packed, const uint32_t* __restrict__ nmask,
                                        uint64_t pos, int ncode) {

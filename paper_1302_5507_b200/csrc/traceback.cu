@@ -9,6 +9,7 @@
 // "extended") resolve exactly as in the full-table oracle.
 // W == 0 means the alignment is gapless: CIGAR nM, no DP at all.
 #include "sdp_host.cuh"
+#include "seq_bits.cuh"
 
 namespace sdp {
 
@@ -53,6 +54,19 @@ __global__ void k_post_forward(const PostParams pp)
         const int slack = n * pp.sc.match - S - pp.sc.gap_open;
         int W = slack >= pp.sc.gap_extend ? slack / pp.sc.gap_extend : 0;
         W = min(W, n + i_end);
+        if (W > 0 && i_end >= n) {
+            // Ungapped shortcut. If the gap-free alignment on the end cell's diagonal already scores S, it is the
+            // alignment the traceback reports: every prefix of an optimal path is optimal for its end cell, so
+            // the walk's first test (diagonal) succeeds at every step of it. Such a pair is gapless (W = 0):
+            // CIGAR nM, no band to recompute. Costs one XOR + popcount pass over ~n/16 words.
+            const sdp_batch& b = pp.b;
+            const uint32_t ri = b.pairs[2 * p], wi = b.pairs[2 * p + 1];
+            const long long rpos = (long long)b.read_off[ri], wpos = (long long)b.win_off[wi] + (i_end - n);
+            const int eq = count_equal_bases(b.reads_packed, b.read_nmask, rpos, (long long)((b.reads_bases + 15) / 16),
+                                             (long long)((b.reads_bases + 31) / 32), b.wins_packed, b.win_nmask, wpos,
+                                             (long long)((b.wins_bases + 15) / 16), (long long)((b.wins_bases + 31) / 32), n);
+            if (pp.sc.match * eq + pp.sc.mismatch * (n - eq) == S) W = 0;
+        }
         pp.tbW[p] = W;
         uint32_t words = 0;
         int bw = 1, rows = 0;
