@@ -87,8 +87,11 @@ __global__ void k_post_forward(const PostParams pp)
             ktb = (uint32_t)W * TB_KEY_STRIDE + (uint32_t)min((int)TB_KEY_STRIDE - 1, W ? rows : n);
             c_tb = (unsigned long long)bw * rows;
         } else if (wide) {
-            krev = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, rows >> 6);
-            kwide = (uint32_t)(n - 1) * 64u + (uint32_t)min(63, (rows + 7) >> 3);
+            // 64 row classes per read length, scaled to the rows a read of this length can need (rows <= 2.5 n),
+            // so that the pairs of one warp walk nearly the same number of rows
+            const uint32_t rbin = (uint32_t)min(63, (rows * 64) / (5 * n / 2 + 1));
+            krev = (uint32_t)(n - 1) * 64u + rbin;
+            kwide = (uint32_t)(n - 1) * 64u + rbin;
             c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
         } else {
             words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows;
