@@ -151,10 +151,14 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
         if (rc_ != SDP_OK) return rc_;                         \
     } while (0)
 
-// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. Cost model fitted to
-// measurements on B200: a warp runs 2*floor(32/G) pairs for (m + G - 1) steps;
-// a step costs 4 ALU slots per column plus ~17 of row bookkeeping, ~2.5 more when the read length is not
-// G*K (padded variant), and 12 % more beyond K = 25, where the register budget gets tight.
+// (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. A warp runs 2*floor(32/G) pairs
+// for (m + G - 1) steps, and a step costs what the (K, padded) kernel variant was MEASURED to cost on B200
+// (200,000 pairs, m = n + 300, G = 4; relative units; K = 1 extrapolated). A table, not a formula, because the
+// per-variant cost depends on how ptxas happened to allocate registers for that K (e.g. K = 21 exact is 6 %
+// slower than K = 21 padded), which no smooth model captures; DESIGN.md "Score kernel".
+static const double kStepCostExact[SDP_MAX_K] = {6.7, 8.4, 10.0, 12.1, 13.8, 15.7, 17.5, 19.5, 21.1, 23.4, 25.0, 27.0, 29.4, 31.3, 33.8, 34.5, 36.2, 40.1, 41.0, 44.0, 48.3, 45.9, 47.7, 49.1, 50.5, 56.6, 58.4, 60.4, 61.4, 65.5, 70.1, 67.6};
+static const double kStepCostPadded[SDP_MAX_K] = {7.5, 9.2, 11.0, 12.8, 14.7, 16.5, 18.4, 20.0, 22.1, 23.8, 26.4, 27.1, 30.3, 31.2, 33.8, 36.0, 39.4, 43.3, 41.6, 43.2, 45.4, 49.4, 49.2, 50.4, 53.4, 57.5, 60.4, 59.2, 65.3, 66.0, 64.7, 66.7};
+
 void choose_geometry(sdp_ctx* c) {
     struct Ent { uint16_t n, G, K, pad; };
     Ent ents[SDP_NSLOTS];
@@ -170,7 +174,7 @@ void choose_geometry(sdp_ctx* c) {
                 force_g * ((n + force_g - 1) / force_g) - n < force_g) continue;
             double ppw = 2.0 * (32 / G);
             double rows = (double)n + 300.0 + G - 1;
-            double thr = ppw / (rows * (4.0 * K + 17.0 + (G * K != n ? 2.5 : 0.0)) * (K > 25 ? 1.12 : 1.0));
+            double thr = ppw / (rows * (G * K != n ? kStepCostPadded[K - 1] : kStepCostExact[K - 1]));
             if (thr > best) { best = thr; bG = G; bK = K; }
         }
         ents[n - 1] = Ent{(uint16_t)n, (uint16_t)bG, (uint16_t)bK, (uint16_t)(bG * bK != n ? 1 : 0)};
