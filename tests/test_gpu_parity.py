@@ -154,6 +154,55 @@ def test_band_widths(ctx):
     parity.check_batch(ctx, b, DEFAULT, "band widths")
 
 
+def test_extreme_shapes(ctx):
+    # the longest windows the int16 range rule admits for n = 100, the longest reads, a single pair, 200,000 copies
+    # of one pair, one read against many overlapping windows of one reference, reads longer than tiny windows
+    rng = random.Random(99)
+
+    def rnd(k):
+        return "".join(rng.choice("ACGT") for _ in range(k))
+
+    def mutate(seq, subs, indel):
+        seq = list(seq)
+        for _ in range(subs):
+            seq[rng.randrange(len(seq))] = rng.choice("ACGT")
+        if indel:
+            k = rng.randrange(5, len(seq) - 5)
+            seq = seq[:k] + (list(rnd(indel)) if rng.random() < 0.5 else []) + seq[k + (0 if rng.random() < 0.5 else indel):]
+        return "".join(seq)
+
+    wins, reads = [], []
+    for m in (7000, 7500, 7800):
+        for _ in range(4):
+            T = rnd(m)
+            s = rng.randrange(0, m - 100)
+            reads.append(mutate(T[s:s + 100], rng.randint(0, 6), rng.choice([0, 0, 2, 7]))[:100].ljust(100, "A"))
+            wins.append(T)
+    parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "longest windows")
+    wins, reads = [], []
+    for n in (1000, 1024):
+        for _ in range(5):
+            m = n + rng.randint(0, 900)
+            T = rnd(m)
+            s = rng.randrange(0, m - n + 1)
+            reads.append((mutate(T[s:s + n], rng.randint(0, 40), rng.choice([0, 3, 15])) + rnd(n))[:n])
+            wins.append(T)
+    parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "longest reads")
+    T = rnd(400)
+    R = mutate(T[120:220], 3, 2)[:100].ljust(100, "C")
+    parity.check_batch(ctx, W.batch_from_strings([T], [R]), DEFAULT, "one pair")
+    b = W.batch_from_strings([T], [R], pairs=np.zeros((200000, 2), dtype=np.uint32))
+    parity.check_batch(ctx, b, DEFAULT, "200k identical pairs", host_path=False)
+    ref = rnd(2000)
+    R = mutate(ref[900:1050], 4, 3)[:150].ljust(150, "G")
+    wins = [ref[k:k + 600] for k in range(500, 1000, 7)]
+    b = W.batch_from_strings(wins, [R], pairs=np.array([[0, k] for k in range(len(wins))], dtype=np.uint32))
+    parity.check_batch(ctx, b, DEFAULT, "one read, many overlapping windows")
+    wins = [rnd(rng.randint(1, 20)) for _ in range(300)]
+    reads = [rnd(rng.randint(1, 60)) for _ in range(300)]
+    parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "reads longer than tiny windows")
+
+
 def test_n_bases_both_sides(ctx):
     rng = random.Random(13)
     reads, wins = [], []
