@@ -122,6 +122,11 @@ typedef struct sdp_stats {
  * SDP_ECUDA / SDP_ENOMEM otherwise; *out is written only on success. Not thread-safe: use one
  * ctx per thread; separate ctxs are independent. */
 int sdp_create(const sdp_scoring* scoring, int cuda_device, sdp_ctx** out);
+/* Environment variables read by sdp_create (tests and tuning only; results never depend on them):
+ *   SDP_NO_EXACT=1  use the general five-instruction score kernels even when 2*extend + mismatch >= 0
+ *   SDP_NO_THIN=1   send pairs with gap bound W >= 1 to the wide / generic traceback instead of the narrow-band kernels
+ *   SDP_NO_WIDE=1   send wide pairs to the generic scalar band kernel instead of the wavefront traceback kernel
+ *   SDP_FORCE_G=g   threads per pair group for every read length that admits it (geometry experiments) */
 
 /* Align every pair of `batch` (DEVICE pointers). Work is enqueued on `cuda_stream`
  * (a cudaStream_t; NULL = default stream) and the call returns after the stream has completed
