@@ -271,6 +271,21 @@ def test_general_score_kernel_with_default_scoring(monkeypatch):
         c.destroy()
 
 
+@pytest.mark.parametrize("env", [{"SDP_NO_THIN": "1"}, {"SDP_NO_WIDE": "1"}, {"SDP_NO_THIN": "1", "SDP_NO_WIDE": "1"}],
+                         ids=["no_thin", "no_wide", "generic_only"])
+def test_alternative_traceback_paths(monkeypatch, env):
+    # route the same pairs through the other traceback kernels (wide wavefront for every W >= 1; generic scalar band
+    # kernel instead of the wavefront; generic kernel for everything): all must agree with the oracle
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    c = make_ctx(DEFAULT)
+    try:
+        parity.check_batch(c, W.make_config(3, n_pairs=1200, ref_bases=500_000), DEFAULT, f"cfg3 {env}", host_path=False)
+        parity.check_batch(c, W.make_config(5, n_pairs=1500, ref_bases=500_000), DEFAULT, f"cfg5 {env}", host_path=False)
+    finally:
+        c.destroy()
+
+
 def test_mixed_window_lengths_in_one_warp(ctx):
     # same read length, window lengths from 1 to 900 in one batch: lanes of a warp finish at
     # different rows (the masked tail loop of the score kernel)
