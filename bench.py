@@ -234,6 +234,21 @@ def main():
     barrier()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1)
+    # ---- the same steps with the optional ungapped pre-pass on (sdp_set_prefilter; NOT the headline: pairs it
+    # settles skip the DP, so "GCUPS" here counts cells that were never updated)
+    ctx.set_prefilter(True)
+    pf_ms = []
+    for it in range(2 + args.steps):
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.align_batch(dbatch, stream)
+        e1.record(stream)
+        e1.synchronize()
+        if it >= 2:
+            pf_ms.append(e0.elapsed_time(e1))
+    pf_stats = ctx.stats()
+    ctx.set_prefilter(False)
     ctx.set_timing(False)
     total_ms = sum(step_ms)
     if world > 1:
@@ -362,6 +377,12 @@ def main():
         "stages_ms": {k: stats.get(k) for k in ("ms_total", "ms_bucket", "ms_forward", "ms_reverse", "ms_traceback",
                                                 "ms_compact")},
         "roofline": roofline, "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
+        "with_ungapped_prepass": {
+            "ms_per_step": statistics.mean(pf_ms) if pf_ms else None,
+            "effective_gcups": (cells / (statistics.mean(pf_ms) * 1e-3) / 1e9) if pf_ms else None,
+            "cells_settled_without_dp_frac": pf_stats.get("cells_prefiltered", 0) / max(1, cells),
+            "note": "optional sdp_set_prefilter(1), off in every other number of this line: near-exact pairs get score and "
+                    "ref_end from a Hamming scan and skip the forward DP; outputs are bit-identical; rank 0 only"},
     }
     if not args.no_cpu_baseline and world == 1:
         import oracle

@@ -116,6 +116,8 @@ typedef struct sdp_stats {
     float ms_reverse;             /* a4                                                          */
     float ms_traceback;           /* a5 + a6                                                     */
     float ms_compact;             /* a7 + a8                                                     */
+    uint64_t cells_prefiltered;   /* sum n*m of the pairs the ungapped pre-pass settled (sdp_set_prefilter);
+                                     cells_forward counts only the pairs that went through the DP   */
 } sdp_stats;
 
 /* Create a context on CUDA device `cuda_device`. SDP_EINVAL for bad scoring or null arguments,
@@ -167,6 +169,13 @@ int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* re
  * `read_start`, `n_match`, `n_cols`, `pass`, `cigar_len`, `cigar_off` are 0 and n_cigar_ops is 0. A caller scores every
  * candidate this way, picks winners with sdp_best_per_read and aligns only those with score-only off (0, default). */
 int sdp_set_score_only(sdp_ctx* ctx, int enabled);
+
+/* Optional ungapped pre-pass (off by default; the analogue of the paper's step 1, inside one window).
+ * A gapped alignment scores at most n*match - (gap_open + gap_extend). With the pre-pass on (1), a pair whose best
+ * gap-free placement in the window has x mismatches with x*(match - mismatch) < gap_open + gap_extend gets its score and
+ * lowest ref_end from a word-parallel Hamming scan and skips the forward DP; every other pair, and every later stage,
+ * is unchanged, and so is every output (tests/test_gpu_parity.py::test_prefilter_changes_nothing). */
+int sdp_set_prefilter(sdp_ctx* ctx, int enabled);
 
 /* Counters of the last align call on this ctx. */
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);

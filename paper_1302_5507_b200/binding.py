@@ -22,7 +22,7 @@ SDP_MAX_CELL_VALUE = 16000
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only"]
+           "sdp_set_score_only", "sdp_set_prefilter"]
 
 
 class SdpError(RuntimeError):
@@ -65,7 +65,8 @@ class sdp_stats(ctypes.Structure):
                 ("cells_traceback", ctypes.c_uint64), ("n_reverse_pairs", ctypes.c_uint64),
                 ("kernel_launches", ctypes.c_uint32), ("forward_launches", ctypes.c_uint32),
                 ("ms_total", ctypes.c_float), ("ms_bucket", ctypes.c_float), ("ms_forward", ctypes.c_float),
-                ("ms_reverse", ctypes.c_float), ("ms_traceback", ctypes.c_float), ("ms_compact", ctypes.c_float)]
+                ("ms_reverse", ctypes.c_float), ("ms_traceback", ctypes.c_float), ("ms_compact", ctypes.c_float),
+                ("cells_prefiltered", ctypes.c_uint64)]
 
     def as_dict(self) -> dict:
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -94,6 +95,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_best_per_read.restype = ctypes.c_int
     lib.sdp_best_per_read.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result),
                                       ctypes.c_void_p, ctypes.POINTER(sdp_read_best)]
+    lib.sdp_set_prefilter.restype = ctypes.c_int
+    lib.sdp_set_prefilter.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_score_only.restype = ctypes.c_int
     lib.sdp_set_score_only.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_get_stats.restype = ctypes.c_int
@@ -223,6 +226,9 @@ class Context:
 
     def set_timing(self, enabled: bool):
         self._lib.sdp_set_timing(self._h, int(bool(enabled)))
+
+    def set_prefilter(self, enabled: bool):
+        self._lib.sdp_set_prefilter(self._h, int(bool(enabled)))
 
     def set_score_only(self, enabled: bool):
         self._lib.sdp_set_score_only(self._h, int(bool(enabled)))

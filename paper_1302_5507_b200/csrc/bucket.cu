@@ -6,15 +6,70 @@
 // work of different complexity classes separately; here pairs are binned by
 // (read length, rows >> 6) so that the lanes of one warp walk the same number of DP rows.
 #include "sdp_host.cuh"
+#include "seq_bits.cuh"
 
 namespace sdp {
+
+// ---------------------------------------------------------------------------------------------
+// Optional ungapped pre-pass (sdp_set_prefilter; the analogue of the paper's step 1, for one window).
+// A gapped alignment scores at most n*match - (o + e). If the best gap-free placement of the read in the window
+// has x mismatches with x*(match - mismatch) < o + e, its score n*match - x*(match - mismatch) beats every gapped
+// alignment, so it is the optimum, and the lowest offset reaching x is the lowest maximising end row: score and
+// ref_end without any DP. Word-parallel Hamming scan over all m - n + 1 offsets with early exit. Returns false
+// when no placement has few enough mismatches (the pair then takes the DP).
+__device__ bool ungapped_optimum(const sdp_batch& b, const Scoring& sc, uint64_t ro, uint64_t wo, int n, int m,
+                                 int32_t* score, int32_t* ref_end)
+{
+    const int delta = sc.match - sc.mismatch;
+    const int xmax = (sc.gap_open + sc.gap_extend + delta - 1) / delta - 1;     // largest x with x*delta < o + e
+    if (xmax < 0 || n > m) return false;
+    const long long rwords = (long long)((b.reads_bases + 15) / 16), wwords = (long long)((b.wins_bases + 15) / 16);
+    const long long rnwords = (long long)((b.reads_bases + 31) / 32), wnwords = (long long)((b.wins_bases + 31) / 32);
+    int best_x = xmax + 1, best_s = -1;
+    // first 16 read bases in a register, the window as a sliding 32-base buffer: one shift, XOR and popcount per
+    // offset reject almost every placement; only the survivors look at the rest of the read
+    const int cnt0 = min(16, n);
+    const uint32_t mask0 = cnt0 < 16 ? (1u << (2 * cnt0)) - 1u : 0xFFFFFFFFu;
+    const uint32_t r0 = bases16(b.reads_packed, (long long)ro, rwords);
+    const uint32_t rn0 = nbits16_spread(b.read_nmask, (long long)ro, rnwords);
+    uint64_t wb = 0, wnb = 0;
+    for (int s = 0; s + n <= m; ++s) {
+        const int k = s & 15;
+        if (k == 0) {
+            wb = (uint64_t)bases16(b.wins_packed, (long long)wo + s, wwords) |
+                 ((uint64_t)bases16(b.wins_packed, (long long)wo + s + 16, wwords) << 32);
+            if (b.win_nmask != nullptr)
+                wnb = (uint64_t)nbits16_spread(b.win_nmask, (long long)wo + s, wnwords) |
+                      ((uint64_t)nbits16_spread(b.win_nmask, (long long)wo + s + 16, wnwords) << 32);
+        }
+        const int limit = best_x - 1;                     // only a strictly better placement replaces an earlier one
+        int x = cnt0 - __popc(eq16(r0, (uint32_t)(wb >> (2 * k)), rn0 | (uint32_t)(wnb >> (2 * k))) & mask0);
+        for (int j0 = 16; j0 < n && x <= limit; j0 += 16) {
+            const uint32_t r = bases16(b.reads_packed, (long long)ro + j0, rwords);
+            const uint32_t t = bases16(b.wins_packed, (long long)wo + s + j0, wwords);
+            const uint32_t nm = nbits16_spread(b.read_nmask, (long long)ro + j0, rnwords) |
+                                nbits16_spread(b.win_nmask, (long long)wo + s + j0, wnwords);
+            uint32_t eq = eq16(r, t, nm);
+            const int cnt = min(16, n - j0);
+            if (cnt < 16) eq &= (1u << (2 * cnt)) - 1u;
+            x += cnt - __popc(eq);
+        }
+        if (x <= limit) { best_x = x; best_s = s; if (x == 0) break; }
+    }
+    if (best_s < 0) return false;
+    *score = sc.match * n - best_x * delta;
+    *ref_end = best_s + n - 1;
+    return true;
+}
 
 // ---------------------------------------------------------------------------------------------
 // a1: validate every pair and emit its bucket key. One thread per pair.
 __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __restrict__ keys,
                                uint32_t* __restrict__ pn, uint32_t* __restrict__ pm,
                                uint32_t* __restrict__ hist, uint32_t* __restrict__ err_flag,
-                               unsigned long long* __restrict__ cells)
+                               unsigned long long* __restrict__ cells, int prefilter,
+                               int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
+                               unsigned long long* __restrict__ cells_skipped)
 {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t key = SDP_KEY_SKIP, err = 0;
@@ -35,6 +90,13 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
                 key = (n - 1) * 64u + min(63u, m >> 6);
                 pn[p] = n; pm[p] = m;
                 my_cells = (unsigned long long)n * m;
+                int32_t s_u, e_u;
+                if (prefilter && ungapped_optimum(b, sc, ro, wo, (int)n, (int)m, &s_u, &e_u)) {
+                    score[p] = s_u; ref_end[p] = e_u;     // no DP for this pair: it never enters the forward buckets
+                    key = SDP_KEY_SKIP;
+                    atomicAdd(cells_skipped, my_cells);
+                    my_cells = 0;
+                }
             }
         }
         keys[p] = key;
@@ -252,7 +314,8 @@ __global__ void k_mailbox(const uint32_t* __restrict__ tb_bin_start, uint32_t st
 {
     const uint32_t t = threadIdx.x;
     if (t < nbounds) host_bounds[t] = tb_bin_start[(size_t)t * stride];
-    if (t < 4) { host_totals[t] = totals[t]; host_counters[t] = counters[t]; }
+    if (t < 4) host_totals[t] = totals[t];
+    if (t < 8) host_counters[t] = counters[t];
 }
 
 void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbounds, const uint64_t* totals,
@@ -265,10 +328,11 @@ void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbou
 // ---------------------------------------------------------------------------------------------
 // host wrappers
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
-                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st)
+                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
+                         int32_t* ref_end, unsigned long long* cells_skipped, cudaStream_t st)
 {
     const uint32_t grid = (uint32_t)((b.n_pairs + 255) / 256);
-    k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells);
+    k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells, prefilter, score, ref_end, cells_skipped);
 }
 
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,

@@ -50,7 +50,8 @@ struct Mailbox {                    // pinned host memory the device results lan
     uint32_t tb_bounds[THIN_NW + TB_NCLASS + 1];   // narrow-band launches (one per W), then the generic band classes
     uint32_t err_flag;
     uint64_t totals[4];             // [0] thin direction-bit words, [1] run capacity, [2] CIGAR runs, [3] wide nibble words
-    unsigned long long counters[4]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
+    unsigned long long counters[8]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
+                                    // [4] cells of pairs the ungapped pre-pass settled
 };
 
 constexpr int SDP_FAN_STREAMS = 4;
@@ -69,6 +70,7 @@ struct sdp_ctx {
     int no_thin = 0;                 // SDP_NO_THIN=1: keep W >= 1 pairs off the narrow-band kernel (debugging)
     char err[512] = {0};
     bool timing = false;
+    bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
     bool score_only = false;         // sdp_set_score_only: stop after the forward pass
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
@@ -283,7 +285,7 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
             CU(cudaMalloc(&ctx->task_prefix[i], (SDP_NSLOTS + 1) * 4));
         }
         CU(cudaMalloc(&ctx->err_flag, 4));
-        CU(cudaMalloc(&ctx->counters, 4 * 8));
+        CU(cudaMalloc(&ctx->counters, 8 * 8));
         CU(cudaMalloc(&ctx->totals, 4 * 8));
         return SDP_OK;
     };
@@ -333,6 +335,13 @@ int sdp_set_timing(sdp_ctx* ctx, int enabled)
 {
     if (!ctx) return SDP_EINVAL;
     ctx->timing = enabled != 0;
+    return SDP_OK;
+}
+
+int sdp_set_prefilter(sdp_ctx* ctx, int enabled)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->prefilter = enabled != 0;
     return SDP_OK;
 }
 
@@ -457,9 +466,10 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     // ---- a1 + a2
     for (int i = 0; i < 4; ++i) CU(cudaMemsetAsync(ctx->hist[i], 0, (SDP_NBINS + 1) * 4, st));
     CU(cudaMemsetAsync(ctx->err_flag, 0, 4, st));
-    CU(cudaMemsetAsync(ctx->counters, 0, 4 * 8, st));
+    CU(cudaMemsetAsync(ctx->counters, 0, 8 * 8, st));
     launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
-                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, st);
+                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, ctx->prefilter ? 1 : 0, ctx->score.as<int32_t>(),
+                        ctx->ref_end.as<int32_t>(), ctx->counters + 4, st);
     launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0],
                      ctx->mb->task_prefix[0], &ctx->mb->bin_total[0], st);
@@ -470,7 +480,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         return fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)");
     if (ctx->mb->err_flag & SDP_ERRF_RANGE)
         return fail(ctx, SDP_ERANGE, "a pair breaks the int16 range rule or SDP_MAX_READ_LEN (see sdp.h)");
-    launch_fill_desc_fwd(b, ctx->order.as<uint32_t>(), (uint32_t)P, ctx->desc.as<PairDesc>(), st);
+    // (with the ungapped pre-pass on, fewer than P pairs are in the forward buckets)
+    launch_fill_desc_fwd(b, ctx->order.as<uint32_t>(), ctx->mb->bin_total[0], ctx->desc.as<PairDesc>(), st);
     ++nl;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_BUCKET], st));
 
@@ -495,10 +506,11 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         CU(cudaMemsetAsync(ctx->n_cols.p, 0, P * 4, st));
         CU(cudaMemsetAsync(ctx->cigar_off.p, 0, P * 8, st));
         CU(cudaMemsetAsync(ctx->cigar_len.p, 0, P * 4, st));
-        CU(cudaMemcpyAsync(ctx->mb->counters + 3, ctx->counters + 3, 8, cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(ctx->mb->counters + 3, ctx->counters + 3, 16, cudaMemcpyDeviceToHost, st));
         if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
         CU(cudaStreamSynchronize(st));
         stats.cells_forward = ctx->mb->counters[3];
+        stats.cells_prefiltered = ctx->mb->counters[4];
         stats.kernel_launches = nl;
         if (ctx->timing) {
             cudaEventElapsedTime(&stats.ms_total, ctx->ev[EV_START], ctx->ev[EV_END]);
@@ -644,6 +656,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
                     "disagrees with the forward score", ctx->mb->err_flag);
 
     stats.cells_forward = ctx->mb->counters[3];
+    stats.cells_prefiltered = ctx->mb->counters[4];
     stats.cells_reverse = ctx->mb->counters[0];
     stats.cells_traceback = ctx->mb->counters[1];
     stats.n_reverse_pairs = ctx->mb->counters[2];

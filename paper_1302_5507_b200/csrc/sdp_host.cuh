@@ -12,7 +12,8 @@ struct Scoring {
 
 // ---- bucket.cu
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
-                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, cudaStream_t st);
+                         uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
+                         int32_t* ref_end, unsigned long long* cells_skipped, cudaStream_t st);
 // scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,

@@ -286,6 +286,29 @@ def test_alternative_traceback_paths(monkeypatch, env):
         c.destroy()
 
 
+@pytest.mark.parametrize("sc", [DEFAULT, OracleScoring(2, -1, 1, 1, 0.5), OracleScoring(1, -4, 6, 1, 0.9), OracleScoring(1, -1, 9, 3, 0.6)],
+                         ids=lambda s: f"{s.match}_{s.mismatch}_{s.gap_open}_{s.gap_extend}")
+def test_prefilter_changes_nothing(sc):
+    # the ungapped pre-pass (sdp_set_prefilter) settles near-exact pairs without DP; every output must stay bit-exact.
+    # Scorings: at most 1 / 0 / 1 / 5 mismatches allowed by x*(match-mismatch) < open+extend
+    c = make_ctx(sc)
+    try:
+        c.set_prefilter(True)
+        for cfg, P in ((2, 3000), (5, 4000), (3, 1500)):
+            parity.check_batch(c, W.make_config(cfg, n_pairs=P, ref_bases=500_000), sc, f"prefilter cfg{cfg}")
+            st = c.stats()
+            assert st["cells_prefiltered"] > 0 or sc.mismatch == -1 and sc.match == 2
+        rng = random.Random(31)
+        wins = ["".join(rng.choice("AC") for _ in range(rng.randint(1, 80))) for _ in range(500)]     # ties everywhere
+        reads = ["".join(rng.choice("AC") for _ in range(rng.randint(1, 30))) for _ in range(500)]
+        parity.check_batch(c, W.batch_from_strings(wins, reads), sc, "prefilter low complexity", host_path=False)
+        wins = ["ACGTNNACGTACGTNACGTACGTAAC" * 3 for _ in range(40)]
+        reads = [w[k:k + 20] for k, w in enumerate(wins)]
+        parity.check_batch(c, W.batch_from_strings(wins, reads), sc, "prefilter with N", host_path=False)
+    finally:
+        c.destroy()
+
+
 def test_mixed_window_lengths_in_one_warp(ctx):
     # same read length, window lengths from 1 to 900 in one batch: lanes of a warp finish at
     # different rows (the masked tail loop of the score kernel)
