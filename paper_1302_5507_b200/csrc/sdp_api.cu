@@ -609,7 +609,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         launch_walk(wp, st);
         ++nl;
     }
-    // ---- a5 + a6, narrow bands (W <= 7: one thread per pair, band in registers) and the generic band kernel.
+    // ---- a5 + a6, narrow bands (W < THIN_NW: one thread per pair, band in registers) and the generic band kernel.
     // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on a
     // side stream beside it (the stream synchronisation above has completed everything they read).
     cudaStream_t ss = ctx->side_stream;

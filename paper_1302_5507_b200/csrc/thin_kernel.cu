@@ -3,8 +3,8 @@
 // The forward score S bounds the gap content of every co-optimal alignment,
 // W = floor((n*match - S - o) / e), so every co-optimal path lies in the
 // band |i - j - (i_end - n)| <= W of rows (i_end - n - W, i_end]. For W = 0 the alignment is
-// gapless: CIGAR nM, n_match from the score alone. For 1 <= W <= 7 the band
-// (2W+1 <= 15 columns) is recomputed with the paper's recurrences in the same
+// gapless: CIGAR nM, n_match from the score alone. For 1 <= W < THIN_NW (24) the band
+// (2W+1 <= 47 columns) is recomputed with the paper's recurrences in the same
 // x8 tagged integer domain as trace_kernel.cuh -- scalar int32 here, band cells in registers, the
 // row loop fully unrolled over the band -- and leaves four direction bits per cell in a per-thread
 // (hardware-interleaved, hence coalesced) local-memory array; the walk of PAPER.md:353 /

@@ -75,7 +75,7 @@ __global__ void k_post_forward(const PostParams pp)
             bw = min(2 * W + 1, n + 1);
         }
         pp.tb_rows[p] = rows;
-        // Three paths. Narrow: W <= 7 and a real band -> one thread per pair,
+        // Three paths. Narrow: W < THIN_NW and a real band -> one thread per pair,
         // band in registers (thin_kernel.cu). Wide: the register-resident wavefront recomputes the
         // whole rectangle rows x n (trace_kernel.cuh) when its x8 scaled values fit 16 bits; the
         // reverse pass first trims the rectangle's rows. Anything else: the generic band kernel.
