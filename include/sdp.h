@@ -177,6 +177,34 @@ int sdp_set_score_only(sdp_ctx* ctx, int enabled);
  * is unchanged, and so is every output (tests/test_gpu_parity.py::test_prefilter_changes_nothing). */
 int sdp_set_prefilter(sdp_ctx* ctx, int enabled);
 
+/*
+ * Mate-rescue wrapper (step 2: "a candidate region flanking the mapped end is aligned to the unmapped
+ * end"; expected minimum and maximum fragment lengths -v / -u and the orientation of the ends).
+ * The paper does not say how the region follows from the bounds; reading taken (R17), forward-reverse
+ * orientation: a fragment is the reference interval [f, f + ins) with min_insert <= ins <= max_insert, its forward-strand
+ * end starts at f and its reverse-strand end stops at f + ins.
+ *   mate on the forward strand at [p, p + L):  the other end lies in  [p + min_insert - n, p + max_insert)
+ *   mate on the reverse strand at [p, p + L):  the other end lies in  [p + L - max_insert, p + L - min_insert + n)
+ * clipped to [0, ref_bases); n = length of the unmapped read. win_len is 0 when nothing is left (the caller drops the
+ * pair: sdp_align_batch rejects empty windows). All pointers are DEVICE pointers; outputs are caller-owned.
+ */
+typedef struct sdp_mates {
+    const uint64_t* mate_pos;      /* leftmost reference base of the mapped end                 */
+    const uint32_t* mate_len;      /* reference bases the mapped end covers                      */
+    const uint8_t*  mate_reverse;  /* 0 = mapped end on the forward strand, 1 = reverse          */
+    const uint32_t* read_len;      /* length n of the unmapped end                               */
+    uint64_t        n;             /* number of rescues                                          */
+} sdp_mates;
+int sdp_mate_windows(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, uint64_t ref_bases,
+                     void* cuda_stream, uint64_t* win_off, uint32_t* win_len);
+/* After aligning rescue k against window k (pair k of the batch = (read k, window k)): proper[k] = 1 iff the alignment
+ * exists (win_len > 0), passed the similarity filter, and the implied fragment length is within the bounds:
+ * mate forward: (win_off + ref_end + 1) - p;  mate reverse: (p + L) - (win_off + ref_start). `ref_start`, `ref_end`,
+ * `pass` are the arrays of the sdp_result of that alignment (device pointers). */
+int sdp_proper_pairs(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, const uint64_t* win_off,
+                     const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
+                     void* cuda_stream, uint8_t* proper);
+
 /* Counters of the last align call on this ctx. */
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);
 

@@ -12,4 +12,6 @@ from .oracle import (  # noqa: F401
     best_per_read,
     build,
     decode_cigar,
+    mate_windows,
+    proper_pairs,
 )

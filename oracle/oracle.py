@@ -222,3 +222,36 @@ def best_per_read(pairs: np.ndarray, score: np.ndarray, n_reads: int) -> dict:
         else:
             second[r] = max(int(second[r]), s)
     return dict(best_pair=best_pair, best_score=best_score, second_score=second, n_candidates=ncand)
+
+
+def mate_windows(mate_pos, mate_len, mate_reverse, read_len, min_insert: int, max_insert: int, ref_bases: int):
+    """Candidate region of a mate rescue (TEST INFRASTRUCTURE; R17).
+
+    Forward-reverse orientation: a fragment is [f, f + ins) with min_insert <= ins <= max_insert; its forward end starts
+    at f, its reverse end stops at f + ins. Mapped end forward at [p, p+L): the other end stops at p + ins, so it lies in
+    [p + min - n, p + max). Mapped end reverse at [p, p+L): the fragment stops at p + L, the other end starts at
+    p + L - ins, so it lies in [p + L - max, p + L - min + n). Clipped to the reference; length 0 when nothing is left.
+    Plain Python loop on purpose."""
+    off, ln = [], []
+    for p, L, rev, n in zip(mate_pos, mate_len, mate_reverse, read_len):
+        p, L, n = int(p), int(L), int(n)
+        lo, hi = (p + min_insert - n, p + max_insert) if not rev else (p + L - max_insert, p + L - min_insert + n)
+        lo, hi = max(lo, 0), min(hi, int(ref_bases))
+        ok = hi > lo
+        off.append(lo if ok else 0)
+        ln.append(hi - lo if ok else 0)
+    return np.array(off, dtype=np.uint64), np.array(ln, dtype=np.uint32)
+
+
+def proper_pairs(mate_pos, mate_len, mate_reverse, min_insert: int, max_insert: int, win_off, win_len, ref_start, ref_end,
+                 passed):
+    """Properly paired = aligned, passed the similarity filter, implied fragment length within the bounds (same reading)."""
+    out = []
+    for k in range(len(mate_pos)):
+        ok = 0
+        if int(win_len[k]) > 0 and int(passed[k]):
+            p, L, w = int(mate_pos[k]), int(mate_len[k]), int(win_off[k])
+            ins = (w + int(ref_end[k]) + 1) - p if not mate_reverse[k] else (p + L) - (w + int(ref_start[k]))
+            ok = 1 if min_insert <= ins <= max_insert else 0
+        out.append(ok)
+    return np.array(out, dtype=np.uint8)

@@ -22,7 +22,8 @@ SDP_MAX_CELL_VALUE = 16000
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only", "sdp_set_prefilter"]
+           "sdp_set_score_only", "sdp_set_prefilter", "sdp_mate_windows",
+           "sdp_proper_pairs"]
 
 
 class SdpError(RuntimeError):
@@ -55,6 +56,11 @@ class sdp_result(ctypes.Structure):
 class sdp_read_best(ctypes.Structure):
     _fields_ = [("best_pair", ctypes.c_void_p), ("best_score", ctypes.c_void_p), ("second_score", ctypes.c_void_p),
                 ("n_candidates", ctypes.c_void_p), ("n_reads", ctypes.c_uint32)]
+
+
+class sdp_mates(ctypes.Structure):
+    _fields_ = [("mate_pos", ctypes.c_void_p), ("mate_len", ctypes.c_void_p), ("mate_reverse", ctypes.c_void_p),
+                ("read_len", ctypes.c_void_p), ("n", ctypes.c_uint64)]
 
 
 SDP_NO_PAIR = 0xFFFFFFFF
@@ -95,6 +101,13 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_best_per_read.restype = ctypes.c_int
     lib.sdp_best_per_read.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result),
                                       ctypes.c_void_p, ctypes.POINTER(sdp_read_best)]
+    lib.sdp_mate_windows.restype = ctypes.c_int
+    lib.sdp_mate_windows.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_mates), ctypes.c_uint32, ctypes.c_uint32,
+                                     ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    lib.sdp_proper_pairs.restype = ctypes.c_int
+    lib.sdp_proper_pairs.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_mates), ctypes.c_uint32, ctypes.c_uint32,
+                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                     ctypes.c_void_p, ctypes.c_void_p]
     lib.sdp_set_prefilter.restype = ctypes.c_int
     lib.sdp_set_prefilter.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_score_only.restype = ctypes.c_int
@@ -320,6 +333,40 @@ class Context:
 
         return dict(best_pair=down(rb.best_pair, np.uint32), best_score=down(rb.best_score, np.int32),
                     second_score=down(rb.second_score, np.int32), n_candidates=down(rb.n_candidates, np.uint32))
+
+    # -- mate rescue (device tensors in, device tensors out; argument marshalling only)
+    @staticmethod
+    def _mates(mate_pos, mate_len, mate_reverse, read_len) -> sdp_mates:
+        return sdp_mates(mate_pos.data_ptr(), mate_len.data_ptr(), mate_reverse.data_ptr(), read_len.data_ptr(),
+                         int(mate_pos.numel()))
+
+    def mate_windows(self, mate_pos, mate_len, mate_reverse, read_len, min_insert: int, max_insert: int, ref_bases: int):
+        """sdp_mate_windows: torch CUDA tensors (int64 / int32 / uint8 / int32) -> (win_off int64, win_len int32) tensors."""
+        import torch
+        n = int(mate_pos.numel())
+        win_off = torch.empty(n, dtype=torch.int64, device=mate_pos.device)
+        win_len = torch.empty(n, dtype=torch.int32, device=mate_pos.device)
+        m = self._mates(mate_pos, mate_len, mate_reverse, read_len)
+        st = torch.cuda.current_stream(self.device)
+        self._check(self._lib.sdp_mate_windows(self._h, ctypes.byref(m), int(min_insert), int(max_insert), int(ref_bases),
+                                               ctypes.c_void_p(st.cuda_stream), ctypes.c_void_p(win_off.data_ptr()),
+                                               ctypes.c_void_p(win_len.data_ptr())))
+        return win_off, win_len
+
+    def proper_pairs(self, mate_pos, mate_len, mate_reverse, read_len, min_insert: int, max_insert: int, win_off, win_len,
+                     res: sdp_result):
+        """sdp_proper_pairs on the sdp_result of aligning rescue k against window k; returns a uint8 CUDA tensor."""
+        import torch
+        n = int(mate_pos.numel())
+        proper = torch.empty(n, dtype=torch.uint8, device=mate_pos.device)
+        m = self._mates(mate_pos, mate_len, mate_reverse, read_len)
+        st = torch.cuda.current_stream(self.device)
+        self._check(self._lib.sdp_proper_pairs(self._h, ctypes.byref(m), int(min_insert), int(max_insert),
+                                               ctypes.c_void_p(win_off.data_ptr()), ctypes.c_void_p(win_len.data_ptr()),
+                                               ctypes.c_void_p(res.ref_start), ctypes.c_void_p(res.ref_end),
+                                               ctypes.c_void_p(res.pass_), ctypes.c_void_p(st.cuda_stream),
+                                               ctypes.c_void_p(proper.data_ptr())))
+        return proper
 
     # -- host path
     def align_batch_host(self, batch) -> HostResult:

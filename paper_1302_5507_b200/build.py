@@ -43,7 +43,7 @@ def _deps_hash(extra: str) -> str:
 
 def _units():
     units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []), ("thin_kernel", "thin_kernel.cu", []),
-             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", [])]
+             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("mate", "mate.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"score_r{r}", "score_inst.cu",
                       [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_K_FN=launch_score_r{r}",

@@ -699,6 +699,38 @@ int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* re
     return SDP_OK;
 }
 
+int sdp_mate_windows(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, uint64_t ref_bases,
+                     void* cuda_stream, uint64_t* win_off, uint32_t* win_len)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!mates || !win_off || !win_len || min_insert > max_insert) return fail(ctx, SDP_EINVAL, "null argument or min_insert > max_insert");
+    if (mates->n && (!mates->mate_pos || !mates->mate_len || !mates->mate_reverse || !mates->read_len))
+        return fail(ctx, SDP_EINVAL, "null input array");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->device));
+    launch_mate_windows(*mates, min_insert, max_insert, ref_bases, win_off, win_len, st);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    return SDP_OK;
+}
+
+int sdp_proper_pairs(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, const uint64_t* win_off,
+                     const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
+                     void* cuda_stream, uint8_t* proper)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!mates || !win_off || !win_len || !ref_start || !ref_end || !pass || !proper || min_insert > max_insert)
+        return fail(ctx, SDP_EINVAL, "null argument or min_insert > max_insert");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->device));
+    launch_proper_pairs(*mates, min_insert, max_insert, win_off, win_len, ref_start, ref_end, pass, proper, st);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    return SDP_OK;
+}
+
 int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
 {
     if (!ctx) return SDP_EINVAL;
