@@ -185,8 +185,9 @@ int sdp_set_prefilter(sdp_ctx* ctx, int enabled);
  * end starts at f and its reverse-strand end stops at f + ins.
  *   mate on the forward strand at [p, p + L):  the other end lies in  [p + min_insert - n, p + max_insert)
  *   mate on the reverse strand at [p, p + L):  the other end lies in  [p + L - max_insert, p + L - min_insert + n)
- * clipped to [0, ref_bases); n = length of the unmapped read. win_len is 0 when nothing is left (the caller drops the
- * pair: sdp_align_batch rejects empty windows). All pointers are DEVICE pointers; outputs are caller-owned.
+ * clipped to [0, ref_bases); n = length of the unmapped read. win_len is 0 when nothing is left; sdp_align_batch rejects
+ * empty windows, so such a rescue must stay out of the pair list: sdp_mate_pairs builds that list. All pointers are DEVICE
+ * pointers; outputs are caller-owned.
  */
 typedef struct sdp_mates {
     const uint64_t* mate_pos;      /* leftmost reference base of the mapped end                 */
@@ -197,13 +198,19 @@ typedef struct sdp_mates {
 } sdp_mates;
 int sdp_mate_windows(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, uint64_t ref_bases,
                      void* cuda_stream, uint64_t* win_off, uint32_t* win_len);
-/* After aligning rescue k against window k (pair k of the batch = (read k, window k)): proper[k] = 1 iff the alignment
- * exists (win_len > 0), passed the similarity filter, and the implied fragment length is within the bounds:
+/* Pair list of a rescue batch in which read k and window k belong to rescue k: the rescues with win_len[k] > 0, in rescue
+ * order, as pairs (k, k). pairs receives 2 * (*n_pairs) entries (capacity 2 * n), pair_of_rescue[k] the index of rescue k
+ * in that list or SDP_NO_PAIR when its window is empty; *n_pairs is a HOST pointer. The other pointers are DEVICE memory. */
+int sdp_mate_pairs(sdp_ctx* ctx, const uint32_t* win_len, uint64_t n, void* cuda_stream, uint32_t* pairs,
+                   uint32_t* pair_of_rescue, uint64_t* n_pairs);
+/* After aligning the rescue batch: proper[k] = 1 iff rescue k was aligned (win_len[k] > 0 and, when pair_of_rescue is given,
+ * pair_of_rescue[k] != SDP_NO_PAIR), passed the similarity filter, and the implied fragment length is within the bounds:
  * mate forward: (win_off + ref_end + 1) - p;  mate reverse: (p + L) - (win_off + ref_start). `ref_start`, `ref_end`,
- * `pass` are the arrays of the sdp_result of that alignment (device pointers). */
+ * `pass` are the arrays of the sdp_result of that alignment (device pointers), read at index pair_of_rescue[k]; a NULL
+ * pair_of_rescue means pair k = rescue k (only valid when no window is empty). */
 int sdp_proper_pairs(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, const uint64_t* win_off,
-                     const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
-                     void* cuda_stream, uint8_t* proper);
+                     const uint32_t* win_len, const uint32_t* pair_of_rescue, const int32_t* ref_start, const int32_t* ref_end,
+                     const uint8_t* pass, void* cuda_stream, uint8_t* proper);
 
 /* Counters of the last align call on this ctx. */
 int sdp_get_stats(const sdp_ctx* ctx, sdp_stats* out);

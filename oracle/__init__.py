@@ -12,6 +12,7 @@ from .oracle import (  # noqa: F401
     best_per_read,
     build,
     decode_cigar,
+    mate_pairs,
     mate_windows,
     proper_pairs,
 )

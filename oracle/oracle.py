@@ -243,15 +243,30 @@ def mate_windows(mate_pos, mate_len, mate_reverse, read_len, min_insert: int, ma
     return np.array(off, dtype=np.uint64), np.array(ln, dtype=np.uint32)
 
 
+def mate_pairs(win_len):
+    """Pair list of a rescue batch (same reading): rescues whose window is not empty, in rescue order, as (k, k);
+    pair_of_rescue[k] = index of rescue k in that list, 0xFFFFFFFF when its window is empty."""
+    pairs, por = [], []
+    for k, ln in enumerate(win_len):
+        if int(ln) > 0:
+            por.append(len(pairs))
+            pairs.append((k, k))
+        else:
+            por.append(0xFFFFFFFF)
+    return np.array(pairs, dtype=np.uint32).reshape(-1, 2), np.array(por, dtype=np.uint32)
+
+
 def proper_pairs(mate_pos, mate_len, mate_reverse, min_insert: int, max_insert: int, win_off, win_len, ref_start, ref_end,
-                 passed):
-    """Properly paired = aligned, passed the similarity filter, implied fragment length within the bounds (same reading)."""
+                 passed, pair_of_rescue=None):
+    """Properly paired = aligned, passed the similarity filter, implied fragment length within the bounds (same reading).
+    ref_start / ref_end / passed are indexed by pair_of_rescue[k] (rescue k itself when pair_of_rescue is None)."""
     out = []
     for k in range(len(mate_pos)):
         ok = 0
-        if int(win_len[k]) > 0 and int(passed[k]):
+        q = k if pair_of_rescue is None else int(pair_of_rescue[k])
+        if int(win_len[k]) > 0 and q != 0xFFFFFFFF and int(passed[q]):
             p, L, w = int(mate_pos[k]), int(mate_len[k]), int(win_off[k])
-            ins = (w + int(ref_end[k]) + 1) - p if not mate_reverse[k] else (p + L) - (w + int(ref_start[k]))
+            ins = (w + int(ref_end[q]) + 1) - p if not mate_reverse[k] else (p + L) - (w + int(ref_start[q]))
             ok = 1 if min_insert <= ins <= max_insert else 0
         out.append(ok)
     return np.array(out, dtype=np.uint8)

@@ -22,7 +22,7 @@ SDP_MAX_CELL_VALUE = 16000
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only", "sdp_set_prefilter", "sdp_mate_windows",
+           "sdp_set_score_only", "sdp_set_prefilter", "sdp_mate_windows", "sdp_mate_pairs",
            "sdp_proper_pairs"]
 
 
@@ -107,7 +107,10 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_proper_pairs.restype = ctypes.c_int
     lib.sdp_proper_pairs.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_mates), ctypes.c_uint32, ctypes.c_uint32,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
-                                     ctypes.c_void_p, ctypes.c_void_p]
+                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    lib.sdp_mate_pairs.restype = ctypes.c_int
+    lib.sdp_mate_pairs.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p,
+                                   ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]
     lib.sdp_set_prefilter.restype = ctypes.c_int
     lib.sdp_set_prefilter.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_score_only.restype = ctypes.c_int
@@ -353,9 +356,22 @@ class Context:
                                                ctypes.c_void_p(win_len.data_ptr())))
         return win_off, win_len
 
+    def mate_pairs(self, win_len):
+        """sdp_mate_pairs: win_len CUDA tensor -> (pairs (P, 2) int32 CUDA tensor, pair_of_rescue int32 CUDA tensor)."""
+        import torch
+        n = int(win_len.numel())
+        pairs = torch.empty(max(2 * n, 1), dtype=torch.int32, device=win_len.device)
+        por = torch.empty(max(n, 1), dtype=torch.int32, device=win_len.device)
+        cnt = ctypes.c_uint64(0)
+        st = torch.cuda.current_stream(self.device)
+        self._check(self._lib.sdp_mate_pairs(self._h, ctypes.c_void_p(win_len.data_ptr()), n, ctypes.c_void_p(st.cuda_stream),
+                                             ctypes.c_void_p(pairs.data_ptr()), ctypes.c_void_p(por.data_ptr()),
+                                             ctypes.byref(cnt)))
+        return pairs[:2 * int(cnt.value)].reshape(-1, 2), por[:n]
+
     def proper_pairs(self, mate_pos, mate_len, mate_reverse, read_len, min_insert: int, max_insert: int, win_off, win_len,
-                     res: sdp_result):
-        """sdp_proper_pairs on the sdp_result of aligning rescue k against window k; returns a uint8 CUDA tensor."""
+                     res: sdp_result, pair_of_rescue=None):
+        """sdp_proper_pairs on the sdp_result of aligning the rescue batch; returns a uint8 CUDA tensor."""
         import torch
         n = int(mate_pos.numel())
         proper = torch.empty(n, dtype=torch.uint8, device=mate_pos.device)
@@ -363,6 +379,7 @@ class Context:
         st = torch.cuda.current_stream(self.device)
         self._check(self._lib.sdp_proper_pairs(self._h, ctypes.byref(m), int(min_insert), int(max_insert),
                                                ctypes.c_void_p(win_off.data_ptr()), ctypes.c_void_p(win_len.data_ptr()),
+                                               ctypes.c_void_p(pair_of_rescue.data_ptr()) if pair_of_rescue is not None else None,
                                                ctypes.c_void_p(res.ref_start), ctypes.c_void_p(res.ref_end),
                                                ctypes.c_void_p(res.pass_), ctypes.c_void_p(st.cuda_stream),
                                                ctypes.c_void_p(proper.data_ptr())))

@@ -22,19 +22,38 @@ __global__ void k_mate_windows(const sdp_mates mt, uint32_t min_ins, uint32_t ma
 }
 
 __global__ void k_proper_pairs(const sdp_mates mt, uint32_t min_ins, uint32_t max_ins, const uint64_t* __restrict__ win_off,
-                               const uint32_t* __restrict__ win_len, const int32_t* __restrict__ ref_start,
-                               const int32_t* __restrict__ ref_end, const uint8_t* __restrict__ pass,
-                               uint8_t* __restrict__ proper)
+                               const uint32_t* __restrict__ win_len, const uint32_t* __restrict__ pair_of_rescue,
+                               const int32_t* __restrict__ ref_start, const int32_t* __restrict__ ref_end,
+                               const uint8_t* __restrict__ pass, uint8_t* __restrict__ proper)
 {
     const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= mt.n) return;
     uint8_t ok = 0;
-    if (win_len[k] > 0 && pass[k]) {
+    const uint64_t q = pair_of_rescue ? (uint64_t)pair_of_rescue[k] : k;      // where rescue k sits in the aligned pair list
+    if (win_len[k] > 0 && q != (uint64_t)SDP_NO_PAIR && pass[q]) {
         const long long p = (long long)mt.mate_pos[k], L = (long long)mt.mate_len[k], w = (long long)win_off[k];
-        const long long ins = mt.mate_reverse[k] == 0 ? (w + ref_end[k] + 1) - p : (p + L) - (w + ref_start[k]);
+        const long long ins = mt.mate_reverse[k] == 0 ? (w + ref_end[q] + 1) - p : (p + L) - (w + ref_start[q]);
         ok = (ins >= (long long)min_ins && ins <= (long long)max_ins) ? 1 : 0;
     }
     proper[k] = ok;
+}
+
+// pair list of a rescue batch: rescues with a non-empty window, in rescue order (off = exclusive scan of the flags)
+__global__ void k_mate_flags(const uint32_t* __restrict__ win_len, uint64_t n, uint32_t* __restrict__ flag)
+{
+    const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) flag[k] = win_len[k] > 0 ? 1u : 0u;
+}
+__global__ void k_mate_pairs(const uint32_t* __restrict__ flag, const uint64_t* __restrict__ off, uint64_t n,
+                             uint32_t* __restrict__ pairs, uint32_t* __restrict__ pair_of_rescue)
+{
+    const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    if (flag[k]) {
+        const uint64_t q = off[k];
+        pairs[2 * q] = (uint32_t)k; pairs[2 * q + 1] = (uint32_t)k;
+        pair_of_rescue[k] = (uint32_t)q;
+    } else pair_of_rescue[k] = SDP_NO_PAIR;
 }
 
 void launch_mate_windows(const sdp_mates& mt, uint32_t min_ins, uint32_t max_ins, uint64_t ref_bases, uint64_t* win_off,
@@ -44,11 +63,22 @@ void launch_mate_windows(const sdp_mates& mt, uint32_t min_ins, uint32_t max_ins
 }
 
 void launch_proper_pairs(const sdp_mates& mt, uint32_t min_ins, uint32_t max_ins, const uint64_t* win_off,
-                         const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
-                         uint8_t* proper, cudaStream_t st)
+                         const uint32_t* win_len, const uint32_t* pair_of_rescue, const int32_t* ref_start,
+                         const int32_t* ref_end, const uint8_t* pass, uint8_t* proper, cudaStream_t st)
 {
-    if (mt.n) k_proper_pairs<<<(uint32_t)((mt.n + 255) / 256), 256, 0, st>>>(mt, min_ins, max_ins, win_off, win_len, ref_start,
-                                                                              ref_end, pass, proper);
+    if (mt.n) k_proper_pairs<<<(uint32_t)((mt.n + 255) / 256), 256, 0, st>>>(mt, min_ins, max_ins, win_off, win_len,
+                                                                              pair_of_rescue, ref_start, ref_end, pass, proper);
+}
+
+void launch_mate_flags(const uint32_t* win_len, uint64_t n, uint32_t* flag, cudaStream_t st)
+{
+    if (n) k_mate_flags<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(win_len, n, flag);
+}
+
+void launch_mate_pairs(const uint32_t* flag, const uint64_t* off, uint64_t n, uint32_t* pairs, uint32_t* pair_of_rescue,
+                       cudaStream_t st)
+{
+    if (n) k_mate_pairs<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(flag, off, n, pairs, pair_of_rescue);
 }
 
 }  // namespace sdp

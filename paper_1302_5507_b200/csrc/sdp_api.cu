@@ -106,8 +106,10 @@ struct sdp_ctx {
     DevBuf h_out;                    // one pinned slab, carved per call
     // sdp_best_per_read
     DevBuf rb_key, rb_pair, rb_score, rb_second, rb_ncand;
+    DevBuf mp_flag, mp_off;          // sdp_mate_pairs
     const uint32_t* last_pairs = nullptr;   // pair list of the last successful align call (to match results to it)
     uint64_t last_n_pairs = 0;
+    uint32_t last_n_reads = 0;
 };
 
 namespace {
@@ -309,7 +311,7 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
                       &ctx->in_win_nmask, &ctx->in_pairs, &ctx->tb_rows, &ctx->keys_wide, &ctx->order_wide,
                       &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits,
-                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand};
+                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
     for (int i = 0; i < 4; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
@@ -431,6 +433,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (P > 0xFFFFFFF0ull) return fail(ctx, SDP_EINVAL, "too many pairs");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CU(cudaSetDevice(ctx->device));
+    // a failed call may already have overwritten result buffers: its batch must not pass for the "last aligned" one
+    ctx->last_pairs = nullptr; ctx->last_n_pairs = 0; ctx->last_n_reads = 0;
     sdp_stats stats{};
     stats.n_pairs = P;
     uint32_t nl = 0;
@@ -457,7 +461,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (P == 0) {
         EN(cigar_ops, 16);
         ctx->stats = stats;
-        ctx->last_pairs = b.pairs; ctx->last_n_pairs = 0;
+        ctx->last_pairs = b.pairs; ctx->last_n_pairs = 0; ctx->last_n_reads = b.n_reads;
         finish(0);
         return SDP_OK;
     }
@@ -518,7 +522,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
             cudaEventElapsedTime(&stats.ms_forward, ctx->ev[EV_BUCKET], ctx->ev[EV_FORWARD]);
         }
         ctx->stats = stats;
-        ctx->last_pairs = b.pairs; ctx->last_n_pairs = P;
+        ctx->last_pairs = b.pairs; ctx->last_n_pairs = P; ctx->last_n_reads = b.n_reads;
         finish(0);
         return SDP_OK;
     }
@@ -670,7 +674,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         cudaEventElapsedTime(&stats.ms_compact, ctx->ev[EV_TRACE], ctx->ev[EV_END]);
     }
     ctx->stats = stats;
-    ctx->last_pairs = b.pairs; ctx->last_n_pairs = P;
+    ctx->last_pairs = b.pairs; ctx->last_n_pairs = P; ctx->last_n_reads = b.n_reads;
     finish(ctx->mb->totals[2]);
     return SDP_OK;
 }
@@ -682,7 +686,7 @@ int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* re
     ctx->err[0] = 0;
     if (!batch || !result || !out) return fail(ctx, SDP_EINVAL, "null batch, result or output");
     if (result->score != ctx->score.as<int32_t>() || result->n_pairs != batch->n_pairs ||
-        batch->pairs != ctx->last_pairs || batch->n_pairs != ctx->last_n_pairs)
+        batch->pairs != ctx->last_pairs || batch->n_pairs != ctx->last_n_pairs || batch->n_reads != ctx->last_n_reads)
         return fail(ctx, SDP_EINVAL, "result does not belong to the last sdp_align_batch of this ctx on this batch");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CU(cudaSetDevice(ctx->device));
@@ -715,17 +719,44 @@ int sdp_mate_windows(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, 
     return SDP_OK;
 }
 
+int sdp_mate_pairs(sdp_ctx* ctx, const uint32_t* win_len, uint64_t n, void* cuda_stream, uint32_t* pairs,
+                   uint32_t* pair_of_rescue, uint64_t* n_pairs)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (!n_pairs || (n && (!win_len || !pairs || !pair_of_rescue))) return fail(ctx, SDP_EINVAL, "null argument");
+    if (n > 0xFFFFFFF0ull) return fail(ctx, SDP_EINVAL, "too many rescues");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->device));
+    const size_t N = (size_t)(n ? n : 1);
+    EN(mp_flag, N * 4); EN(mp_off, N * 8);
+    EN(scan_local[0], N * 4); EN(scan_tiles[0], (N / 4096 + 2) * 4); EN(scan_tile_base[0], (N / 4096 + 2) * 8);
+    uint32_t nl = 0;
+    launch_mate_flags(win_len, n, ctx->mp_flag.as<uint32_t>(), st);
+    exclusive_scan_u32_u64(ctx->mp_flag.as<uint32_t>(), n, ctx->mp_off.as<uint64_t>(), ctx->totals + 2,
+                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
+                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
+    launch_mate_pairs(ctx->mp_flag.as<uint32_t>(), ctx->mp_off.as<uint64_t>(), n, pairs, pair_of_rescue, st);
+    CU(cudaMemcpyAsync(&ctx->mb->totals[2], ctx->totals + 2, 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    *n_pairs = ctx->mb->totals[2];
+    return SDP_OK;
+}
+
 int sdp_proper_pairs(sdp_ctx* ctx, const sdp_mates* mates, uint32_t min_insert, uint32_t max_insert, const uint64_t* win_off,
-                     const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
-                     void* cuda_stream, uint8_t* proper)
+                     const uint32_t* win_len, const uint32_t* pair_of_rescue, const int32_t* ref_start, const int32_t* ref_end,
+                     const uint8_t* pass, void* cuda_stream, uint8_t* proper)
 {
     if (!ctx) return SDP_EINVAL;
     ctx->err[0] = 0;
     if (!mates || !win_off || !win_len || !ref_start || !ref_end || !pass || !proper || min_insert > max_insert)
         return fail(ctx, SDP_EINVAL, "null argument or min_insert > max_insert");
+    if (mates->n && (!mates->mate_pos || !mates->mate_len || !mates->mate_reverse))
+        return fail(ctx, SDP_EINVAL, "null input array");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CU(cudaSetDevice(ctx->device));
-    launch_proper_pairs(*mates, min_insert, max_insert, win_off, win_len, ref_start, ref_end, pass, proper, st);
+    launch_proper_pairs(*mates, min_insert, max_insert, win_off, win_len, pair_of_rescue, ref_start, ref_end, pass, proper, st);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(st));
     return SDP_OK;

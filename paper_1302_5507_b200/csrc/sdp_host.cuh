@@ -105,8 +105,11 @@ void launch_best_per_read(uint64_t n_pairs, uint32_t n_reads, const uint32_t* pa
 void launch_mate_windows(const sdp_mates& mt, uint32_t min_ins, uint32_t max_ins, uint64_t ref_bases, uint64_t* win_off,
                          uint32_t* win_len, cudaStream_t st);
 void launch_proper_pairs(const sdp_mates& mt, uint32_t min_ins, uint32_t max_ins, const uint64_t* win_off,
-                         const uint32_t* win_len, const int32_t* ref_start, const int32_t* ref_end, const uint8_t* pass,
-                         uint8_t* proper, cudaStream_t st);
+                         const uint32_t* win_len, const uint32_t* pair_of_rescue, const int32_t* ref_start,
+                         const int32_t* ref_end, const uint8_t* pass, uint8_t* proper, cudaStream_t st);
+void launch_mate_flags(const uint32_t* win_len, uint64_t n, uint32_t* flag, cudaStream_t st);
+void launch_mate_pairs(const uint32_t* flag, const uint64_t* off, uint64_t n, uint32_t* pairs, uint32_t* pair_of_rescue,
+                       cudaStream_t st);
 
 // ---- microbench.cu
 int measure_dpx_rate(int device, double* rate, int32_t* sms, double* mhz);

@@ -1,10 +1,10 @@
 """GPU parity at BASELINE.json's full sizes (-m gpu), in the launch configuration bench.py times:
 one Context, device-resident inputs, one sdp_align_batch call per config on the full pair list.
 
-Config 2 (the headline workload, 1,000,000 pairs) is compared with the oracle on EVERY pair; for the
-other configs the oracle recomputes a seeded random sample of pairs one by one, and properties that
-hold at any size are checked on all pairs (score bounds, CIGAR consumes the read and the reported
-window span, offsets are the exclusive scan of the lengths)."""
+Every config is compared with the oracle on EVERY pair (the oracle needs about two minutes for the four
+configs on 16 host cores), and properties that hold at any size are checked on all pairs as well (score
+bounds, CIGAR consumes the read and the reported window span, offsets are the exclusive scan of the
+lengths). `sample` stays as a knob for quick local runs."""
 import os
 
 import numpy as np
@@ -63,7 +63,7 @@ def compare_sample(batch, got, idx, sc, what):
 
 
 @pytest.mark.skipif(not FULL, reason="SDP_FULL_SIZE_TESTS=0")
-@pytest.mark.parametrize("cfg,sample", [(2, None), (3, 60000), (4, 30000), (5, 60000)])
+@pytest.mark.parametrize("cfg,sample", [(2, None), (3, None), (4, None), (5, None)])
 def test_full_size_config(cfg, sample):
     batch = W.make_config(cfg)
     with Context(DEFAULT.match, DEFAULT.mismatch, DEFAULT.gap_open, DEFAULT.gap_extend, DEFAULT.min_similarity,

@@ -255,3 +255,48 @@ def test_similarity_threshold_edges():
     assert (r["n_match"], r["n_cols"], r["pass"]) == (9, 10, 1)
     r = oracle.align_pair(T, "ACGTTCGTAC", OracleScoring(1, -3, 5, 2, 0.900001))
     assert r["pass"] == 0
+
+
+# ---------------------------------------------------------------- batch wrapper: packed decode with N masks on BOTH sides
+def test_batch_decode_with_n_in_reads_and_windows():
+    """oracle_align_batch decodes 2-bit packed reads AND windows through their N bitmaps (reading R8). The expected
+    values come from the single-pair path on the original strings and, for the tiny cases, from brute force: a batch
+    wrapper that drops either mask (N then decodes as 'A') fails here."""
+    rng = random.Random(511)
+    sc = DEFAULT
+    wins, reads = [], []
+    for case in range(140):                         # brute-force sized, N-rich on both sides
+        wins.append(_rand_seq(rng, rng.randint(1, 6), "ACGNN"))
+        reads.append(_rand_seq(rng, rng.randint(1, 5), "ACNNA"))
+    for case in range(60):                          # longer, so that offsets cross word and mask-word boundaries
+        wins.append(_rand_seq(rng, rng.randint(20, 90), "ACGTN"))
+        reads.append(_rand_seq(rng, rng.randint(5, 40), "ACGTNA"))
+    # "A" vs "N": the mask is the only thing that separates them (N is packed as code 0 = A)
+    wins += ["AAAAAAAA", "NNNNNNNN", "AAAAAAAA", "ANANANAN"]
+    reads += ["ANAA", "AAAA", "NNNN", "NANA"]
+    b = W.batch_from_strings(wins, reads)
+    assert b.read_nmask is not None and b.win_nmask is not None
+    res = oracle.align_batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len, b.pairs, sc,
+                             read_nmask=b.read_nmask, win_nmask=b.win_nmask, threads=3)
+    n_read_n_matters = 0
+    for p, (T, R) in enumerate(zip(wins, reads)):
+        one = oracle.align_pair(T, R, sc)
+        got = dict(score=int(res.score[p]), ref_start=int(res.ref_start[p]), ref_end=int(res.ref_end[p]),
+                   read_start=int(res.read_start[p]), read_end=int(res.read_end[p]), n_match=int(res.n_match[p]),
+                   n_cols=int(res.n_cols[p]), cigar=res.cigar(p))
+        got["pass"] = int(res.passed[p])
+        for k, v in got.items():
+            assert one[k] == v, (p, T, R, k, one[k], v)
+        assert ref.rescore(T, R, got["ref_start"], got["cigar"], sc_tuple(sc)) == got["score"]
+        if len(R) <= 5 and len(T) <= 6:
+            c = ref.canonical(T, R, sc_tuple(sc))
+            for k in ("score", "ref_start", "ref_end", "cigar", "n_match", "n_cols"):
+                assert c[k] == got[k], (p, T, R, "bruteforce", k, c[k], got[k])
+        if "N" in R and oracle.align_pair(T, R.replace("N", "A"), sc)["score"] != got["score"]:
+            n_read_n_matters += 1
+    assert n_read_n_matters >= 20        # the read mask really decides scores in this batch
+    # hand-computed: read ANAA in AAAAAAAA is 3 matches + 1 mismatch = 0; all-N read or window: four mismatches = -12;
+    # NANA against ANANANAN at offset 1 pairs N with N (mismatch) and A with A: 2 - 6 = -4
+    k0 = len(wins) - 4
+    assert [int(x) for x in res.score[k0:]] == [0, -12, -12, -4]
+    assert [int(x) for x in res.n_match[k0:]] == [3, 0, 0, 2]
