@@ -43,21 +43,23 @@ extern "C" {
 #define SDP_MAX_READ_LEN 1024
 /*
  * int16 range rule (per pair, n = read length, m = window length):
- *     match*n + gap_extend*(n + m) + 3*gap_open + 64 <= SDP_MAX_CELL_VALUE
- * The kernels store H + gap_extend*(i+j) + bias in 16-bit lanes;
- * pairs that break the rule are rejected with SDP_ERANGE, never clamped.
+ *     match*n + gap_extend*(n + m + 32) + 3*gap_open + 8 + |2*gap_extend + mismatch| <= SDP_MAX_CELL_VALUE
+ * The kernels store H + gap_extend*(i+j) + bias in 16-bit lanes; the left side bounds every stored value and every
+ * intermediate sum (R13). Pairs that break the rule are never clamped.
  */
-#define SDP_MAX_CELL_VALUE 16000
+#define SDP_MAX_CELL_VALUE 32000
+/* Largest magnitude of match, mismatch, gap_open and gap_extend sdp_create accepts. */
+#define SDP_MAX_SCORE_PARAM 4000
 
 typedef struct sdp_ctx sdp_ctx;   /* opaque; owns device scratch, result buffers, pinned staging */
 
 /* Scoring of PAPER.md:283: S_MA = match, S_MI = mismatch, S_GO = -(gap_open + gap_extend),
  * S_GE = -gap_extend, i.e. a gap of k bases costs gap_open + k*gap_extend. */
 typedef struct sdp_scoring {
-    int32_t match;           /* >= 0, and match - mismatch > 0                                  */
-    int32_t mismatch;        /* <= 0                                                            */
-    int32_t gap_open;        /* >= 0                                                            */
-    int32_t gap_extend;      /* >= 1                                                            */
+    int32_t match;           /* 0 .. SDP_MAX_SCORE_PARAM, and match - mismatch > 0              */
+    int32_t mismatch;        /* -SDP_MAX_SCORE_PARAM .. 0                                       */
+    int32_t gap_open;        /* 0 .. SDP_MAX_SCORE_PARAM                                        */
+    int32_t gap_extend;      /* 1 .. SDP_MAX_SCORE_PARAM                                        */
     double  min_similarity;  /* in [0,1]; quantised once as q = llround(x * 1e6); a pair passes  */
                              /* iff n_match * 1e6 >= q * n_cols (n_cols = CIGAR columns)         */
 } sdp_scoring;
@@ -124,11 +126,16 @@ typedef struct sdp_stats {
  * SDP_ECUDA / SDP_ENOMEM otherwise; *out is written only on success. Not thread-safe: use one
  * ctx per thread; separate ctxs are independent. */
 int sdp_create(const sdp_scoring* scoring, int cuda_device, sdp_ctx** out);
-/* Environment variables read by sdp_create (tests and tuning only; results never depend on them):
- *   SDP_NO_EXACT=1  use the general five-instruction score kernels even when 2*extend + mismatch >= 0
- *   SDP_NO_THIN=1   send pairs with gap bound W >= 1 to the wide / generic traceback instead of the narrow-band kernels
- *   SDP_NO_WIDE=1   send wide pairs to the generic scalar band kernel instead of the wavefront traceback kernel
- *   SDP_FORCE_G=g   threads per pair group for every read length that admits it (geometry experiments) */
+/* Test and tuning hook; results never depend on it (tests/test_gpu_parity.py routes the same pairs through every
+ * traceback kernel and requires identical output). flags = OR of the SDP_ROUTE_* bits and SDP_ROUTE_FORCE_G(g):
+ *   SDP_ROUTE_NO_THIN      pairs with gap bound W >= 1 go to the wide / generic traceback instead of the narrow-band kernels
+ *   SDP_ROUTE_NO_WIDE      wide pairs go to the generic scalar band kernel instead of the wavefront traceback kernel
+ *   SDP_ROUTE_FORCE_G(g)   g threads per pair group for every read length that admits it (geometry experiments), 0 = off
+ * 0 restores the default routing. SDP_EINVAL for unknown bits. */
+#define SDP_ROUTE_NO_THIN 1u
+#define SDP_ROUTE_NO_WIDE 2u
+#define SDP_ROUTE_FORCE_G(g) (((uint32_t)(g) & 0x3Fu) << 8)
+int sdp_set_debug_route(sdp_ctx* ctx, uint32_t flags);
 
 /* Align every pair of `batch` (DEVICE pointers). Work is enqueued on `cuda_stream`
  * (a cudaStream_t; NULL = default stream) and the call returns after the stream has completed

@@ -18,11 +18,12 @@ LIB_PATH = os.path.join(_HERE, "libsdp.so")
 
 SDP_OK, SDP_EINVAL, SDP_ERANGE, SDP_ECUDA, SDP_ENOMEM = 0, -1, -2, -3, -4
 SDP_MAX_READ_LEN = 1024
-SDP_MAX_CELL_VALUE = 16000
+SDP_MAX_CELL_VALUE = 32000
+SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE = 1, 2
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only", "sdp_set_prefilter", "sdp_mate_windows", "sdp_mate_pairs",
+           "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_mate_windows", "sdp_mate_pairs",
            "sdp_proper_pairs"]
 
 
@@ -113,6 +114,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
                                    ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]
     lib.sdp_set_prefilter.restype = ctypes.c_int
     lib.sdp_set_prefilter.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    lib.sdp_set_debug_route.restype = ctypes.c_int
+    lib.sdp_set_debug_route.argtypes = [ctypes.c_void_p, ctypes.c_uint32]
     lib.sdp_set_score_only.restype = ctypes.c_int
     lib.sdp_set_score_only.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_get_stats.restype = ctypes.c_int
@@ -245,6 +248,11 @@ class Context:
 
     def set_prefilter(self, enabled: bool):
         self._lib.sdp_set_prefilter(self._h, int(bool(enabled)))
+
+    def set_debug_route(self, no_thin: bool = False, no_wide: bool = False, force_g: int = 0):
+        """sdp_set_debug_route: route pairs through the other traceback kernels / force a thread-group size (tests)."""
+        flags = (SDP_ROUTE_NO_THIN if no_thin else 0) | (SDP_ROUTE_NO_WIDE if no_wide else 0) | ((int(force_g) & 0x3F) << 8)
+        self._check(self._lib.sdp_set_debug_route(self._h, flags))
 
     def set_score_only(self, enabled: bool):
         self._lib.sdp_set_score_only(self._h, int(bool(enabled)))

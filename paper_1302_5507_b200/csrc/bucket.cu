@@ -83,8 +83,8 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
             if (n < 1 || m < 1 || ro + n > b.reads_bases || wo + m > b.wins_bases || ro + n < ro || wo + m < wo)
                 err = SDP_ERRF_INDEX;
             else if (n > SDP_MAX_READ_LEN ||
-                     (long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + m) + 3LL * sc.gap_open + 64 >
-                         SDP_MAX_CELL_VALUE)
+                     (long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + m + 32) + 3LL * sc.gap_open + 8 +
+                             llabs(2LL * sc.gap_extend + sc.mismatch) > SDP_MAX_CELL_VALUE)
                 err = SDP_ERRF_RANGE;
             else {
                 key = (n - 1) * 64u + min(63u, m >> 6);

@@ -12,7 +12,7 @@ namespace sdp {
 
 template <int K>
 static inline bool dispatch_range(int k, bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
-    if (k == K) { launch_score_K<K>(pad, rev, p.c.exact != 0, p, st); return true; }
+    if (k == K) { launch_score_K<K>(pad, rev, p, st); return true; }
     if constexpr (K < SDP_K_HI) return dispatch_range<K + 1>(k, pad, rev, p, st);
     else return false;
 }

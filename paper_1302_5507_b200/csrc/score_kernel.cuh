@@ -11,24 +11,22 @@
 // How: nothing like the paper's global-memory tables survives.
 //  * int16x2 lanes hold TWO pairs; a group of G threads owns the read's n columns, K per thread,
 //    H/F columns live in registers, the window streams by as rows, and thread g works on row
-//    s - g at step s (anti-diagonal wavefront); H and E of the chunk's last column cross to the
-//    right neighbour with one warp shuffle each per row.
-//  * drift form: stored values are H + e*(i+j) + beta, so gap extension needs no add:
-//        E' = max(H'(i,j-1) - o, E'(i,j-1))          VIADDMNMX.S16x2   (on the row's serial chain)
-//        F' = max(H'(i-1,j) - o, F'(i-1,j))          VIADDMNMX.S16x2   (off the chain)
-//        u  = max(H'(i-1,j-1) + q, F')               VIADDMNMX.S16x2   (off the chain)
-//        H' = max(u, E')                             VIMNMX.S16x2      (on the chain)
-//    with q = 2e + delta(T[i], R[j]) EXACT: 2e+match or 2e+mismatch. Four ALU-pipe instructions per
-//    two cells. q comes from the FMA pipe, which runs beside the ALU pipe (measured: DESIGN.md
-//    "Pipes"): base codes are fp16 values at least 1 apart, d = t - r (HADD2),
-//    g = sat(1 - d*d) (HFMA2.SAT: 1.0 iff the bases are equal, else 0.0), q = g*Cd + Cy (HFMA2) with
-//    Cd, Cy the fp16 DENORMALS whose bit patterns are the integers (match - mismatch) and
-//    (2e + mismatch): the result's bit pattern IS the integer q. This needs 2e + mismatch >= 0
-//    (EXACT variant). Otherwise (general variant) q = Cf - d*d with Cf the denormal 2e+match: d == 0
-//    gives exactly Cf, d != 0 a negative half whose bits read as int16 are below -15000, and the
-//    mismatch candidate costs a fifth instruction t = max(H'(i-1,j-1) + (2e+mismatch), F').
-//    No integer multiply-add and no register move is wanted in the loop: IMAD and IMAD.MOV issue at
-//    a quarter of the HFMA2 rate on sm_100a (measured) and starve the FMA pipe.
+//    s - 2g at step s (anti-diagonal wavefront, two rows of skew per thread: SDP_SCORE_SKEW); H and E of the
+//    chunk's last column cross to the right neighbour with one warp shuffle each per row.
+//  * drift form: stored values are H + e*(i+j) + beta, so gap extension needs no add. With
+//    c = 2e + mismatch (any sign) and q' = delta - mismatch = (match - mismatch) or 0:
+//        F~ = max(H'(i-1,j) - (o + c), F~(i-1,j))      VIADDMNMX.S16x2   F~ = F' - c         (off the chain)
+//        u~ = max(H'(i-1,j-1) + q', F~)                VIADDMNMX.S16x2   u~ = u - c          (off the chain)
+//        E' = max(H'(i,j-1) - o, E'(i,j-1))            VIADDMNMX.S16x2                       (the row's serial chain)
+//        H' = max(u~ + c, E')                          VIADDMNMX.S16x2                       (the row's serial chain)
+//    Four ALU-pipe instructions per two cells, for EVERY scoring. q' comes from the FMA pipe, which runs beside the ALU pipe (measured: DESIGN.md "Pipes"), in
+//    two instructions: base codes are fp16 values at least 1 apart, d = t - r (HADD2) and
+//    q' = relu(Cd - d*d) (HFMA2.RELU) with Cd the fp16 DENORMAL whose bit pattern is the integer match - mismatch:
+//    d == 0 gives exactly Cd (the FMA is not flush-to-zero), |d| >= 1 a negative value that relu turns into +0,
+//    so the result's bit pattern IS the integer q'. Shifting F and u by c moves the constant part of the
+//    diagonal increment into the add of the H' update, which a plain max left unused.
+//    No integer multiply-add and no register move is wanted in the column loop: IMAD and IMAD.MOV cost two
+//    FMA-pipe slots on sm_100a (measured).
 //  * window rows: the 2-bit window bases of both lanes are expanded once per chunk of rows into
 //    a per-group shared-memory ring of 16-bit PRMT selectors; a row then costs one LDS.U16 and one
 //    PRMT to obtain the fp16 codes of both lanes (instead of two address computations, two global
@@ -63,11 +61,15 @@ __device__ __forceinline__ uint32_t prmt_raw(uint32_t a, uint32_t b, uint32_t se
 __device__ __forceinline__ uint32_t hsub2_u(uint32_t a, uint32_t b) {
     uint32_t d; asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d;
 }
-// c - d*d per fp16 lane; non-ftz so a denormal addend survives
-__device__ __forceinline__ uint32_t hfma2_negsq(uint32_t d, uint32_t c) {
+// relu(c - d*d) per fp16 lane; non-ftz so a denormal c survives: c when d == 0, +0 when d*d > c
+__device__ __forceinline__ uint32_t hfma2_relu_negsq(uint32_t d, uint32_t c) {
     uint32_t r;
-    asm("{.reg .b32 nd; neg.f16x2 nd, %1; fma.rn.f16x2 %0, %1, nd, %2;}" : "=r"(r) : "r"(d), "r"(c));
+    asm("{.reg .b32 nd; neg.f16x2 nd, %1; fma.rn.relu.f16x2 %0, %1, nd, %2;}" : "=r"(r) : "r"(d), "r"(c));
     return r;
+}
+// a * m + c as a 32-bit integer multiply-add (FMA pipe): with m in {0, 1} a select that stays off the ALU pipe
+__device__ __forceinline__ uint32_t imad_sel(uint32_t a, uint32_t m, uint32_t c) {
+    uint32_t r; asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(m), "r"(c)); return r;
 }
 // sat(1 - d*d) per fp16 lane: 1.0 when d == 0, 0.0 when |d| >= 1
 __device__ __forceinline__ uint32_t hfma2_is_zero(uint32_t d) {
@@ -98,6 +100,36 @@ __device__ __forceinline__ uint32_t vibmax_s16x2(uint32_t a, uint32_t b, bool* a
         "selp.b32 %2, 1, 0, pv;} \n\t"
         : "=&r"(val), "=&r"(phi), "=&r"(plo) : "r"(a), "r"(b));
     *a_ge_b_hi = (phi != 0); *a_ge_b_lo = (plo != 0);
+    return val;
+}
+// running maximum with its row: val = max(a, b) per int16 lane; a lane's index becomes i when the lane of `a` LOST
+// (KEEP_A_ON_TIE) or when the lane of `a` won or tied (!KEEP_A_ON_TIE ... see callers). One VIMNMX.S16x2 that also
+// writes the two "a >= b" predicates, and two predicated moves.
+template <bool MOVE_IF_A_WINS>
+__device__ __forceinline__ uint32_t vibmax_track(uint32_t a, uint32_t b, int i, int& idx_lo, int& idx_hi) {
+    uint32_t val;
+    if (MOVE_IF_A_WINS)
+        asm("{.reg .pred pu, pv; \n\t"
+            ".reg .s16 rs0, rs1, rs2, rs3; \n\t"
+            "max.s16x2 %0, %3, %4; \n\t"
+            "mov.b32 {rs0, rs1}, %0; \n\t"
+            "mov.b32 {rs2, rs3}, %3; \n\t"
+            "setp.eq.s16 pv, rs0, rs2; \n\t"
+            "setp.eq.s16 pu, rs1, rs3; \n\t"
+            "@pv mov.b32 %1, %5; \n\t"
+            "@pu mov.b32 %2, %5;} \n\t"
+            : "=&r"(val), "+r"(idx_lo), "+r"(idx_hi) : "r"(a), "r"(b), "r"(i));
+    else
+        asm("{.reg .pred pu, pv; \n\t"
+            ".reg .s16 rs0, rs1, rs2, rs3; \n\t"
+            "max.s16x2 %0, %3, %4; \n\t"
+            "mov.b32 {rs0, rs1}, %0; \n\t"
+            "mov.b32 {rs2, rs3}, %3; \n\t"
+            "setp.eq.s16 pv, rs0, rs2; \n\t"
+            "setp.eq.s16 pu, rs1, rs3; \n\t"
+            "@!pv mov.b32 %1, %5; \n\t"
+            "@!pu mov.b32 %2, %5;} \n\t"
+            : "=&r"(val), "+r"(idx_lo), "+r"(idx_hi) : "r"(a), "r"(b), "r"(i));
     return val;
 }
 __device__ __forceinline__ uint32_t blend(uint32_t mask, uint32_t a, uint32_t b) {  // mask ? a : b
@@ -143,13 +175,14 @@ __device__ __forceinline__ uint32_t reverse_bits16(uint32_t x) { return __brev(x
 
 // Shared-memory ring of window-row selectors: per warp SDP_RING_WORDS 32-bit words, carved into one
 // region per group. A region holds `ring` 16-bit entries (row i at slot (i-1) & (ring-1), stored at
-// position slot + 32) plus a 32-entry mirror of the ring's tail in front of it, so that thread g
-// can read row s-g at position ((s-1) & (ring-1)) + 32 - g without a wrap test.
+// position slot + mirror) plus a `mirror`-entry copy of the ring's tail in front of it, so that thread g
+// can read row s - skew*g at position ((s-1) & (ring-1)) + mirror - skew*g without a wrap test.
 struct RingGeom {
-    int chunk, ring, stride_w;
+    int chunk, ring, stride_w, mirror;
 };
-__device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups) {
+__device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups, int skew) {
     RingGeom r;
+    r.mirror = skew * (G - 1) > 32 ? 64 : 32;             // (64 only when one group fills the warp)
     if (G == 1)      { r.chunk = 32; r.stride_w = 49; }
     else if (G == 2) { r.chunk = 32; r.stride_w = 50; }
     else {
@@ -187,8 +220,8 @@ __device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingG
                          : load_bits16(P.win_nmask, (long long)woffB + r0, nm_words);
         }
         const int slot0 = r0 & (rg.ring - 1);
-        uint32_t* dst = ring_w + 16 + (slot0 >> 1);
-        uint32_t* mir = (slot0 >= rg.ring - 32) ? ring_w + ((slot0 - (rg.ring - 32)) >> 1) : nullptr;
+        uint32_t* dst = ring_w + ((rg.mirror + slot0) >> 1);
+        uint32_t* mir = (slot0 >= rg.ring - rg.mirror) ? ring_w + ((slot0 - (rg.ring - rg.mirror)) >> 1) : nullptr;
 #pragma unroll
         for (int tt = 0; tt < 8; ++tt) {
             // two rows -> two 16-bit selectors (idxA * 0x11 | idxB * 0x1100)
@@ -214,13 +247,29 @@ __device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingG
 #define SDP_ROWS_UNROLL 8
 #endif
 
+// Rows between neighbouring threads of a group: thread g works on row s - SDP_SCORE_SKEW*g at step s. With 1 the
+// H'/E' a thread receives at step s were finished by its left neighbour at the very end of step s-1, so the serial
+// chains of consecutive steps cannot overlap and a warp waits out the ALU latency between dependent chain
+// instructions (measured: a third of the issue slots idle). With 2 they were finished at step s-2: the chains of two
+// consecutive steps are independent (row i+1 only trails row i by a column inside the thread) and ptxas interleaves them.
+#ifndef SDP_SCORE_SKEW
+#define SDP_SCORE_SKEW 2
+#endif
+
 // resident CTAs per SM the register budget is sized for: 128 registers up to K = 21, 168 above
 #ifndef SDP_SCORE_MIN_CTAS
 #define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)
 #endif
 
-// EXACT: 2e + mismatch >= 0, the four-instruction recurrence; otherwise the general five-instruction one
-template <int K, bool REV, bool PAD, bool EXACT>
+// IMM: the scoring constants are the compile-time values SDP_IMM_* (instruction immediates) instead of registers.
+// Each VIADDMNMX then reads two registers instead of three, which matters because the register file delivers one
+// operand per bank per cycle to BOTH pipes: with three-register DPX instructions the fp16 instructions of the
+// FMA pipe no longer fit beside them (measured: 10.1 against 9.0 cycles per column for the same instruction mix).
+#define SDP_IMM_MATCH 1
+#define SDP_IMM_MISMATCH (-3)
+#define SDP_IMM_OPEN 5
+#define SDP_IMM_EXTEND 2
+template <int K, bool REV, bool PAD, bool IMM>
 __global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))
 score_kernel(const ScoreParams P)
 {
@@ -281,25 +330,33 @@ score_kernel(const ScoreParams P)
         }
         rh[k] = read_code_half(cA) | (read_code_half(cB) << 16);
         H[k] = h_row0;
-        F[k] = 0u;                                        // F'(0,j) = -inf: 0 <= beta - 2o
+        F[k] = 0u;                                        // F~(0,j) = -inf: 0 <= beta - 2o - c
     }
 
     // ---- window-row selector ring of this group
-    const RingGeom rg = ring_geometry(G, ngroups);
+    constexpr int SKEW = SDP_SCORE_SKEW;
+    const RingGeom rg = ring_geometry(G, ngroups, SKEW);
     uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
-    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
+    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - SKEW * g;
 
     auto fill_ring = [&](const int s0) {                  // rows s0+1 .. s0+chunk
         if (in_group) fill_ring_rows<REV>(P, rg, ring_w, g, G, s0, dA.woff, mA, dB.woff, mB);
     };
 
-    const uint32_t negO = P.c.negO, cmis = P.c.cmis, Cf = P.c.Cf, Cd = P.c.Cd, e2 = P.c.e2;
-    const uint32_t notfirst = opaque_u32(is_first ? 0u : 0xFFFFFFFFu);   // a mask, not a predicate: one LOP3 per use
-    // boundary column 0 as seen by the group's first thread: H'(i,0) = beta + e*i (forward, free
-    // start) or beta - o (reverse, start anchored: a leading deletion of i bases costs o + e*i)
+    constexpr int IMM_C = 2 * SDP_IMM_EXTEND + SDP_IMM_MISMATCH;
+    const uint32_t negOc = IMM ? sdp_pack2(-(SDP_IMM_OPEN + IMM_C)) : P.c.negOc, negO = IMM ? sdp_pack2(-SDP_IMM_OPEN) : P.c.negO;
+    const uint32_t c2 = IMM ? sdp_pack2(IMM_C) : P.c.c2, Cd = IMM ? sdp_pack2(SDP_IMM_MATCH - SDP_IMM_MISMATCH) : P.c.Cd;
+    const uint32_t e2 = IMM ? sdp_pack2(SDP_IMM_EXTEND) : P.c.e2;
+    // 1 for every thread but the group's first: hin * notfirst + fv is a select on the FMA pipe (kept opaque so
+    // that it stays a multiplier instead of becoming a predicate and an ALU-pipe SEL)
+    const uint32_t notfirst = opaque_u32(is_first ? 0u : 1u);
+    // boundary column 0 as seen by the group's first thread: H'(i,0) = beta + e*i (forward, free start) or
+    // beta - o (reverse, start anchored: a leading deletion of i bases costs o + e*i)
     uint32_t fv = is_first ? (REV ? P.c.betaMinusO2 : P.c.beta2) : 0u;
     const uint32_t fstep = (is_first && !REV) ? e2 : 0u;
-    uint32_t hout = h_row0, eout = 0u;
+    // what the right neighbour fetches: H'(i, last column), E'(i, last column). With a skew of two rows the values of
+    // two steps are in flight, alternating between the two sets.
+    uint32_t houtA = h_row0, eoutA = 0u, houtB = h_row0, eoutB = 0u;
     uint32_t hdiag = is_first ? P.c.beta2 : h_row0;       // H'(0, left boundary column)
     // running maximum of H(i,n) in the drift frame of the current row: best += e per row, so that
     // H'(i,n) can be compared with it directly. Reverse: row 0 (all-insertion) counts.
@@ -307,9 +364,9 @@ score_kernel(const ScoreParams P)
     int idxA = 0, idxB = 0;
 
     // One DP row of this thread's K columns. Hs = H'(i-1, .) is only read, Hn receives H'(i, .):
-    // two register sets that swap roles from row to row, so that no H' value is ever copied (the
-    // diagonal term of column k is accumulated in Hn[k] before the serial chain reaches it).
-    auto row_step = [&](const int i, const uint16_t* rp, auto slow_tag, const uint32_t (&Hs)[K], uint32_t (&Hn)[K]) {
+    // two register sets that swap roles from row to row, so that no H' value is ever copied.
+    auto row_step = [&](const int i, const uint16_t* rp, auto slow_tag, const uint32_t (&Hs)[K], uint32_t (&Hn)[K],
+                        uint32_t& hout, uint32_t& eout) {
         constexpr bool SLOW = decltype(slow_tag)::value;
         uint32_t hin = __shfl_up_sync(0xffffffffu, hout, 1);
         uint32_t ein = __shfl_up_sync(0xffffffffu, eout, 1);
@@ -319,35 +376,35 @@ score_kernel(const ScoreParams P)
             return;
         }
         fv = __vadd2(fv, fstep);
-        hin = (hin & notfirst) | fv;
-        ein = ein & notfirst;
+        hin = imad_sel(hin, notfirst, fv);
+        ein = imad_sel(ein, notfirst, 0u);                // E'(i,0) = -inf
         // fp16 codes of the window bases of row i, both lanes
         const uint32_t nt = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
 
         uint32_t Hl = hin, E = ein;
         uint32_t Hsk = hin, Esk = ein;                    // outputs if the last column is skipped
-        // u[k] = max(H'(i-1,k-1) + q, F'(i,k)): everything of column k that does not wait for the chain
+        // u~[k] = max(H'(i-1,k-1) + q', F~(i,k)): everything of column k that does not wait for the chain
         auto off_chain = [&](const int k, const uint32_t hd) -> uint32_t {
             const uint32_t d = hsub2_u(nt, rh[k]);
-            F[k] = __viaddmax_s16x2(Hs[k], negO, F[k]);
-            if (EXACT) return __viaddmax_s16x2(hd, hfma2_u(hfma2_is_zero(d), Cd, cmis), F[k]);
-            const uint32_t t = __viaddmax_s16x2(hd, cmis, F[k]);
-            return __viaddmax_s16x2(hd, hfma2_negsq(d, Cf), t);
+            F[k] = __viaddmax_s16x2(Hs[k], negOc, F[k]);
+            return __viaddmax_s16x2(hd, hfma2_relu_negsq(d, Cd), F[k]);
         };
         Hn[0] = off_chain(0, hdiag);
         hdiag = hin;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             if (k + 1 < K) Hn[k + 1] = off_chain(k + 1, Hs[k]);
-            E = __viaddmax_s16x2(Hl, negO, E);
-            Hl = __vmaxs2(Hn[k], E);
+            E = __viaddmax_s16x2(Hl, negO, E);            // E'(i,k)
+            Hl = __viaddmax_s16x2(Hn[k], c2, E);          // H'(i,k) = max(u~ + c, E')
             Hn[k] = Hl;
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }
         if (PAD) { hout = blend(skipmask, Hsk, Hl); eout = blend(skipmask, Esk, E); }
         else     { hout = Hl; eout = E; }
 
-        if (is_last) {
+        {   // Running maximum of the thread's last column; only the group's last thread holds H'(i,n) there, the other
+            // threads' copies are never read. Unconditional on purpose: under a predicate ptxas computes into
+            // temporaries and pays a conditional register move per value.
             // strict > keeps the lowest row (forward), >= keeps the highest (reverse)
             best = __vadd2(best, e2);
             uint32_t cmp = Hl;
@@ -355,29 +412,86 @@ score_kernel(const ScoreParams P)
                 const uint32_t ok = (i <= mA ? 0x0000FFFFu : 0u) | (i <= mB ? 0xFFFF0000u : 0u);
                 cmp = blend(ok, cmp, 0x80008000u);
             }
-            bool p_hi, p_lo;
-            if (REV) {
-                best = vibmax_s16x2(cmp, best, &p_hi, &p_lo);       // p = cmp >= best
-                if (p_lo) idxA = i;
-                if (p_hi) idxB = i;
-            } else {
-                best = vibmax_s16x2(best, cmp, &p_hi, &p_lo);       // p = best >= cmp
-                if (!p_lo) idxA = i;
-                if (!p_hi) idxB = i;
-            }
+            if (REV) best = vibmax_track<true>(cmp, best, i, idxA, idxB);     // row i takes over when cmp >= best
+            else     best = vibmax_track<false>(best, cmp, i, idxA, idxB);    // ... when not (best >= cmp)
         }
     };
+    // Two consecutive steps of the steady state (rows ia and ia + 1 of this thread) as ONE skewed pass: column k of
+    // the first row, then column k-1 of the second, which needs nothing of the first row beyond column k-1. The two
+    // rows' serial chains are independent (SKEW == 2: both rows' inputs were shuffled in before the pass), so each
+    // chain instruction has the other row's work between itself and its successor, and no second H' register set
+    // is needed: the second row takes H'(ia, k-1) straight from the first row's chain.
+    auto row_pair = [&](const int ia, const uint16_t* rp) {
+        uint32_t hinA = __shfl_up_sync(0xffffffffu, houtA, 1);
+        uint32_t einA = __shfl_up_sync(0xffffffffu, eoutA, 1);
+        uint32_t hinB = __shfl_up_sync(0xffffffffu, houtB, 1);
+        uint32_t einB = __shfl_up_sync(0xffffffffu, eoutB, 1);
+        fv = __vadd2(fv, fstep);
+        hinA = imad_sel(hinA, notfirst, fv);
+        einA = imad_sel(einA, notfirst, 0u);
+        fv = __vadd2(fv, fstep);
+        hinB = imad_sel(hinB, notfirst, fv);
+        einB = imad_sel(einB, notfirst, 0u);
+        const uint32_t ntA = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[0]);
+        const uint32_t ntB = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[1]);
+
+        uint32_t HlA = hinA, EA = einA, HlB = hinB, EB = einB;
+        uint32_t hdA = hdiag, hdB = hinA;                 // H'(ia-1, left), H'(ia, left)
+        hdiag = hinB;
+        uint32_t HskA = hinA, EskA = einA, HskB = hinB, EskB = einB;
+        uint32_t prevA = hinA;                            // H'(ia, k-1)
+#pragma unroll
+        for (int k = 0; k <= K; ++k) {
+            const uint32_t upB = prevA;                   // H'(ia, k-1): the second row's "row above" at column k-1
+            if (k < K) {                                  // first row, column k
+                const uint32_t d = hsub2_u(ntA, rh[k]);
+                F[k] = __viaddmax_s16x2(H[k], negOc, F[k]);
+                const uint32_t u = __viaddmax_s16x2(hdA, hfma2_relu_negsq(d, Cd), F[k]);
+                hdA = H[k];
+                EA = __viaddmax_s16x2(HlA, negO, EA);
+                HlA = __viaddmax_s16x2(u, c2, EA);
+                prevA = HlA;
+                if (PAD && k == K - 2) { HskA = HlA; EskA = EA; }
+            }
+            if (k >= 1) {                                 // second row, column k-1
+                const uint32_t d = hsub2_u(ntB, rh[k - 1]);
+                F[k - 1] = __viaddmax_s16x2(upB, negOc, F[k - 1]);
+                const uint32_t u = __viaddmax_s16x2(hdB, hfma2_relu_negsq(d, Cd), F[k - 1]);
+                hdB = upB;
+                EB = __viaddmax_s16x2(HlB, negO, EB);
+                HlB = __viaddmax_s16x2(u, c2, EB);
+                H[k - 1] = HlB;
+                if (PAD && k - 1 == K - 2) { HskB = HlB; EskB = EB; }
+            }
+        }
+        if (PAD) {
+            houtA = blend(skipmask, HskA, HlA); eoutA = blend(skipmask, EskA, EA);
+            houtB = blend(skipmask, HskB, HlB); eoutB = blend(skipmask, EskB, EB);
+        } else { houtA = HlA; eoutA = EA; houtB = HlB; eoutB = EB; }
+        best = __vadd2(best, e2);
+        if (REV) best = vibmax_track<true>(HlA, best, ia, idxA, idxB);
+        else     best = vibmax_track<false>(best, HlA, ia, idxA, idxB);
+        best = __vadd2(best, e2);
+        if (REV) best = vibmax_track<true>(HlB, best, ia + 1, idxA, idxB);
+        else     best = vibmax_track<false>(best, HlB, ia + 1, idxA, idxB);
+    };
+    // one step outside the unrolled loop; the two output sets trade places afterwards
     auto row_step1 = [&](const int i, const uint16_t* rp, auto slow_tag) {
         uint32_t H2[K];
-        row_step(i, rp, slow_tag, H, H2);
+        row_step(i, rp, slow_tag, H, H2, houtA, eoutA);
 #pragma unroll
         for (int k = 0; k < K; ++k) H[k] = H2[k];
+        if (SKEW == 2) {
+            const uint32_t th = houtA, te = eoutA;
+            houtA = houtB; eoutA = eoutB; houtB = th; eoutB = te;
+        }
     };
 
-    // step s: thread g works on row s - g. Steps 1..G-1 fill the wavefront, steps up to
-    // Mmin+G-1 are the steady state (two rows per iteration), the rest drain lanes whose
+    // step s: thread g works on row s - SKEW*g. Steps 1..SKEW*(G-1) fill the wavefront, steps up to
+    // Mmin+SKEW*(G-1) are the steady state (SDP_ROWS_UNROLL rows per iteration), the rest drain lanes whose
     // window is longer.
-    const int fast_end = Mmin + G - 1, all_end = Mmax + G - 1;
+    const int lead = SKEW * (G - 1);
+    const int fast_end = Mmin + lead, all_end = Mmax + lead;
     for (int s0 = 0; s0 < all_end; s0 += rg.chunk) {
         fill_ring(s0);
         __syncwarp();
@@ -385,21 +499,26 @@ score_kernel(const ScoreParams P)
         const uint16_t* rp = rp0 + (s0 & (rg.ring - 1));
         int s = s0 + 1;
 #pragma unroll 1
-        for (; s <= min(send, G - 1); ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+        for (; s <= min(send, lead); ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
         const int fe = min(send, fast_end);
 #pragma unroll 1
         for (; s + SDP_ROWS_UNROLL - 1 <= fe; s += SDP_ROWS_UNROLL, rp += SDP_ROWS_UNROLL) {
-            uint32_t H2[K];
+            if (SKEW == 2) {
 #pragma unroll
-            for (int r = 0; r < SDP_ROWS_UNROLL; r += 2) {
-                row_step(s + r - g, rp + r, std::false_type{}, H, H2);
-                row_step(s + r + 1 - g, rp + r + 1, std::false_type{}, H2, H);
+                for (int r = 0; r < SDP_ROWS_UNROLL; r += 2) row_pair(s + r - SKEW * g, rp + r);
+            } else {
+                uint32_t H2[K];
+#pragma unroll
+                for (int r = 0; r < SDP_ROWS_UNROLL; r += 2) {
+                    row_step(s + r - SKEW * g, rp + r, std::false_type{}, H, H2, houtA, eoutA);
+                    row_step(s + r + 1 - SKEW * g, rp + r + 1, std::false_type{}, H2, H, houtA, eoutA);
+                }
             }
         }
 #pragma unroll 1
-        for (; s <= fe; ++s, ++rp) row_step1(s - g, rp, std::false_type{});
+        for (; s <= fe; ++s, ++rp) row_step1(s - SKEW * g, rp, std::false_type{});
 #pragma unroll 1
-        for (; s <= send; ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+        for (; s <= send; ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
     }
 
     if (is_last) {
@@ -419,20 +538,19 @@ score_kernel(const ScoreParams P)
 }
 
 template <int K>
-static void launch_score_K(bool pad, bool rev, bool exact, const ScoreParams& p, cudaStream_t st) {
+static void launch_score_K(bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
     const uint32_t ntasks = p.task_end - p.task_begin;
     if (ntasks == 0) return;
     const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
-    if (!exact) {                                         // general scoring: the padded variant serves every length
-        if (rev) score_kernel<K, true, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-        else     score_kernel<K, false, true, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-    } else if (rev) {
-        if (pad) score_kernel<K, true, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-        else     score_kernel<K, true, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+#define SDP_LAUNCH(R, P_, I) score_kernel<K, R, P_, I><<<grid, SDP_SCORE_THREADS, 0, st>>>(p)
+    if (p.c.imm) {
+        if (rev) { if (pad) SDP_LAUNCH(true, true, true); else SDP_LAUNCH(true, false, true); }
+        else     { if (pad) SDP_LAUNCH(false, true, true); else SDP_LAUNCH(false, false, true); }
     } else {
-        if (pad) score_kernel<K, false, true, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
-        else     score_kernel<K, false, false, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p);
+        if (rev) { if (pad) SDP_LAUNCH(true, true, false); else SDP_LAUNCH(true, false, false); }
+        else     { if (pad) SDP_LAUNCH(false, true, false); else SDP_LAUNCH(false, false, false); }
     }
+#undef SDP_LAUNCH
 }
 
 }  // namespace sdp

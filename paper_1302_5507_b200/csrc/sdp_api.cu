@@ -67,7 +67,8 @@ struct sdp_ctx {
     ScoreConsts consts{};
     TraceConsts tconsts{};
     int wide_ok = 0;                 // scoring fits the x8 tagged domain of the traceback DP kernel
-    int no_thin = 0;                 // SDP_NO_THIN=1: keep W >= 1 pairs off the narrow-band kernel (debugging)
+    int wide_fits = 0;               // wide_ok before sdp_set_debug_route masked it
+    int no_thin = 0;                 // sdp_set_debug_route: keep W >= 1 pairs off the narrow-band kernel
     char err[512] = {0};
     bool timing = false;
     bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
@@ -163,11 +164,9 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
 static const double kStepCostExact[SDP_MAX_K] = {6.7, 8.4, 10.0, 12.1, 13.8, 15.7, 17.5, 19.5, 21.1, 23.4, 25.0, 27.0, 29.4, 31.3, 33.8, 34.5, 36.2, 40.1, 41.0, 44.0, 48.3, 45.9, 47.7, 49.1, 50.5, 56.6, 58.4, 60.4, 61.4, 65.5, 70.1, 67.6};
 static const double kStepCostPadded[SDP_MAX_K] = {7.5, 9.2, 11.0, 12.8, 14.7, 16.5, 18.4, 20.0, 22.1, 23.8, 26.4, 27.1, 30.3, 31.2, 33.8, 36.0, 39.4, 43.3, 41.6, 43.2, 45.4, 49.4, 49.2, 50.4, 53.4, 57.5, 60.4, 59.2, 65.3, 66.0, 64.7, 66.7};
 
-void choose_geometry(sdp_ctx* c) {
+void choose_geometry(sdp_ctx* c, int force_g) {      // force_g: sdp_set_debug_route (geometry experiments), 0 = off
     struct Ent { uint16_t n, G, K, pad; };
     Ent ents[SDP_NSLOTS];
-    int force_g = 0;                                  // SDP_FORCE_G: tuning experiments only
-    if (const char* v = getenv("SDP_FORCE_G")) force_g = atoi(v);
     for (int n = 1; n <= SDP_NSLOTS; ++n) {
         double best = -1; int bG = 32, bK = (n + 31) / 32;
         for (int G = 1; G <= 32; ++G) {
@@ -212,8 +211,11 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     if (s->match < 0 || s->mismatch > 0 || s->match - s->mismatch <= 0 || s->gap_open < 0 || s->gap_extend < 1 ||
         !(s->min_similarity >= 0.0 && s->min_similarity <= 1.0))
         return SDP_EINVAL;
-    // the fp16 selector needs 2e + match to stay a denormal bit pattern; beta = 3o + 8 must fit too
-    if (2 * (long long)s->gap_extend + s->match > 1000 || s->gap_open > 2000 || s->mismatch < -4000) return SDP_EINVAL;
+    // limits of the int16 kernels (documented at sdp_scoring in sdp.h): match - mismatch must read as an fp16 value
+    // below 1.0 (bit pattern < 0x3C00), and no constant may come near the 16-bit range by itself
+    if (s->match > SDP_MAX_SCORE_PARAM || s->mismatch < -SDP_MAX_SCORE_PARAM || s->gap_open > SDP_MAX_SCORE_PARAM ||
+        s->gap_extend > SDP_MAX_SCORE_PARAM)
+        return SDP_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return SDP_ECUDA;
     sdp_ctx* ctx = new (std::nothrow) sdp_ctx();
@@ -221,17 +223,20 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     ctx->device = cuda_device;
     ctx->user_sc = *s;
     ctx->sc = Scoring{s->match, s->mismatch, s->gap_open, s->gap_extend, llround(s->min_similarity * 1e6)};
-    const int o = s->gap_open, e = s->gap_extend, beta = 3 * o + 8;
-    ctx->consts.exact = (2 * e + s->mismatch >= 0) ? 1u : 0u;
-    if (const char* v = getenv("SDP_NO_EXACT")) { if (atoi(v)) ctx->consts.exact = 0u; }
-    ctx->consts.negO = sdp_pack2(-o);
-    ctx->consts.cmis = sdp_pack2(2 * e + s->mismatch);
-    ctx->consts.Cf = sdp_pack2(2 * e + s->match);
-    ctx->consts.Cd = sdp_pack2(s->match - s->mismatch);
-    ctx->consts.e2 = sdp_pack2(e);
-    ctx->consts.beta2 = sdp_pack2(beta);
-    ctx->consts.betaMinusO2 = sdp_pack2(beta - o);
-    ctx->consts.o = o; ctx->consts.e = e; ctx->consts.beta = beta; ctx->consts.match = s->match;
+    const int o = s->gap_open, e = s->gap_extend, beta = 3 * o + 8;      // beta: traceback DP kernel
+    {   // score kernel (score_kernel.cuh): c = 2e + mismatch; F~ = F' - c starts at 0 = "minus infinity", which needs
+        // beta >= 2o + c
+        const int c = 2 * e + s->mismatch, beta_s = 3 * o + 8 + (c > 0 ? c : 0);
+        ctx->consts.negOc = sdp_pack2(-(o + c));
+        ctx->consts.negO = sdp_pack2(-o);
+        ctx->consts.c2 = sdp_pack2(c);
+        ctx->consts.Cd = sdp_pack2(s->match - s->mismatch);
+        ctx->consts.e2 = sdp_pack2(e);
+        ctx->consts.beta2 = sdp_pack2(beta_s);
+        ctx->consts.betaMinusO2 = sdp_pack2(beta_s - o);
+        ctx->consts.o = o; ctx->consts.e = e; ctx->consts.beta = beta_s; ctx->consts.match = s->match;
+        ctx->consts.imm = (s->match == 1 && s->mismatch == -3 && o == 5 && e == 2) ? 1u : 0u;
+    }
     {   // traceback DP kernel: x8 scaled values with tags in the low three bits (trace_kernel.cuh)
         const int sc8 = SDP_TB_SCALE;
         const int qm = sc8 * (2 * e + s->match) + 7, qx = sc8 * (2 * e + s->mismatch) + 7;
@@ -248,10 +253,9 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         // the diagonal increment is added with a 32-bit IMAD: it must be non-negative in both lanes,
         // and the match increment must stay an fp16 denormal bit pattern
         ctx->wide_ok = (qx >= 0 && qm < 2048 && sc8 * beta <= 32000) ? 1 : 0;
-        if (const char* v = getenv("SDP_NO_THIN")) ctx->no_thin = atoi(v);
-        if (const char* v = getenv("SDP_NO_WIDE")) { if (atoi(v)) ctx->wide_ok = 0; }
+        ctx->wide_fits = ctx->wide_ok;
     }
-    choose_geometry(ctx);
+    choose_geometry(ctx, 0);
 
     auto init = [&]() -> int {
         CU(cudaSetDevice(cuda_device));
@@ -337,6 +341,23 @@ int sdp_set_timing(sdp_ctx* ctx, int enabled)
 {
     if (!ctx) return SDP_EINVAL;
     ctx->timing = enabled != 0;
+    return SDP_OK;
+}
+
+int sdp_set_debug_route(sdp_ctx* ctx, uint32_t flags)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    const int force_g = (int)((flags >> 8) & 0x3Fu);
+    if ((flags & ~(SDP_ROUTE_NO_THIN | SDP_ROUTE_NO_WIDE | 0x3F00u)) || force_g > 32) return fail(ctx, SDP_EINVAL, "unknown route flags");
+    ctx->no_thin = (flags & SDP_ROUTE_NO_THIN) ? 1 : 0;
+    ctx->wide_ok = (flags & SDP_ROUTE_NO_WIDE) ? 0 : ctx->wide_fits;
+    choose_geometry(ctx, force_g);
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaMemcpy(ctx->d_slot_n, ctx->h_slot_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_slot_G, ctx->h_slot_G, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_slot_K, ctx->h_slot_K, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_slot_of_n, ctx->h_slot_of_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
     return SDP_OK;
 }
 

@@ -44,16 +44,16 @@ struct SlotInfo {
     uint16_t K;        // columns per thread; G*K - n in [0, G)
 };
 
-struct ScoreConsts {
-    uint32_t exact;    // 2e + mismatch >= 0: the exact-delta (four-instruction) score kernels apply
-    uint32_t negO;     // packed (-o, -o)
-    uint32_t cmis;     // packed (2e + mismatch)
-    uint32_t Cf;       // packed fp16 bit pattern == integer (2e + match), a denormal
-    uint32_t Cd;       // packed fp16 bit pattern == integer (match - mismatch), a denormal
-    uint32_t e2;       // packed (e, e)
-    uint32_t beta2;    // packed (beta, beta)
+struct ScoreConsts {           // packed int16x2 unless noted; c = 2e + mismatch (score_kernel.cuh)
+    uint32_t negOc;    // -(o + c)
+    uint32_t negO;     // -o
+    uint32_t c2;       // c
+    uint32_t Cd;       // fp16 bit pattern == integer (match - mismatch), a denormal
+    uint32_t e2;       // e
+    uint32_t beta2;    // beta
     uint32_t betaMinusO2;
-    int32_t  o, e, beta, match;
+    int32_t  o, e, beta, match;    // scalars
+    uint32_t imm;      // the scoring equals the compiled-in SDP_IMM_* values: the immediate-operand kernels apply
 };
 
 struct ScoreParams {
@@ -96,6 +96,6 @@ struct TraceDP {
 };
 
 // packed helpers
-__host__ __device__ static inline uint32_t sdp_pack2(int v) {
+__host__ __device__ constexpr static inline uint32_t sdp_pack2(int v) {
     return ((uint32_t)(uint16_t)(int16_t)v) | (((uint32_t)(uint16_t)(int16_t)v) << 16);
 }

@@ -102,9 +102,9 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         F[k] = 0x00020002u;                               // D(0,j) = -inf, carrying the "extended" tag
     }
 
-    const RingGeom rg = ring_geometry(G, ngroups);
+    const RingGeom rg = ring_geometry(G, ngroups, 1);
     uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
-    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + 32 - g;
+    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - g;
 
     const bool st_ok = hasA;                              // hasB implies hasA
     constexpr uint32_t rowstride = 32u * NW;              // word (step, w, lane): a warp-wide store is one 128-byte line

@@ -172,7 +172,7 @@ def test_extreme_shapes(ctx):
         return "".join(seq)
 
     wins, reads = [], []
-    for m in (7000, 7500, 7800):
+    for m in (7800, 12000, 15800):
         for _ in range(4):
             T = rnd(m)
             s = rng.randrange(0, m - 100)
@@ -257,31 +257,30 @@ def test_other_scorings(sc):
         c.destroy()
 
 
-def test_general_score_kernel_with_default_scoring(monkeypatch):
-    # SDP_NO_EXACT=1 (read by sdp_create) sends the default scoring through the general five-instruction
-    # score kernels that scorings with 2*extend + mismatch < 0 use; results must not change
-    monkeypatch.setenv("SDP_NO_EXACT", "1")
+@pytest.mark.parametrize("route", [dict(no_thin=True), dict(no_wide=True), dict(no_thin=True, no_wide=True)],
+                         ids=["no_thin", "no_wide", "generic_only"])
+def test_alternative_traceback_paths(route):
+    # route the same pairs through the other traceback kernels (wide wavefront for every W >= 1; generic scalar band
+    # kernel instead of the wavefront; generic kernel for everything): all must agree with the oracle
     c = make_ctx(DEFAULT)
     try:
-        parity.check_batch(c, W.make_config(2, n_pairs=1500, ref_bases=500_000), DEFAULT, "general kernels cfg2",
-                           host_path=False)
-        parity.check_batch(c, W.make_config(5, n_pairs=3000, ref_bases=500_000), DEFAULT, "general kernels cfg5",
-                           host_path=False)
+        c.set_debug_route(**route)
+        parity.check_batch(c, W.make_config(3, n_pairs=1200, ref_bases=500_000), DEFAULT, f"cfg3 {route}", host_path=False)
+        parity.check_batch(c, W.make_config(5, n_pairs=1500, ref_bases=500_000), DEFAULT, f"cfg5 {route}", host_path=False)
+        c.set_debug_route()                                   # back to the default routing
+        parity.check_batch(c, W.make_config(5, n_pairs=700, ref_bases=500_000), DEFAULT, "cfg5 default route", host_path=False)
     finally:
         c.destroy()
 
 
-@pytest.mark.parametrize("env", [{"SDP_NO_THIN": "1"}, {"SDP_NO_WIDE": "1"}, {"SDP_NO_THIN": "1", "SDP_NO_WIDE": "1"}],
-                         ids=["no_thin", "no_wide", "generic_only"])
-def test_alternative_traceback_paths(monkeypatch, env):
-    # route the same pairs through the other traceback kernels (wide wavefront for every W >= 1; generic scalar band
-    # kernel instead of the wavefront; generic kernel for everything): all must agree with the oracle
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+@pytest.mark.parametrize("g", [1, 2, 3, 5, 8, 16, 32])
+def test_forced_group_sizes(g):
+    # every thread-group size G the geometry table can pick, forced for all read lengths that admit it
     c = make_ctx(DEFAULT)
     try:
-        parity.check_batch(c, W.make_config(3, n_pairs=1200, ref_bases=500_000), DEFAULT, f"cfg3 {env}", host_path=False)
-        parity.check_batch(c, W.make_config(5, n_pairs=1500, ref_bases=500_000), DEFAULT, f"cfg5 {env}", host_path=False)
+        c.set_debug_route(force_g=g)
+        parity.check_batch(c, W.make_config(5, n_pairs=2500, ref_bases=500_000), DEFAULT, f"cfg5 G={g}", host_path=False)
+        parity.check_batch(c, W.make_config(1, n_pairs=300, ref_bases=200_000), DEFAULT, f"cfg1 G={g}", host_path=False)
     finally:
         c.destroy()
 
@@ -331,8 +330,8 @@ def test_errors(ctx):
     with pytest.raises(SdpError) as e:
         ctx.align_batch(ctx.upload(bad))
     assert e.value.code == -1
-    # int16 range rule: 1*100 + 2*(100 + 9000) > 16000
-    long_win = "ACGT" * 2250
+    # int16 range rule: 1*100 + 2*(100 + 17000 + 32) > 32000
+    long_win = "ACGT" * 4250
     rb = W.batch_from_strings([long_win], ["ACGT" * 25])
     with pytest.raises(SdpError) as e:
         ctx.align_batch(ctx.upload(rb))
