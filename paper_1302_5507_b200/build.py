@@ -2,7 +2,10 @@
 
 ``python -m paper_1302_5507_b200.build`` or ``build()`` from ``__graft_entry__``. Objects are
 compiled in parallel; the score and traceback-DP kernels are instantiated for 32 column counts x
-{forward, reverse, traceback} x {exact, padded}, split over sixteen translation units by ``-DSDP_K_LO/-DSDP_K_HI``.
+{forward, reverse, traceback} x {exact, padded}, split over sixteen K ranges by ``-DSDP_K_LO/-DSDP_K_HI``.
+The score kernels (``score_cubin.cu``) are compiled to cubins whose scoring constants are sentinel immediates;
+the cubins are embedded in the library as data (``.incbin``) and patched per context at load time
+(``score_modules.cu``). The build checks that every sentinel sits only where the loader looks for it.
 """
 from __future__ import annotations
 
@@ -41,14 +44,46 @@ def _deps_hash(extra: str) -> str:
     return h.hexdigest()
 
 
+SENTINELS = {"negOc": 0x5D1A37C2, "negO": 0x2B6E4A91, "c2": 0x63C5195D, "Cd": 0x39E2746B, "e2": 0x1F83528E}   # score_kernel.cuh
+
+
 def _units():
     units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []), ("thin_kernel", "thin_kernel.cu", []),
-             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("mate", "mate.cu", [])]
+             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("mate", "mate.cu", []),
+             ("score_modules", "score_modules.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"score_r{r}", "score_inst.cu",
-                      [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_K_FN=launch_score_r{r}",
-                       f"-DSDP_T_FN=launch_trace_r{r}"]))
+                      [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_T_FN=launch_trace_r{r}"]))
+        units.append((f"cubin_r{r}", "score_cubin.cu", [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}"]))
     return units
+
+
+def check_cubin_sentinels(path: str) -> dict:
+    """Every sentinel must occur in the cubin, and only as the 32-bit immediate of an instruction: bytes 4..7 of a
+    16-byte slot of an executable section. Returns the hit counts. (Same walk as patch_score_image in score_modules.cu.)"""
+    import struct
+    img = open(path, "rb").read()
+    assert img[:4] == b"\x7fELF" and img[4] == 2 and img[5] == 1, f"{path}: not a little-endian ELF64"
+    shoff, = struct.unpack_from("<Q", img, 0x28)
+    shentsize, shnum = struct.unpack_from("<HH", img, 0x3A)
+    assert shentsize == 64
+    hits = {k: 0 for k in SENTINELS}
+    by_val = {v: k for k, v in SENTINELS.items()}
+    for s in range(shnum):
+        _, typ, flags, _, off, size = struct.unpack_from("<IIQQQQ", img, shoff + 64 * s)
+        if typ != 1 or not (flags & 4):
+            continue
+        assert off % 16 == 0
+        for at in range(off, off + size - 15, 16):
+            w, = struct.unpack_from("<I", img, at + 4)
+            if w in by_val:
+                hits[by_val[w]] += 1
+    for name, v in SENTINELS.items():
+        total = img.count(struct.pack("<I", v))
+        if hits[name] == 0 or total != hits[name]:
+            raise RuntimeError(f"{path}: sentinel {name} found {total} times in the file but {hits[name]} times as an "
+                               "instruction immediate: the immediate patching of score_modules.cu would miss a use")
+    return hits
 
 
 def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -> str:
@@ -62,7 +97,13 @@ def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -
     def compile_one(unit):
         name, src, defs = unit
         obj = os.path.join(OBJ, name + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
+        if name.startswith("cubin_"):
+            # device code only -> cubin -> checked -> wrapped into an object file as read-only data
+            cubin = os.path.join(OBJ, name + ".cubin")
+            flags = [f for f in NVCC_FLAGS if f not in ("-Xcompiler", "-fPIC")]
+            cmd = [nvcc, *flags, *defs, "-cubin", os.path.join(CSRC, src), "-o", cubin]
+        else:
+            cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {name}:\n{r.stdout}\n{r.stderr}")
@@ -70,6 +111,16 @@ def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -
             f.write(r.stderr)
         if verbose:
             sys.stderr.write(r.stderr)
+        if name.startswith("cubin_"):
+            check_cubin_sentinels(cubin)
+            sym = "sdp_" + name                       # sdp_cubin_r<r>_start / _end
+            asm = os.path.join(OBJ, name + ".S")
+            with open(asm, "w") as f:
+                f.write(f'.section .rodata\n.balign 64\n.global {sym}_start\n.global {sym}_end\n{sym}_start:\n'
+                        f'.incbin "{cubin}"\n{sym}_end:\n.section .note.GNU-stack,"",@progbits\n')
+            r2 = subprocess.run(["gcc", "-c", "-fPIC", asm, "-o", obj], capture_output=True, text=True)
+            if r2.returncode != 0:
+                raise RuntimeError(f"embedding {cubin} failed:\n{r2.stderr}")
         return obj
 
     jobs = jobs or min(12, (os.cpu_count() or 4))

@@ -261,19 +261,23 @@ __device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingG
 #define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)
 #endif
 
-// IMM: the scoring constants are the compile-time values SDP_IMM_* (instruction immediates) instead of registers.
-// Each VIADDMNMX then reads two registers instead of three, which matters because the register file delivers one
-// operand per bank per cycle to BOTH pipes: with three-register DPX instructions the fp16 instructions of the
-// FMA pipe no longer fit beside them (measured: 10.1 against 9.0 cycles per column for the same instruction mix).
-#define SDP_IMM_MATCH 1
-#define SDP_IMM_MISMATCH (-3)
-#define SDP_IMM_OPEN 5
-#define SDP_IMM_EXTEND 2
-template <int K, bool REV, bool PAD, bool IMM>
-__global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))
-score_kernel(const ScoreParams P)
+// The scoring constants of the column loop are INSTRUCTION IMMEDIATES, not registers. Each VIADDMNMX then reads two
+// registers instead of three, which matters because the register file delivers one operand per bank per cycle to
+// BOTH pipes: with three-register DPX instructions the fp16 instructions of the FMA pipe no longer fit beside them
+// (measured on B200: 10.1 against 9.0 cycles per column for the same instruction mix; the forward pass of config 2
+// went from 7.4 to 6.7 ms). The scoring is a run-time argument of sdp_create, so the kernels are compiled to a cubin
+// with the SENTINEL values below as immediates, and score_modules.cu rewrites those immediates in a copy of the
+// cubin with the context's scoring before loading it. Sentinels are arbitrary
+// 32-bit patterns (both halves finite fp16 values) that occur nowhere else in the code.
+#define SDP_SENT_NEGOC 0x5D1A37C2u      // packed -(o + c)
+#define SDP_SENT_NEGO  0x2B6E4A91u      // packed -o
+#define SDP_SENT_C2    0x63C5195Du      // packed c = 2e + mismatch
+#define SDP_SENT_CD    0x39E2746Bu      // packed match - mismatch (bit pattern of an fp16 pair)
+#define SDP_SENT_E2    0x1F83528Eu      // packed e
+
+template <int K, bool REV, bool PAD>
+__device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring_mem)[SDP_RING_WORDS])
 {
-    __shared__ uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];
     const int lane = threadIdx.x & 31;
     const uint32_t task = P.task_begin + blockIdx.x * SDP_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (task >= P.task_end) return;                       // warp-uniform
@@ -343,10 +347,7 @@ score_kernel(const ScoreParams P)
         if (in_group) fill_ring_rows<REV>(P, rg, ring_w, g, G, s0, dA.woff, mA, dB.woff, mB);
     };
 
-    constexpr int IMM_C = 2 * SDP_IMM_EXTEND + SDP_IMM_MISMATCH;
-    const uint32_t negOc = IMM ? sdp_pack2(-(SDP_IMM_OPEN + IMM_C)) : P.c.negOc, negO = IMM ? sdp_pack2(-SDP_IMM_OPEN) : P.c.negO;
-    const uint32_t c2 = IMM ? sdp_pack2(IMM_C) : P.c.c2, Cd = IMM ? sdp_pack2(SDP_IMM_MATCH - SDP_IMM_MISMATCH) : P.c.Cd;
-    const uint32_t e2 = IMM ? sdp_pack2(SDP_IMM_EXTEND) : P.c.e2;
+    constexpr uint32_t negOc = SDP_SENT_NEGOC, negO = SDP_SENT_NEGO, c2 = SDP_SENT_C2, Cd = SDP_SENT_CD, e2 = SDP_SENT_E2;
     // 1 for every thread but the group's first: hin * notfirst + fv is a select on the FMA pipe (kept opaque so
     // that it stays a multiplier instead of becoming a predicate and an ALU-pipe SEL)
     const uint32_t notfirst = opaque_u32(is_first ? 0u : 1u);
@@ -535,22 +536,6 @@ score_kernel(const ScoreParams P)
             if (hasB) { P.score[dB.pid] = sB; P.ref_end[dB.pid] = idxB - 1; }
         }
     }
-}
-
-template <int K>
-static void launch_score_K(bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
-    const uint32_t ntasks = p.task_end - p.task_begin;
-    if (ntasks == 0) return;
-    const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
-#define SDP_LAUNCH(R, P_, I) score_kernel<K, R, P_, I><<<grid, SDP_SCORE_THREADS, 0, st>>>(p)
-    if (p.c.imm) {
-        if (rev) { if (pad) SDP_LAUNCH(true, true, true); else SDP_LAUNCH(true, false, true); }
-        else     { if (pad) SDP_LAUNCH(false, true, true); else SDP_LAUNCH(false, false, true); }
-    } else {
-        if (rev) { if (pad) SDP_LAUNCH(true, true, false); else SDP_LAUNCH(true, false, false); }
-        else     { if (pad) SDP_LAUNCH(false, true, false); else SDP_LAUNCH(false, false, false); }
-    }
-#undef SDP_LAUNCH
 }
 
 }  // namespace sdp

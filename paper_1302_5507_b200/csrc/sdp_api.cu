@@ -19,14 +19,6 @@ using namespace sdp;
 
 namespace sdp {
 #define SDP_SCORE_UNITS(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15)
-#define SDP_DECL(r) bool launch_score_r##r(int, bool, bool, const ScoreParams&, cudaStream_t);
-SDP_SCORE_UNITS(SDP_DECL)
-#undef SDP_DECL
-void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t st) {
-#define SDP_TRY(r) if (launch_score_r##r(K, pad, rev, p, st)) return;
-    SDP_SCORE_UNITS(SDP_TRY)
-#undef SDP_TRY
-}
 #define SDP_DECL(r) bool launch_trace_r##r(int, bool, const ScoreParams&, const TraceDP&, cudaStream_t);
 SDP_SCORE_UNITS(SDP_DECL)
 #undef SDP_DECL
@@ -66,6 +58,8 @@ struct sdp_ctx {
     Scoring sc{};
     ScoreConsts consts{};
     TraceConsts tconsts{};
+    ScorePatch patch{};              // the scoring as the score kernels' immediates (score_modules.cu)
+    ScoreModules modules;            // score kernels loaded so far, patched with `patch`
     int wide_ok = 0;                 // scoring fits the x8 tagged domain of the traceback DP kernel
     int wide_fits = 0;               // wide_ok before sdp_set_debug_route masked it
     int no_thin = 0;                 // sdp_set_debug_route: keep W >= 1 pairs off the narrow-band kernel
@@ -227,15 +221,11 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     {   // score kernel (score_kernel.cuh): c = 2e + mismatch; F~ = F' - c starts at 0 = "minus infinity", which needs
         // beta >= 2o + c
         const int c = 2 * e + s->mismatch, beta_s = 3 * o + 8 + (c > 0 ? c : 0);
-        ctx->consts.negOc = sdp_pack2(-(o + c));
-        ctx->consts.negO = sdp_pack2(-o);
-        ctx->consts.c2 = sdp_pack2(c);
-        ctx->consts.Cd = sdp_pack2(s->match - s->mismatch);
-        ctx->consts.e2 = sdp_pack2(e);
+        ctx->patch = ScorePatch{sdp_pack2(-(o + c)), sdp_pack2(-o), sdp_pack2(c), sdp_pack2(s->match - s->mismatch), sdp_pack2(e)};
+        score_modules_init(&ctx->modules);
         ctx->consts.beta2 = sdp_pack2(beta_s);
         ctx->consts.betaMinusO2 = sdp_pack2(beta_s - o);
-        ctx->consts.o = o; ctx->consts.e = e; ctx->consts.beta = beta_s; ctx->consts.match = s->match;
-        ctx->consts.imm = (s->match == 1 && s->mismatch == -3 && o == 5 && e == 2) ? 1u : 0u;
+        ctx->consts.e = e; ctx->consts.beta = beta_s;
     }
     {   // traceback DP kernel: x8 scaled values with tags in the low three bits (trace_kernel.cuh)
         const int sc8 = SDP_TB_SCALE;
@@ -305,6 +295,7 @@ void sdp_destroy(sdp_ctx* ctx)
 {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    score_modules_destroy(&ctx->modules);
     DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->order_rev, &ctx->desc_rev,
                       &ctx->order_tb, &ctx->keys_rev, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
                       &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local[0], &ctx->scan_local[1], &ctx->scan_local[2],
@@ -428,7 +419,11 @@ static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const
         cudaStream_t ls = (fan && (turn % SDP_FAN_STREAMS)) ? ctx->fan_stream[turn % SDP_FAN_STREAMS] : st;
         ++turn;
         if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, ls);
-        else launch_score(cls >> 1, (cls & 1) != 0, rev, sp, ls);
+        else {
+            const int rc = score_modules_launch(&ctx->modules, ctx->patch, cls >> 1, (cls & 1) != 0, rev, sp, ls, ctx->err,
+                                                sizeof(ctx->err));
+            if (rc != SDP_OK) return rc;
+        }
         ++*nlaunch;
     }
     if (fan) {

@@ -26,8 +26,22 @@ void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint6
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
                             cudaStream_t st, uint32_t* launches);
 
-// ---- score_inst.cu (compiled once per K range)
-void launch_score(int K, bool pad, bool rev, const ScoreParams& p, cudaStream_t st);
+// ---- score_modules.cu: the score kernels, loaded per context with the scoring patched into their immediates
+constexpr int SDP_SCORE_UNITS_N = 16;     // cubins, two column counts each (K = 2r+1, 2r+2)
+constexpr int SDP_N_SENTINELS = 5;
+struct ScorePatch { uint32_t negOc, negO, c2, Cd, e2; };       // packed int16x2 values, see score_kernel.cuh
+struct ScoreModules {
+    cudaLibrary_t lib[SDP_SCORE_UNITS_N];
+    unsigned char loaded[SDP_SCORE_UNITS_N];
+    cudaKernel_t kern[SDP_MAX_K + 1][2][2];                     // [K][reverse][padded]
+};
+void score_modules_init(ScoreModules* m);
+void score_modules_destroy(ScoreModules* m);
+bool patch_score_image(unsigned char* img, size_t len, const ScorePatch& pv, uint32_t hits[SDP_N_SENTINELS]);
+int score_modules_launch(ScoreModules* m, const ScorePatch& pv, int K, bool pad, bool rev, const ScoreParams& p,
+                         cudaStream_t st, char* err, size_t errlen);
+
+// ---- score_inst.cu (compiled once per K range): the traceback DP kernels
 void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st);
 
 // ---- traceback.cu

@@ -44,16 +44,11 @@ struct SlotInfo {
     uint16_t K;        // columns per thread; G*K - n in [0, G)
 };
 
-struct ScoreConsts {           // packed int16x2 unless noted; c = 2e + mismatch (score_kernel.cuh)
-    uint32_t negOc;    // -(o + c)
-    uint32_t negO;     // -o
-    uint32_t c2;       // c
-    uint32_t Cd;       // fp16 bit pattern == integer (match - mismatch), a denormal
-    uint32_t e2;       // e
-    uint32_t beta2;    // beta
-    uint32_t betaMinusO2;
-    int32_t  o, e, beta, match;    // scalars
-    uint32_t imm;      // the scoring equals the compiled-in SDP_IMM_* values: the immediate-operand kernels apply
+struct ScoreConsts {           // what the score kernels take as arguments; the constants of their column loop are
+                               // instruction immediates (ScorePatch in sdp_host.cuh, score_kernel.cuh)
+    uint32_t beta2;            // packed int16x2 beta
+    uint32_t betaMinusO2;      // packed beta - o
+    int32_t  e, beta;          // scalars
 };
 
 struct ScoreParams {
