@@ -119,9 +119,14 @@ def cpu_baseline(batch, budget_s: float = 15.0):
     rate = n / max(dt, 1e-6)
     want = int(max(n, min(batch.n_pairs, rate * budget_s)))
     dt, cells, used, n = oracle_timed(batch, want, threads)
+    # one thread on the first 20,000 pairs -> per-core figure (bounded to a few seconds)
+    n1 = int(min(20_000, batch.n_pairs, max(200, rate / max(used, 1) * 4.0)))
+    dt1, cells1, used1, n1 = oracle_timed(batch, n1, 1)
     return {"value": cells / dt / 1e9, "unit": UNIT, "cores": used, "kind": "oracle",
             "pairs_per_s": n / dt, "seconds": dt,
-            "sample": f"first {n} pairs of the workload, {used} OpenMP threads over disjoint pair ranges"}
+            "sample": f"first {n} pairs of the workload, {used} OpenMP threads over disjoint pair ranges",
+            "single_thread": {"value": cells1 / dt1 / 1e9, "unit": UNIT, "cores": used1, "pairs_per_s": n1 / dt1,
+                              "seconds": dt1, "sample": f"first {n1} pairs of the workload, one thread"}}
 
 
 def run_reference(args, rank):
@@ -133,7 +138,7 @@ def run_reference(args, rank):
     oracle.build()
     threads = os.cpu_count() or 1
     n_sample = args.ref_pairs
-    batch = W.make_config(args.config, n_pairs=max(n_sample, 1), ref_bases=min(args.ref_bases, 20_000_000))
+    batch = W.make_config(args.config, n_pairs=max(n_sample, 1), ref_bases=args.ref_bases if args.config != 1 else 1_000_000)
     for _ in range(args.warmup):
         oracle_timed(batch, min(n_sample, 2000), threads)
     times, cells, used = [], 0, threads
@@ -165,6 +170,49 @@ W_NAME = {
 }
 
 
+def time_config(S, W, torch, dev, local, cfg, n_pairs, ref_bases, seed, steps, warmup, flush, peak):
+    """One BASELINE.json config at full size on this GPU: device-resident timing of the whole sdp_align_batch call
+    (CUDA events on the launching stream, L2 flushed between steps), its own clocks sample, stage split."""
+    batch = W.make_config(cfg, n_pairs=n_pairs, ref_bases=ref_bases if cfg != 1 else 1_000_000, seed=seed)
+    ctx = S.Context(device=local)
+    try:
+        dbatch = ctx.upload(batch)
+        stream = torch.cuda.current_stream(dev)
+        ctx.set_timing(True)
+        for _ in range(warmup):
+            ctx.align_batch(dbatch, stream)
+        sampler = ClockSampler(local)
+        sampler.start()
+        torch.cuda.synchronize(dev)
+        t0 = time.time()
+        ms, fwd, stats = [], [], {}
+        for _ in range(steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            ctx.align_batch(dbatch, stream)
+            e1.record(stream)
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+            stats = ctx.stats()
+            fwd.append(stats["ms_forward"])
+        torch.cuda.synchronize(dev)
+        clocks = sampler.stop(t0, time.time())
+        mean = statistics.mean(ms)
+        fwd_gcups = batch.cells / (statistics.mean(fwd) * 1e-3) / 1e9
+        return {"workload": W_NAME[cfg], "pairs": batch.n_pairs, "cells": batch.cells, "steps": steps, "warmup": warmup,
+                "ms_per_step": mean, "ms_best": min(ms), "ms_median": statistics.median(ms),
+                "gcups": batch.cells / (mean * 1e-3) / 1e9, "pairs_per_s": batch.n_pairs / (mean * 1e-3),
+                "stages_ms": {k: stats.get(k) for k in ("ms_total", "ms_bucket", "ms_forward", "ms_reverse", "ms_traceback",
+                                                        "ms_compact")},
+                "kernel_launches_per_step": stats.get("kernel_launches"),
+                "forward_gcups": fwd_gcups, "forward_frac": fwd_gcups / peak,
+                "whole_path_frac": batch.cells / (mean * 1e-3) / 1e9 / peak, "clocks": clocks}
+    finally:
+        ctx.destroy()
+        del batch
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -176,6 +224,7 @@ def main():
     ap.add_argument("--ref-bases", type=int, default=100_000_000)
     ap.add_argument("--ref-pairs", type=int, default=20_000, help="--impl reference: pairs per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (configs 1, 3, 4, 5 at full size)")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -355,11 +404,14 @@ def main():
             traffic = json.load(f).get("dram_bytes_per_launch")
     except Exception:
         pass
-    roofline = {"bound": "alu", "kernel": "sdp::score_kernel<K, false> (forward score pass)",
+    roofline = {"bound": "alu", "kernel": "sdp_score_k<K>_f* (forward score pass, score_kernel.cuh)",
                 "achieved": fwd, "peak": peak, "unit": UNIT, "frac": (fwd / peak) if fwd else None,
                 "traffic": traffic,
                 "peak_how": f"{sms} SMs x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz) x {DPX_RATE:.0f} int16x2 DPX "
                             f"instr/clk/SM (measured, profiles/) x 2 cells / {INSTR_PER_2_CELLS:.0f} instr",
+                "traffic_how": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this kernel on "
+                               "this workload, stored in profiles/forward_traffic.json (a profiled constant, not re-measured "
+                               "by this run)",
                 "achieved_how": "sum n*m of the batch / mean CUDA-event time of the forward-kernel launches per step, "
                                 "events recorded by libsdp on the launching stream inside the timed steps",
                 "whole_path_frac": value / world / peak, "dpx_rate_measured_now": dpx_live}
@@ -374,6 +426,7 @@ def main():
                    "parallelism": f"independent pair shards x{world} (no collective)",
                    "l2": "256 MiB buffer written between timed steps (L2 flush)",
                    "outputs": "score, ref_start, ref_end, read span, CIGAR, n_match, n_cols, pass for every pair"},
+        "ms_best": min(step_ms) if step_ms else None, "ms_median": statistics.median(step_ms) if step_ms else None,
         "stages_ms": {k: stats.get(k) for k in ("ms_total", "ms_bucket", "ms_forward", "ms_reverse", "ms_traceback",
                                                 "ms_compact")},
         "roofline": roofline, "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
@@ -388,6 +441,18 @@ def main():
         import oracle
         oracle.build()
         out["cpu_baseline"] = cpu_baseline(batch)
+    if not args.no_per_config and world == 1 and cfg == 2 and args.pairs is None:
+        # the other BASELINE.json configs at full size, AFTER every headline number was taken (they cannot disturb it)
+        ctx.destroy()
+        del dbatch, batch
+        per = {}
+        for c in (1, 3, 4, 5):
+            try:
+                per[f"cfg{c}"] = time_config(S, W, torch, dev, local, c, None, args.ref_bases, W.SEED_BASE + c,
+                                             steps=3, warmup=2, flush=flush, peak=peak)
+            except Exception as ex:  # noqa: BLE001
+                per[f"cfg{c}"] = {"error": repr(ex)}
+        out["per_config"] = per
     print(json.dumps(out))
 
 

@@ -20,7 +20,8 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force enumeration of every alignment for
  * n, m <= 6; closed forms; re-scoring of the emitted CIGAR; infix edit distance special case
- * against an independently written Levenshtein DP; worked examples in tests/golden/.
+ * against an independently written Levenshtein DP; worked examples in tests/golden/. The local
+ * variant (oracle_align_pair_local) has its own pins in tests/test_oracle_local.py.
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -145,6 +146,90 @@ int oracle_align_pair(const uint8_t* T, int m, const uint8_t* R, int n,
     return 0;
 }
 
+/*
+ * LOCAL (soft-clipping) variant, SURVEY.md 8(f2). The paper names the algorithm "Smith-Waterman" and
+ * speaks of soft-clipped alignments (Figure 2 legend) although its recurrences are the semi-global ones
+ * above; this function is the textbook Smith-Waterman with the paper's affine gap model (reading R18):
+ *     M(i,0) = M(0,j) = 0;  I, D = -inf on the borders
+ *     I, D as in PAPER.md:289-291;  M(i,j) = max(0, M(i-1,j-1) + delta, I(i,j), D(i,j))
+ *     S = max over 1 <= i <= m, 1 <= j <= n of M(i,j); ties: lowest i, then lowest j.
+ * Traceback from that cell with the rules of R6, stopping at the first cell with M(i,j) == 0 (tested before the
+ * diagonal). read_start / read_end are the first / last aligned read base; unaligned read ends are soft clips and
+ * appear in the CIGAR as BAM op 4 ('S'). n_cols counts aligned columns only. S == 0 means no alignment:
+ * ref_start = 0, ref_end = -1, read_start = 0, read_end = -1, an all-'S' CIGAR, pass = 0.
+ * Filter (R18): soft-clipped read bases count as columns that do not match:
+ *     pass = n_cols > 0 and n_match * 1e6 >= q * (n_cols + clipped bases).
+ */
+int oracle_align_pair_local(const uint8_t* T, int m, const uint8_t* R, int n,
+                            const oracle_scoring* sc, oracle_result* res, uint32_t* ops_out)
+{
+    const int o = sc->gap_open, e = sc->gap_extend;
+    const size_t W = (size_t)n + 1;
+    int32_t* H = (int32_t*)malloc(sizeof(int32_t) * (size_t)(m + 1) * W);
+    int32_t* I = (int32_t*)malloc(sizeof(int32_t) * (size_t)(m + 1) * W);
+    int32_t* D = (int32_t*)malloc(sizeof(int32_t) * (size_t)(m + 1) * W);
+    uint8_t* rev = (uint8_t*)malloc((size_t)n + (size_t)m + 2);
+    if (!H || !I || !D || !rev) { free(H); free(I); free(D); free(rev); return -1; }
+#define AT(X, i, j) X[(size_t)(i) * W + (size_t)(j)]
+    for (int i = 0; i <= m; ++i) { AT(H, i, 0) = 0; AT(I, i, 0) = NEG_INF; AT(D, i, 0) = NEG_INF; }
+    for (int j = 1; j <= n; ++j) { AT(H, 0, j) = 0; AT(I, 0, j) = NEG_INF; AT(D, 0, j) = NEG_INF; }
+    int best = 0, i_end = 0, j_end = 0;
+    for (int i = 1; i <= m; ++i) {
+        for (int j = 1; j <= n; ++j) {
+            int vi = max2(AT(H, i, j - 1) - (o + e), AT(I, i, j - 1) - e);
+            int vd = max2(AT(H, i - 1, j) - (o + e), AT(D, i - 1, j) - e);
+            int vm = AT(H, i - 1, j - 1) + delta(sc, T[i - 1], R[j - 1]);
+            AT(I, i, j) = vi;
+            AT(D, i, j) = vd;
+            AT(H, i, j) = max2(0, max2(vm, max2(vi, vd)));
+            if (AT(H, i, j) > best) { best = AT(H, i, j); i_end = i; j_end = j; }   /* row-major scan: lowest i, then lowest j */
+        }
+    }
+    int i = i_end, j = j_end, nrev = 0, n_match = 0;
+    enum { ST_H, ST_D, ST_I } st = ST_H;
+    while (best > 0) {
+        if (st == ST_H) {
+            if (AT(H, i, j) == 0) break;
+            if (AT(H, i, j) == AT(H, i - 1, j - 1) + delta(sc, T[i - 1], R[j - 1])) {
+                rev[nrev++] = 0;
+                if (T[i - 1] < CODE_N && R[j - 1] < CODE_N && T[i - 1] == R[j - 1]) ++n_match;
+                --i; --j;
+            } else if (AT(H, i, j) == AT(D, i, j)) {
+                st = ST_D;
+            } else {
+                st = ST_I;
+            }
+        } else if (st == ST_D) {
+            rev[nrev++] = 2;
+            if (AT(D, i, j) == AT(H, i - 1, j) - (o + e)) st = ST_H;
+            --i;
+        } else {
+            rev[nrev++] = 1;
+            if (AT(I, i, j) == AT(H, i, j - 1) - (o + e)) st = ST_H;
+            --j;
+        }
+    }
+    int nops = 0;
+    const int lead = (best > 0) ? j : n, trail = (best > 0) ? n - j_end : 0;
+    if (lead > 0) ops_out[nops++] = ((uint32_t)lead << 4) | 4u;
+    for (int k = nrev - 1; k >= 0; ) {
+        int op = rev[k], len = 0;
+        while (k >= 0 && rev[k] == op) { ++len; --k; }
+        ops_out[nops++] = ((uint32_t)len << 4) | (uint32_t)op;
+    }
+    if (trail > 0) ops_out[nops++] = ((uint32_t)trail << 4) | 4u;
+    res->score = best;
+    if (best > 0) { res->ref_start = i; res->ref_end = i_end - 1; res->read_start = j; res->read_end = j_end - 1; }
+    else          { res->ref_start = 0; res->ref_end = -1; res->read_start = 0; res->read_end = -1; }
+    res->n_match = n_match;
+    res->n_cols = nrev;
+    res->pass = (nrev > 0 && (int64_t)n_match * 1000000LL >= sc->min_sim_q * (int64_t)(nrev + lead + trail)) ? 1 : 0;
+    res->cigar_len = nops;
+#undef AT
+    free(H); free(I); free(D); free(rev);
+    return 0;
+}
+
 /* ---- batch interface over the same packed arrays the C-ABI library consumes ------------- */
 
 /* base k of a 2-bit packed buffer: bits 2*(k mod 16) (LSB first) of little-endian word k/16 */
@@ -168,10 +253,10 @@ typedef struct oracle_batch {
  * caller's arrays (length n_pairs each); CIGAR runs are kept inside the returned handle.
  * Returns NULL on allocation failure. *threads_used receives the thread count actually used.
  */
-oracle_batch* oracle_align_batch(
+oracle_batch* oracle_align_batch_mode(
     const uint32_t* reads_packed, const uint64_t* read_off, const uint32_t* read_len, const uint32_t* read_nmask,
     const uint32_t* wins_packed, const uint64_t* win_off, const uint32_t* win_len, const uint32_t* win_nmask,
-    const uint32_t* pairs, uint64_t n_pairs, const oracle_scoring* sc, int n_threads,
+    const uint32_t* pairs, uint64_t n_pairs, const oracle_scoring* sc, int n_threads, int local_mode,
     int32_t* score, int32_t* ref_start, int32_t* ref_end, int32_t* read_start, int32_t* read_end,
     uint8_t* pass, int32_t* n_match, int32_t* n_cols, uint64_t* cigar_off, uint32_t* cigar_len,
     int32_t* threads_used)
@@ -205,12 +290,13 @@ oracle_batch* oracle_align_batch(
                 int n = (int)read_len[ri], m = (int)win_len[wi];
                 if ((size_t)m > capT) { free(T); capT = (size_t)m * 2; T = (uint8_t*)malloc(capT); }
                 if ((size_t)n > capR) { free(R); capR = (size_t)n * 2; R = (uint8_t*)malloc(capR); }
-                if ((size_t)(n + m + 1) > capO) { free(ops); capO = (size_t)(n + m + 1) * 2; ops = (uint32_t*)malloc(capO * 4); }
+                if ((size_t)(n + m + 3) > capO) { free(ops); capO = (size_t)(n + m + 3) * 2; ops = (uint32_t*)malloc(capO * 4); }
                 if (!T || !R || !ops) { failed = 1; break; }
                 for (int k = 0; k < m; ++k) T[k] = get_base(wins_packed, win_nmask, win_off[wi] + (uint64_t)k);
                 for (int k = 0; k < n; ++k) R[k] = get_base(reads_packed, read_nmask, read_off[ri] + (uint64_t)k);
                 oracle_result r;
-                if (oracle_align_pair(T, m, R, n, sc, &r, ops, NULL) != 0) { failed = 1; break; }
+                if ((local_mode ? oracle_align_pair_local(T, m, R, n, sc, &r, ops)
+                                : oracle_align_pair(T, m, R, n, sc, &r, ops, NULL)) != 0) { failed = 1; break; }
                 score[p] = r.score; ref_start[p] = r.ref_start; ref_end[p] = r.ref_end;
                 read_start[p] = r.read_start; read_end[p] = r.read_end;
                 pass[p] = (uint8_t)r.pass; n_match[p] = r.n_match; n_cols[p] = r.n_cols;
@@ -242,6 +328,20 @@ oracle_batch* oracle_align_batch(
     free(vecs);
     if (failed) { if (b) free(b->ops); free(b); return NULL; }
     return b;
+}
+
+/* the semi-global path of the paper (every caller before the local variant existed) */
+oracle_batch* oracle_align_batch(
+    const uint32_t* reads_packed, const uint64_t* read_off, const uint32_t* read_len, const uint32_t* read_nmask,
+    const uint32_t* wins_packed, const uint64_t* win_off, const uint32_t* win_len, const uint32_t* win_nmask,
+    const uint32_t* pairs, uint64_t n_pairs, const oracle_scoring* sc, int n_threads,
+    int32_t* score, int32_t* ref_start, int32_t* ref_end, int32_t* read_start, int32_t* read_end,
+    uint8_t* pass, int32_t* n_match, int32_t* n_cols, uint64_t* cigar_off, uint32_t* cigar_len,
+    int32_t* threads_used)
+{
+    return oracle_align_batch_mode(reads_packed, read_off, read_len, read_nmask, wins_packed, win_off, win_len, win_nmask,
+                                   pairs, n_pairs, sc, n_threads, 0, score, ref_start, ref_end, read_start, read_end, pass,
+                                   n_match, n_cols, cigar_off, cigar_len, threads_used);
 }
 
 uint64_t oracle_batch_n_ops(const oracle_batch* b) { return b ? b->n_ops : 0; }

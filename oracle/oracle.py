@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 _lock = threading.Lock()
 _lib = None
 
-CIGAR_OPS = "MID"
+CIGAR_OPS = "MIDNS"            # BAM op codes 0..4; the local variant emits 4 = soft clip
 
 
 class _Scoring(ctypes.Structure):
@@ -69,10 +69,13 @@ def _load():
         lib.oracle_align_pair.restype = ctypes.c_int
         lib.oracle_align_pair.argtypes = [u8p, ctypes.c_int, u8p, ctypes.c_int,
                                           ctypes.POINTER(_Scoring), ctypes.POINTER(_Result), u32p, i32p]
-        lib.oracle_align_batch.restype = ctypes.c_void_p
-        lib.oracle_align_batch.argtypes = ([u32p, u64p, u32p, u32p] * 2 + [u32p, ctypes.c_uint64,
-                                           ctypes.POINTER(_Scoring), ctypes.c_int] +
-                                           [i32p] * 5 + [u8p, i32p, i32p, u64p, u32p, i32p])
+        lib.oracle_align_pair_local.restype = ctypes.c_int
+        lib.oracle_align_pair_local.argtypes = [u8p, ctypes.c_int, u8p, ctypes.c_int,
+                                                ctypes.POINTER(_Scoring), ctypes.POINTER(_Result), u32p]
+        lib.oracle_align_batch_mode.restype = ctypes.c_void_p
+        lib.oracle_align_batch_mode.argtypes = ([u32p, u64p, u32p, u32p] * 2 + [u32p, ctypes.c_uint64,
+                                                ctypes.POINTER(_Scoring), ctypes.c_int, ctypes.c_int] +
+                                                [i32p] * 5 + [u8p, i32p, i32p, u64p, u32p, i32p])
         lib.oracle_batch_n_ops.restype = ctypes.c_uint64
         lib.oracle_batch_n_ops.argtypes = [ctypes.c_void_p]
         lib.oracle_batch_fetch_ops.restype = None
@@ -101,24 +104,31 @@ def _codes(seq) -> np.ndarray:
     return np.ascontiguousarray(seq, dtype=np.uint8)
 
 
-def align_pair(window, read, scoring: OracleScoring = OracleScoring(), want_last_row: bool = False):
+def align_pair(window, read, scoring: OracleScoring = OracleScoring(), want_last_row: bool = False,
+               local: bool = False):
     """Align one read against one window. Sequences are strings over ACGTN or code arrays.
 
     Returns a dict with score, ref_start, ref_end, read_start, read_end, n_match, n_cols, pass,
     cigar (string), ops (uint32 runs) and, if asked, last_row = H(i, n) for i = 0..m.
+    ``local=True`` is the Smith-Waterman / soft-clipping variant (oracle_align_pair_local, R18).
     """
     lib = _load()
     T, R = _codes(window), _codes(read)
     m, n = len(T), len(R)
     if m < 1 or n < 1:
         raise ValueError("empty sequence")
-    ops = np.zeros(n + m + 1, dtype=np.uint32)
+    ops = np.zeros(n + m + 3, dtype=np.uint32)
     last = np.zeros(m + 1, dtype=np.int32) if want_last_row else None
     res = _Result()
     sc = scoring._c()
-    rc = lib.oracle_align_pair(_ptr(T, ctypes.c_uint8), m, _ptr(R, ctypes.c_uint8), n,
-                               ctypes.byref(sc), ctypes.byref(res), _ptr(ops, ctypes.c_uint32),
-                               _ptr(last, ctypes.c_int32))
+    if local:
+        assert not want_last_row
+        rc = lib.oracle_align_pair_local(_ptr(T, ctypes.c_uint8), m, _ptr(R, ctypes.c_uint8), n,
+                                         ctypes.byref(sc), ctypes.byref(res), _ptr(ops, ctypes.c_uint32))
+    else:
+        rc = lib.oracle_align_pair(_ptr(T, ctypes.c_uint8), m, _ptr(R, ctypes.c_uint8), n,
+                                   ctypes.byref(sc), ctypes.byref(res), _ptr(ops, ctypes.c_uint32),
+                                   _ptr(last, ctypes.c_int32))
     if rc != 0:
         raise MemoryError("oracle_align_pair")
     ops = ops[:res.cigar_len].copy()
@@ -153,7 +163,7 @@ class OracleBatchResult:
 
 def align_batch(reads_packed, read_off, read_len, wins_packed, win_off, win_len, pairs,
                 scoring: OracleScoring = OracleScoring(), read_nmask=None, win_nmask=None,
-                threads: int = 1) -> OracleBatchResult:
+                threads: int = 1, local: bool = False) -> OracleBatchResult:
     """Same inputs as ``sdp_align_batch`` (host numpy arrays). ``pairs`` is (P, 2) uint32."""
     lib = _load()
     reads_packed = np.ascontiguousarray(reads_packed, dtype=np.uint32)
@@ -177,10 +187,10 @@ def align_batch(reads_packed, read_off, read_len, wins_packed, win_off, win_len,
     used = ctypes.c_int32(0)
     sc = scoring._c()
     u32, u64, i32c, u8 = ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int32, ctypes.c_uint8
-    h = lib.oracle_align_batch(
+    h = lib.oracle_align_batch_mode(
         _ptr(reads_packed, u32), _ptr(read_off, u64), _ptr(read_len, u32), _ptr(read_nmask, u32),
         _ptr(wins_packed, u32), _ptr(win_off, u64), _ptr(win_len, u32), _ptr(win_nmask, u32),
-        _ptr(pairs, u32), P, ctypes.byref(sc), int(threads),
+        _ptr(pairs, u32), P, ctypes.byref(sc), int(threads), 1 if local else 0,
         _ptr(r.score, i32c), _ptr(r.ref_start, i32c), _ptr(r.ref_end, i32c), _ptr(r.read_start, i32c),
         _ptr(r.read_end, i32c), _ptr(r.passed, u8), _ptr(r.n_match, i32c), _ptr(r.n_cols, i32c),
         _ptr(r.cigar_off, u64), _ptr(r.cigar_len, u32), ctypes.byref(used))

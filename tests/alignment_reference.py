@@ -165,3 +165,119 @@ def infix_edit_distance(T: str, R: str) -> int:
             cur[i] = min(sub, prev[i] + 1, cur[i - 1] + 1)
         prev = cur
     return min(prev)               # free end anywhere (i = 0 allowed: costs n, never better than i >= 1 ... see test)
+
+
+# ---------------------------------------------------------------- local (soft-clipping) variant, R18
+def score_ops_from(T: str, R: str, i0: int, j0: int, ops: str, sc) -> int:
+    """Score of an op string that starts at window base i0 and read base j0 (affine: a maximal gap run of k costs o + k e)."""
+    match, mismatch, o, e = sc
+    i, j, s, k = i0, j0, 0, 0
+    while k < len(ops):
+        op = ops[k]
+        if op == "M":
+            s += delta(T[i], R[j], match, mismatch)
+            i += 1
+            j += 1
+            k += 1
+        else:
+            run = 0
+            while k < len(ops) and ops[k] == op:
+                run += 1
+                k += 1
+            s -= o + e * run
+            if op == "I":
+                j += run
+            else:
+                i += run
+    return s
+
+
+def enumerate_all_local(T: str, R: str, sc) -> Iterator[Tuple[int, int, int, int, str, int]]:
+    """Yield (i0, j0, i_end, j_end, ops, score) for every local alignment that starts and ends with an M column:
+    any window start, any read start, any end (an optimum with positive score never starts or ends in a gap when
+    open + extend > 0). True brute force, no dynamic programming."""
+    m, n = len(T), len(R)
+
+    def rec(i: int, j: int, ops: List[str]):
+        if ops and ops[-1] == "M":
+            yield i, j, "".join(ops)
+        if i < m and j < n:
+            ops.append("M")
+            yield from rec(i + 1, j + 1, ops)
+            ops.pop()
+        if ops and j < n:
+            ops.append("I")
+            yield from rec(i, j + 1, ops)
+            ops.pop()
+        if ops and i < m:
+            ops.append("D")
+            yield from rec(i + 1, j, ops)
+            ops.pop()
+
+    for i0 in range(m):
+        for j0 in range(n):
+            for ie, je, ops in rec(i0, j0, []):
+                if ops[0] == "M":
+                    yield i0, j0, ie, je, ops, score_ops_from(T, R, i0, j0, ops, sc)
+
+
+def canonical_local(T: str, R: str, sc):
+    """Brute-force expected result of the local variant: highest score; among the maximisers the lowest end row, then the
+    lowest end column; walking backwards from there stop as soon as what was walked is a maximiser by itself (the DP
+    cell reads 0), otherwise prefer M, then D, then I, and inside a gap prefer to close the run."""
+    assert sc[2] + sc[3] > 0 and sc[2] > 0
+    best, pool = 0, []
+    for i0, j0, ie, je, ops, s in enumerate_all_local(T, R, sc):
+        if s > best:
+            best, pool = s, [(i0, j0, ie, je, ops)]
+        elif s == best and s > 0:
+            pool.append((i0, j0, ie, je, ops))
+    n = len(R)
+    if best == 0:
+        return dict(score=0, ref_start=0, ref_end=-1, read_start=0, read_end=-1, cigar=f"{n}S", n_match=0, n_cols=0)
+    ie = min(p[2] for p in pool)
+    je = min(p[3] for p in pool if p[2] == ie)
+    cands = [p for p in pool if p[2] == ie and p[3] == je]
+    chosen: List[str] = []
+    state = "H"
+    while True:
+        done = [c for c in cands if len(c[4]) == len(chosen)]
+        if done and state == "H":
+            final = done[0]
+            break
+        k = len(chosen) + 1
+        alive = [c for c in cands if len(c[4]) >= k]
+        avail = {c[4][-k] for c in alive}
+        order = ["M", "I", "D"] if state == "D" else ["M", "D", "I"]
+        op = next(x for x in order if x in avail)
+        chosen.append(op)
+        cands = [c for c in alive if c[4][-k] == op]
+        state = {"M": "H", "D": "D", "I": "I"}[op]
+    i0, j0, _, _, ops = final
+    i, j, nm = i0, j0, 0
+    for op in ops:
+        if op == "M":
+            nm += int(T[i] == R[j] and T[i] != "N")
+            i += 1
+            j += 1
+        elif op == "I":
+            j += 1
+        else:
+            i += 1
+    cigar = (f"{j0}S" if j0 else "") + rle(ops) + (f"{n - je}S" if n - je else "")
+    return dict(score=best, ref_start=i0, ref_end=ie - 1, read_start=j0, read_end=je - 1, cigar=cigar, n_match=nm,
+                n_cols=len(ops), n_maximisers=len(pool))
+
+
+def longest_common_substring(T: str, R: str) -> int:
+    """Textbook O(mn) table of common-suffix lengths (N never matches)."""
+    best = 0
+    prev = [0] * (len(R) + 1)
+    for i in range(1, len(T) + 1):
+        cur = [0] * (len(R) + 1)
+        for j in range(1, len(R) + 1):
+            if T[i - 1] == R[j - 1] and T[i - 1] != "N":
+                cur[j] = prev[j - 1] + 1
+                best = max(best, cur[j])
+        prev = cur
+    return best
