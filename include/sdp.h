@@ -19,7 +19,7 @@
  *   readable up to the next multiple of 16 bytes past the last word used.
  *
  * Coordinates are 0-based, inclusive, relative to the window. The whole read is aligned
- * (read_start = 0, read_end = n-1). ref_end - ref_start + 1 is the number of window bases the
+ * (read_start = 0, read_end = n-1; SDP_MODE_LOCAL differs, see sdp_set_mode). ref_end - ref_start + 1 is the number of window bases the
  * CIGAR consumes and may be 0 (an all-insertion alignment reports ref_start = ref_end + 1).
  * CIGAR runs use the BAM encoding (len << 4) | op with M=0, I=1, D=2; runs of one pair are
  * contiguous, in alignment order, at cigar_ops[cigar_off[p] .. cigar_off[p] + cigar_len[p]).
@@ -35,19 +35,23 @@ extern "C" {
 
 #define SDP_OK       0
 #define SDP_EINVAL  (-1)  /* null pointer, bad scoring, empty sequence, index / offset out of range  */
-#define SDP_ERANGE  (-2)  /* a pair's lengths break the int16 range rule below                        */
+#define SDP_ERANGE  (-2)  /* a pair is beyond even the int32 lane (see the range rule below)                 */
 #define SDP_ECUDA   (-3)  /* a CUDA call failed; sdp_last_error() has the CUDA message                */
 #define SDP_ENOMEM  (-4)  /* host or device allocation failed                                         */
 
-/* Longest read the register-resident kernels take (32 lanes x 32 columns). */
+/* Longest read the register-resident int16 kernels take (32 lanes x 32 columns). */
 #define SDP_MAX_READ_LEN 1024
 /*
  * int16 range rule (per pair, n = read length, m = window length):
  *     match*n + gap_extend*(n + m + 32) + 3*gap_open + 8 + |2*gap_extend + mismatch| <= SDP_MAX_CELL_VALUE
- * The kernels store H + gap_extend*(i+j) + bias in 16-bit lanes; the left side bounds every stored value and every
- * intermediate sum (R13). Pairs that break the rule are never clamped.
+ * The int16 kernels store H + gap_extend*(i+j) + bias in 16-bit lanes; the left side bounds every stored value and
+ * every intermediate sum (R13). A pair that breaks the rule, or whose read is longer than SDP_MAX_READ_LEN,
+ * is never clamped and never rejected for that: it takes the int32 lane (one thread per pair, much slower, same
+ * results). SDP_ERANGE is left for what that lane cannot hold either: a sequence longer than SDP_MAX_SEQ_LEN, or
+ * traceback scratch of one pair beyond 16 GiB.
  */
 #define SDP_MAX_CELL_VALUE 32000
+#define SDP_MAX_SEQ_LEN 1000000
 /* Largest magnitude of match, mismatch, gap_open and gap_extend sdp_create accepts. */
 #define SDP_MAX_SCORE_PARAM 4000
 
@@ -69,7 +73,7 @@ typedef struct sdp_scoring {
 typedef struct sdp_batch {
     const uint32_t* reads_packed;  /* 2-bit packed read bases                                   */
     const uint64_t* read_off;      /* [n_reads] first base of read r, in bases                  */
-    const uint32_t* read_len;      /* [n_reads] length in bases, 1..SDP_MAX_READ_LEN            */
+    const uint32_t* read_len;      /* [n_reads] length in bases, 1..SDP_MAX_SEQ_LEN             */
     const uint32_t* read_nmask;    /* nullable N bitmap over reads_packed's base offsets        */
     uint32_t        n_reads;
     uint64_t        reads_bases;   /* bases addressable in reads_packed (for bounds checks)     */
@@ -90,8 +94,8 @@ typedef struct sdp_result {
     const int32_t*  score;        /* max_{1<=i<=m} M(i,n)                          */
     const int32_t*  ref_start;    /* first consumed window base (where the traceback stops)     */
     const int32_t*  ref_end;      /* (lowest maximising row i) - 1                               */
-    const int32_t*  read_start;   /* always 0                                                    */
-    const int32_t*  read_end;     /* always n-1                                                  */
+    const int32_t*  read_start;   /* 0 (first aligned read base in SDP_MODE_LOCAL)               */
+    const int32_t*  read_end;     /* n-1 (last aligned read base in SDP_MODE_LOCAL)              */
     const uint8_t*  pass;         /* similarity filter, 1 = pass                                 */
     const int32_t*  n_match;      /* M columns whose two bases are equal and not N               */
     const int32_t*  n_cols;       /* alignment columns = M + I + D bases                         */
@@ -120,6 +124,7 @@ typedef struct sdp_stats {
     float ms_compact;             /* a7 + a8                                                     */
     uint64_t cells_prefiltered;   /* sum n*m of the pairs the ungapped pre-pass settled (sdp_set_prefilter);
                                      cells_forward counts only the pairs that went through the DP   */
+    uint64_t n_slow_words;        /* int32 row-array words of the pairs that took the int32 lane (0 = none did)     */
 } sdp_stats;
 
 /* Create a context on CUDA device `cuda_device`. SDP_EINVAL for bad scoring or null arguments,
@@ -170,6 +175,21 @@ typedef struct sdp_read_best {
  * `cuda_stream`, returns after completion. SDP_EINVAL for null arguments or a result of another batch. */
 int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* result, void* cuda_stream,
                       sdp_read_best* out);
+
+/*
+ * Alignment mode. SDP_MODE_SEMIGLOBAL (default) is the paper's formulation: the whole read against any sub-region of
+ * the window. SDP_MODE_LOCAL is the soft-clipping variant (the paper names
+ * Smith-Waterman, and soft-clipped alignments; R18): M(i,0) = M(0,j) = 0,
+ * M(i,j) = max(0, ...), score = max over all cells (lowest row, then lowest column), the walk stops at the first cell
+ * with M = 0. Then read_start / read_end are the first / last aligned read base, unaligned read ends appear in the
+ * CIGAR as soft clips (BAM op 4), n_cols counts aligned columns only, and the filter counts clipped bases as columns
+ * that do not match: pass iff n_cols > 0 and n_match * 1e6 >= q * (n_cols + clipped). A pair without any positive-
+ * scoring alignment reports score 0, ref_start 0, ref_end -1, read_start 0, read_end -1, CIGAR <n>S, pass 0.
+ * In this release local mode runs on the int32 lane (exact, not tuned). SDP_EINVAL for an unknown mode.
+ */
+#define SDP_MODE_SEMIGLOBAL 0
+#define SDP_MODE_LOCAL 1
+int sdp_set_mode(sdp_ctx* ctx, int mode);
 
 /* Candidate screening for the step-3 shape: with score-only on (1), sdp_align_batch / sdp_align_batch_host stop
  * after the forward score pass (a1-a3): `score` and `ref_end` are as always, `ref_start` and `read_end` are -1,

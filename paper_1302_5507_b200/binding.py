@@ -18,12 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libsdp.so")
 
 SDP_OK, SDP_EINVAL, SDP_ERANGE, SDP_ECUDA, SDP_ENOMEM = 0, -1, -2, -3, -4
 SDP_MAX_READ_LEN = 1024
+SDP_MAX_SEQ_LEN = 1000000
 SDP_MAX_CELL_VALUE = 32000
 SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE = 1, 2
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_mate_windows", "sdp_mate_pairs",
+           "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_set_mode", "sdp_mate_windows", "sdp_mate_pairs",
            "sdp_proper_pairs"]
 
 
@@ -73,7 +74,7 @@ class sdp_stats(ctypes.Structure):
                 ("kernel_launches", ctypes.c_uint32), ("forward_launches", ctypes.c_uint32),
                 ("ms_total", ctypes.c_float), ("ms_bucket", ctypes.c_float), ("ms_forward", ctypes.c_float),
                 ("ms_reverse", ctypes.c_float), ("ms_traceback", ctypes.c_float), ("ms_compact", ctypes.c_float),
-                ("cells_prefiltered", ctypes.c_uint64)]
+                ("cells_prefiltered", ctypes.c_uint64), ("n_slow_words", ctypes.c_uint64)]
 
     def as_dict(self) -> dict:
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -116,6 +117,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_set_prefilter.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_debug_route.restype = ctypes.c_int
     lib.sdp_set_debug_route.argtypes = [ctypes.c_void_p, ctypes.c_uint32]
+    lib.sdp_set_mode.restype = ctypes.c_int
+    lib.sdp_set_mode.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_score_only.restype = ctypes.c_int
     lib.sdp_set_score_only.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_get_stats.restype = ctypes.c_int
@@ -171,7 +174,7 @@ class HostResult:
 
     def cigar(self, p: int) -> str:
         o, l = int(self.cigar_off[p]), int(self.cigar_len[p])
-        return "".join(f"{int(x) >> 4}{'MID'[int(x) & 15]}" for x in self.cigar_ops[o:o + l])
+        return "".join(f"{int(x) >> 4}{'MIDNS'[int(x) & 15]}" for x in self.cigar_ops[o:o + l])
 
 
 _cudart_lib = None
@@ -253,6 +256,10 @@ class Context:
         """sdp_set_debug_route: route pairs through the other traceback kernels / force a thread-group size (tests)."""
         flags = (SDP_ROUTE_NO_THIN if no_thin else 0) | (SDP_ROUTE_NO_WIDE if no_wide else 0) | ((int(force_g) & 0x3F) << 8)
         self._check(self._lib.sdp_set_debug_route(self._h, flags))
+
+    def set_mode(self, local: bool):
+        """sdp_set_mode: False = the paper's semi-global formulation (default), True = local / soft-clipping variant."""
+        self._check(self._lib.sdp_set_mode(self._h, 1 if local else 0))
 
     def set_score_only(self, enabled: bool):
         self._lib.sdp_set_score_only(self._h, int(bool(enabled)))

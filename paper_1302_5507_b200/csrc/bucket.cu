@@ -69,10 +69,11 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
                                uint32_t* __restrict__ hist, uint32_t* __restrict__ err_flag,
                                unsigned long long* __restrict__ cells, int prefilter,
                                int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
-                               unsigned long long* __restrict__ cells_skipped)
+                               unsigned long long* __restrict__ cells_skipped, int local,
+                               uint32_t* __restrict__ slow_words)
 {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t key = SDP_KEY_SKIP, err = 0;
+    uint32_t key = SDP_KEY_SKIP, err = 0, slow = 0;
     unsigned long long my_cells = 0;
     if (p < b.n_pairs) {
         const uint32_t ri = b.pairs[2 * p], wi = b.pairs[2 * p + 1];
@@ -82,11 +83,17 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
             const uint64_t ro = b.read_off[ri], wo = b.win_off[wi];
             if (n < 1 || m < 1 || ro + n > b.reads_bases || wo + m > b.wins_bases || ro + n < ro || wo + m < wo)
                 err = SDP_ERRF_INDEX;
-            else if (n > SDP_MAX_READ_LEN ||
+            else if (n > SDP_MAX_SEQ_LEN || m > SDP_MAX_SEQ_LEN)
+                err = SDP_ERRF_RANGE;                      // beyond even the int32 lane
+            else if (local || n > SDP_MAX_READ_LEN ||
                      (long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + m + 32) + 3LL * sc.gap_open + 8 +
-                             llabs(2LL * sc.gap_extend + sc.mismatch) > SDP_MAX_CELL_VALUE)
-                err = SDP_ERRF_RANGE;
-            else {
+                             llabs(2LL * sc.gap_extend + sc.mismatch) > SDP_MAX_CELL_VALUE) {
+                // outside the int16 kernels' domain (or local mode): the int32 lane (slow_lane.cu) takes the pair; it
+                // never enters the forward buckets. slow_words = its two row arrays of n + 1 entries.
+                pn[p] = n; pm[p] = m;
+                my_cells = (unsigned long long)n * m;
+                slow = 2u * (n + 1u);
+            } else {
                 key = (n - 1) * 64u + min(63u, m >> 6);
                 pn[p] = n; pm[p] = m;
                 my_cells = (unsigned long long)n * m;
@@ -100,6 +107,7 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
             }
         }
         keys[p] = key;
+        slow_words[p] = slow;
     }
     if (err) atomicOr(err_flag, err);
     // warp-aggregated histogram: one atomic per distinct key per warp
@@ -329,10 +337,12 @@ void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbou
 // host wrappers
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
-                         int32_t* ref_end, unsigned long long* cells_skipped, cudaStream_t st)
+                         int32_t* ref_end, unsigned long long* cells_skipped, int local, uint32_t* slow_words,
+                         cudaStream_t st)
 {
     const uint32_t grid = (uint32_t)((b.n_pairs + 255) / 256);
-    k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells, prefilter, score, ref_end, cells_skipped);
+    k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells, prefilter, score, ref_end, cells_skipped,
+                                         local, slow_words);
 }
 
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,

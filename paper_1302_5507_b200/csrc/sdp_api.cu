@@ -42,6 +42,7 @@ struct Mailbox {                    // pinned host memory the device results lan
     uint32_t tb_bounds[THIN_NW + TB_NCLASS + 1];   // narrow-band launches (one per W), then the generic band classes
     uint32_t err_flag;
     uint64_t totals[4];             // [0] thin direction-bit words, [1] run capacity, [2] CIGAR runs, [3] wide nibble words
+    uint64_t slow_total;            // words of int32 row arrays the slow lane needs
     unsigned long long counters[8]; // [0] reverse cells [1] traceback cells [2] reverse pairs [3] forward cells
                                     // [4] cells of pairs the ungapped pre-pass settled
 };
@@ -67,6 +68,7 @@ struct sdp_ctx {
     bool timing = false;
     bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
     bool score_only = false;         // sdp_set_score_only: stop after the forward pass
+    int mode = SDP_MODE_SEMIGLOBAL;  // sdp_set_mode
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
     uint32_t cls_begin[2 * SDP_MAX_K + 3];   // first slot of class c = 2K + padded; [c+1] ends it
@@ -102,6 +104,7 @@ struct sdp_ctx {
     // sdp_best_per_read
     DevBuf rb_key, rb_pair, rb_score, rb_second, rb_ncand;
     DevBuf mp_flag, mp_off;          // sdp_mate_pairs
+    DevBuf slow_words, slow_off, slow_rows;   // int32 lane (slow_lane.cu): per-pair row-array words, their offsets, the arrays
     const uint32_t* last_pairs = nullptr;   // pair list of the last successful align call (to match results to it)
     uint64_t last_n_pairs = 0;
     uint32_t last_n_reads = 0;
@@ -306,7 +309,7 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
                       &ctx->in_win_nmask, &ctx->in_pairs, &ctx->tb_rows, &ctx->keys_wide, &ctx->order_wide,
                       &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits,
-                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off};
+                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off, &ctx->slow_words, &ctx->slow_off, &ctx->slow_rows};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
     for (int i = 0; i < 4; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
@@ -356,6 +359,15 @@ int sdp_set_prefilter(sdp_ctx* ctx, int enabled)
 {
     if (!ctx) return SDP_EINVAL;
     ctx->prefilter = enabled != 0;
+    return SDP_OK;
+}
+
+int sdp_set_mode(sdp_ctx* ctx, int mode)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (mode != SDP_MODE_SEMIGLOBAL && mode != SDP_MODE_LOCAL) return fail(ctx, SDP_EINVAL, "unknown alignment mode %d", mode);
+    ctx->mode = mode;
     return SDP_OK;
 }
 
@@ -465,6 +477,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     for (int k = 0; k < 3; ++k) { EN(scan_local[k], Pp * 4); EN(scan_tiles[k], (Pp / 4096 + 2) * 4); EN(scan_tile_base[k], (Pp / 4096 + 2) * 8); }
     EN(score, Pp * 4); EN(ref_start, Pp * 4); EN(ref_end, Pp * 4); EN(read_start, Pp * 4); EN(read_end, Pp * 4);
     EN(pass, Pp); EN(n_match, Pp * 4); EN(n_cols, Pp * 4); EN(cigar_off, Pp * 8); EN(cigar_len, Pp * 4);
+    EN(slow_words, Pp * 4); EN(slow_off, Pp * 8);
+    const int local = ctx->mode == SDP_MODE_LOCAL ? 1 : 0;
 
     auto finish = [&](uint64_t n_ops) {
         out->score = ctx->score.as<int32_t>(); out->ref_start = ctx->ref_start.as<int32_t>();
@@ -488,8 +502,13 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     CU(cudaMemsetAsync(ctx->err_flag, 0, 4, st));
     CU(cudaMemsetAsync(ctx->counters, 0, 8 * 8, st));
     launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
-                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, ctx->prefilter ? 1 : 0, ctx->score.as<int32_t>(),
-                        ctx->ref_end.as<int32_t>(), ctx->counters + 4, st);
+                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, (ctx->prefilter && !local) ? 1 : 0, ctx->score.as<int32_t>(),
+                        ctx->ref_end.as<int32_t>(), ctx->counters + 4, local, ctx->slow_words.as<uint32_t>(), st);
+    // row arrays of the int32 lane: offsets now, so that the arrays can be allocated after the synchronisation below
+    exclusive_scan_u32_u64(ctx->slow_words.as<uint32_t>(), P, ctx->slow_off.as<uint64_t>(), ctx->totals + 0,
+                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
+                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
+    CU(cudaMemcpyAsync(&ctx->mb->slow_total, ctx->totals + 0, 8, cudaMemcpyDeviceToHost, st));
     launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0],
                      ctx->mb->task_prefix[0], &ctx->mb->bin_total[0], st);
@@ -499,7 +518,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (ctx->mb->err_flag & SDP_ERRF_INDEX)
         return fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)");
     if (ctx->mb->err_flag & SDP_ERRF_RANGE)
-        return fail(ctx, SDP_ERANGE, "a pair breaks the int16 range rule or SDP_MAX_READ_LEN (see sdp.h)");
+        return fail(ctx, SDP_ERANGE, "a sequence is longer than SDP_MAX_SEQ_LEN (see sdp.h)");
     // (with the ungapped pre-pass on, fewer than P pairs are in the forward buckets)
     launch_fill_desc_fwd(b, ctx->order.as<uint32_t>(), ctx->mb->bin_total[0], ctx->desc.as<PairDesc>(), st);
     ++nl;
@@ -511,6 +530,15 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         int rc = launch_score_stage(ctx, 0, b, ctx->desc.as<PairDesc>(), st, &nl);
         if (rc != SDP_OK) return rc;
         stats.forward_launches = nl - before;
+    }
+    stats.n_slow_words = ctx->mb->slow_total;
+    if (ctx->mb->slow_total) {
+        // the int32 lane: pairs outside the int16 kernels' domain, and every pair in local mode (slow_lane.cu)
+        EN(slow_rows, (ctx->mb->slow_total + 4) * 4);
+        launch_forward_i32(b, ctx->sc, local, ctx->slow_words.as<uint32_t>(), ctx->slow_off.as<uint64_t>(),
+                           ctx->slow_rows.as<int32_t>(), ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
+                           ctx->rev_rows.as<int32_t>(), st);
+        ++nl;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_FORWARD], st));
 
@@ -551,6 +579,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
     pp.keys_wide = ctx->keys_wide.as<uint32_t>();
     pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin;
+    pp.local = local; pp.slow_words = ctx->slow_words.as<uint32_t>(); pp.end_col = ctx->rev_rows.as<int32_t>();
+    pp.err_flag = ctx->err_flag;
     pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
     pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
@@ -636,7 +666,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     TraceParams tp{};
     tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
     tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
-    tp.rev_rows = nullptr;
+    tp.rev_rows = nullptr; tp.end_col = ctx->rev_rows.as<int32_t>();
     tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
     tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
     tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
@@ -649,7 +679,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         tp.first = ctx->mb->tb_bounds[c];
         tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
         if (!tp.count) continue;
-        launch_traceback(c - THIN_NW, tp, ss);
+        launch_traceback(c - THIN_NW, local != 0, tp, ss);
         ++nl;
     }
     CU(cudaEventRecord(ctx->side_done, ss));
@@ -671,6 +701,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
+    if (ctx->mb->err_flag & SDP_ERRF_RANGE)
+        return fail(ctx, SDP_ERANGE, "the traceback scratch of one pair exceeds 16 GiB (see sdp.h)");
     if (ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
         return fail(ctx, SDP_ECUDA, "internal consistency check failed (flags 0x%x): reverse pass or traceback "
                     "disagrees with the forward score", ctx->mb->err_flag);

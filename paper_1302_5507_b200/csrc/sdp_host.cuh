@@ -13,7 +13,8 @@ struct Scoring {
 // ---- bucket.cu
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
-                         int32_t* ref_end, unsigned long long* cells_skipped, cudaStream_t st);
+                         int32_t* ref_end, unsigned long long* cells_skipped, int local, uint32_t* slow_words,
+                         cudaStream_t st);
 // scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
@@ -58,6 +59,10 @@ struct PostParams {
     uint32_t* keys_tb;           // bucket key of the one-thread-per-pair traceback (everything else)
     int wide_ok;                 // scoring fits the x8 tagged domain of trace_kernel.cuh
     int no_thin;                 // debugging: keep W >= 1 pairs off the narrow-band kernel
+    int local;                   // SDP_MODE_LOCAL
+    const uint32_t* slow_words;  // != 0: the pair went through the int32 lane
+    const int32_t* end_col;      // local: read column of the end cell
+    uint32_t* err_flag;
     uint32_t* bits_words;        // direction-bit words the pair needs
     uint32_t* ops_cap;           // CIGAR run capacity the pair needs (2W + 1)
     uint32_t* hist_rev; uint32_t* hist_tb; uint32_t* hist_wide;
@@ -73,6 +78,7 @@ struct TraceParams {
     const uint32_t* order;       // traceback bucket order
     uint32_t first, count;       // range of `order` this launch covers
     const int32_t* score; const int32_t* ref_end; const int32_t* tbW; const int32_t* rev_rows;
+    const int32_t* end_col;      // local variant: read column of the end cell
     const uint64_t* bits_off; uint32_t* bits;     // direction bits scratch
     const uint64_t* ops_off;  uint32_t* ops_rev;  // per-pair runs, end -> start order
     int32_t* ref_start; int32_t* read_start; int32_t* read_end; uint8_t* pass;
@@ -98,9 +104,13 @@ struct WalkParams {
 };
 void launch_walk(const WalkParams& wp, cudaStream_t st);
 // band-width classes of the traceback kernel (local-memory row arrays)
-constexpr int TB_NCLASS = 4;
-constexpr int TB_CLASS_BW[TB_NCLASS] = {16, 64, 256, 1032};   // band <= min(2W+1, n+1) <= 1025
-void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st);
+constexpr int TB_NCLASS = 5;               // row arrays of 16 / 64 / 256 / 1032 entries in local memory; the last class keeps
+                                           // them in global scratch (any width: the int32 lane and the local variant)
+void launch_traceback(int cls, bool local, const TraceParams& tp, cudaStream_t st);
+
+// ---- slow_lane.cu: int32 forward pass, one thread per pair (pairs with slow_words[p] != 0)
+void launch_forward_i32(const sdp_batch& b, const Scoring& sc, int local, const uint32_t* slow_words, const uint64_t* slow_off,
+                        int32_t* rows, int32_t* score, int32_t* ref_end, int32_t* end_col, cudaStream_t st);
 // narrow bands (thin_kernel.cu): gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
 constexpr int THIN_NW = 24;
 constexpr int THIN_SPLIT = 8;             // classes below / from here on run in two launches (register budgets differ)

@@ -29,8 +29,8 @@ struct SeqReader {
 // after the forward pass: gap-content bound, bucket keys of the reverse and traceback passes,
 // scratch sizes. One thread per pair.
 __device__ __forceinline__ int tb_class_of(int bw) {
-    static_assert(TB_NCLASS == 4, "update tb_class_of");
-    return bw > 256 ? 3 : (bw > 64 ? 2 : (bw > 16 ? 1 : 0));
+    static_assert(TB_NCLASS == 5, "update tb_class_of");
+    return bw > 1032 ? 4 : (bw > 256 ? 3 : (bw > 64 ? 2 : (bw > 16 ? 1 : 0)));
 }
 static_assert((THIN_NW + TB_NCLASS) * TB_KEY_STRIDE <= SDP_NBINS && SDP_MAX_READ_LEN < TB_KEY_STRIDE, "thin keys must fit the bucket-sort key space");
 
@@ -48,13 +48,17 @@ __global__ void k_post_forward(const PostParams pp)
     const bool valid = p < pp.n_pairs;
     uint32_t krev = SDP_KEY_SKIP, ktb = SDP_KEY_SKIP, kwide = SDP_KEY_SKIP;
     unsigned long long c_rev = 0, c_tb = 0, n_rev = 0;
+    bool too_big = false;
     if (valid) {
-        const int n = (int)pp.pn[p];
+        // slow = the int32 lane (slow_lane.cu): pairs outside the int16 kernels' domain, and every pair in local mode,
+        // where only the first end_col read columns matter (the alignment ends in column end_col)
+        const bool slow = pp.slow_words[p] != 0;
+        const int n = pp.local ? pp.end_col[p] : (int)pp.pn[p];
         const int S = pp.score[p], i_end = pp.ref_end[p] + 1;
-        const int slack = n * pp.sc.match - S - pp.sc.gap_open;
-        int W = slack >= pp.sc.gap_extend ? slack / pp.sc.gap_extend : 0;
+        const long long slack = (long long)n * pp.sc.match - S - pp.sc.gap_open;
+        int W = slack >= pp.sc.gap_extend ? (int)min(slack / pp.sc.gap_extend, (long long)(1 << 29)) : 0;
         W = min(W, n + i_end);
-        if (W > 0 && i_end >= n) {
+        if (W > 0 && i_end >= n && !slow) {
             // Ungapped shortcut. If the gap-free alignment on the end cell's diagonal already scores S, it is the
             // alignment the traceback reports: every prefix of an optimal path is optimal for its end cell, so
             // the walk's first test (diagonal) succeeds at every step of it. Such a pair is gapless (W = 0):
@@ -81,8 +85,9 @@ __global__ void k_post_forward(const PostParams pp)
         // reverse pass first trims the rectangle's rows. Anything else: the generic band kernel.
         const long long vmax = (long long)pp.sc.match * n + (long long)pp.sc.gap_extend * (n + rows) +
                                3LL * pp.sc.gap_open + 8;
-        const bool narrow = W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && !pp.no_thin);
-        const bool wide = !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
+        if (slow && W == 0) { rows = min(i_end, n); bw = 1; }      // (the dynamic kernel walks a gapless pair through its band too)
+        const bool narrow = !slow && (W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && !pp.no_thin));
+        const bool wide = !slow && !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
         if (narrow) {
             ktb = (uint32_t)W * TB_KEY_STRIDE + (uint32_t)min((int)TB_KEY_STRIDE - 1, W ? rows : n);
             c_tb = (unsigned long long)bw * rows;
@@ -94,14 +99,19 @@ __global__ void k_post_forward(const PostParams pp)
             kwide = (uint32_t)(n - 1) * 64u + rbin;
             c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
         } else {
-            words = (uint32_t)rows * (uint32_t)((bw + 7) / 8); c_tb = (unsigned long long)bw * rows;
-            ktb = (uint32_t)(THIN_NW + tb_class_of(bw)) * TB_KEY_STRIDE + (uint32_t)min(bw, (int)TB_KEY_STRIDE - 1);
+            const int cls = slow ? TB_NCLASS - 1 : tb_class_of(bw);
+            const unsigned long long w64 = (unsigned long long)rows * (unsigned long long)((bw + 7) / 8) +
+                                           (cls == TB_NCLASS - 1 ? 2ull * (unsigned long long)(bw + 2) : 0ull);   // + the two row arrays
+            if (w64 > 0xFFFFFFFFull) { words = 0; too_big = true; } else words = (uint32_t)w64;
+            c_tb = (unsigned long long)bw * rows;
+            ktb = (uint32_t)(THIN_NW + cls) * TB_KEY_STRIDE + (uint32_t)min(bw, (int)TB_KEY_STRIDE - 1);
         }
         pp.keys_rev[p] = krev;
         pp.keys_wide[p] = kwide;
         pp.keys_tb[p] = ktb;
         pp.bits_words[p] = words;
-        pp.ops_cap[p] = 2u * (uint32_t)W + 3u;
+        pp.ops_cap[p] = 2u * (uint32_t)W + 5u;            // runs of a path with <= W gap bases, + flush slot + two soft clips
+        if (too_big) atomicOr(pp.err_flag, SDP_ERRF_RANGE);
     }
     hist_add(pp.hist_rev, krev, krev != SDP_KEY_SKIP);
     hist_add(pp.hist_tb, ktb, ktb != SDP_KEY_SKIP);
@@ -150,7 +160,10 @@ void launch_fill_desc_rev(const sdp_batch& b, const uint32_t* order, uint32_t co
 // traceback: one thread per pair, row arrays of the band in local memory (MAXBW + 2 entries).
 // Direction bits per cell: 1 = H came from the diagonal, 2 = H equals D, 4 = D was opened here,
 // 8 = I was opened here. Rows i_lo+1 .. i_end each take wpr = ceil(bw / 8) words.
-template <int MAXBW>
+// MAXBW == 0: any band width, the two row arrays sit in global scratch behind the pair's direction bits (the int32 lane:
+// reads beyond SDP_MAX_READ_LEN, windows beyond the int16 range rule). LOCAL: the soft-clipping variant (R18):
+// zero floor, walk from (i_end, end_col), stops where the remaining score is 0, clips as CIGAR op 4.
+template <int MAXBW, bool LOCAL>
 __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
 {
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -158,7 +171,8 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
     const uint32_t p = tp.order[tp.first + k];
     const sdp_batch& b = tp.b;
     const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
-    const int n = (int)b.read_len[ri];
+    const int n_full = (int)b.read_len[ri];
+    const int n = LOCAL ? tp.end_col[p] : n_full;          // local: the alignment ends in read column end_col
     const uint64_t roff = b.read_off[ri], woff = b.win_off[wi];
     const SeqReader RD{b.reads_packed, b.read_nmask, SDP_CODE_READ_N};
     const SeqReader WN{b.wins_packed, b.win_nmask, SDP_CODE_WIN_N};
@@ -166,9 +180,9 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
     const int W = tp.tbW[p];
     const int o = tp.sc.gap_open, e = tp.sc.gap_extend, oe = o + e;
     uint32_t* ops = tp.ops_rev + tp.ops_off[p];
-    const uint32_t cap = 2u * (uint32_t)W + 3u;
+    const uint32_t cap = 2u * (uint32_t)W + 5u;
 
-    int n_match = 0, n_cols = 0, ref_start = 0;
+    int n_match = 0, n_cols = 0, ref_start = 0, read_start = 0;
     uint32_t nops = 0;
     int cur_op = -1; uint32_t cur_len = 0;
     bool bad = false;
@@ -177,8 +191,11 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
         if (cur_op >= 0) { if (nops < cap) ops[nops] = (cur_len << 4) | (uint32_t)cur_op; else bad = true; ++nops; }
         cur_op = op; cur_len = len;
     };
+    if (LOCAL && n_full > n && tp.score[p] > 0) emit(4, (uint32_t)(n_full - n));   // trailing soft clip (runs are stored end -> start)
 
-    if (W == 0) {
+    if (LOCAL && tp.score[p] == 0) {
+        emit(4, (uint32_t)n_full);                        // no alignment: everything is clipped
+    } else if (W == 0 && MAXBW != 0) {
         // gapless: the only co-optimal alignments are ungapped, so the CIGAR is nM
         ref_start = i_end - n;
         if (ref_start < 0) { bad = true; ref_start = 0; }
@@ -197,15 +214,17 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
         const int shift = banded ? 1 : 0;
         const int wpr = (bw + 7) / 8;
         uint32_t* bits = tp.bits + tp.bits_off[p];
-        if (bw > MAXBW) { bad = true; }
+        if (MAXBW != 0 && bw > MAXBW) { bad = true; }
         else {
-            int Hr[MAXBW + 2], Dr[MAXBW + 2];
-            // row i_lo is the restricted problem's row 0: H = -(o + e j) via insertions, H(.,0) = 0
+            int Hloc[MAXBW + 2], Dloc[MAXBW + 2];
+            int* const Hr = MAXBW != 0 ? Hloc : reinterpret_cast<int*>(bits + (size_t)(i_end - i_lo) * wpr);
+            int* const Dr = MAXBW != 0 ? Dloc : Hr + (bw + 2);
+            // row i_lo is the restricted problem's row 0: H = -(o + e j) via insertions, H(.,0) = 0 (local: all zero)
             {
                 const int jb = banded ? (i_lo - c - W) : 0;
                 for (int jj = 0; jj <= bw; ++jj) {
                     const int j = jj + jb;
-                    Hr[jj] = (jj == bw || j < 0 || j > n) ? NEG : (j == 0 ? 0 : -(o + e * j));
+                    Hr[jj] = (jj == bw || j < 0 || j > n) ? NEG : ((j == 0 || LOCAL) ? 0 : -(o + e * j));
                     Dr[jj] = NEG;
                 }
             }
@@ -232,6 +251,7 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
                         Dn = max(upH - oe, upD - e);
                         const int dg = dgH + ((r == t) ? tp.sc.match : tp.sc.mismatch);
                         Hn = max(dg, max(Dn, In));
+                        if (LOCAL) Hn = max(Hn, 0);
                         f = (Hn == dg ? 1u : 0u) | (Hn == Dn ? 2u : 0u) | (Dn == upH - oe ? 4u : 0u) |
                             (In == Hleft - oe ? 8u : 0u);
                     }
@@ -241,53 +261,69 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
                 }
             }
             if (Hr[n - (banded ? (i_end - c - W) : 0)] != tp.score[p]) bad = true;   // band DP must end on S
-            // walk back from (i_end, n)
+            // walk back from (i_end, n). Local: `rem` is the score still to be explained, i.e. M(i,j) while in state H;
+            // the walk stops where it reaches 0 (R18), and what is left of the read is a soft clip.
             int i = i_end, j = n, st = 0;                  // 0 = H, 1 = D, 2 = I
+            int rem = tp.score[p], run = 0;
             while (j > 0) {
-                if (i == i_lo) { emit(1, (uint32_t)j); n_cols += j; j = 0; break; }
+                if (LOCAL && st == 0 && rem == 0) break;
+                if (i == i_lo) {
+                    if (LOCAL) { bad = true; break; }      // a local alignment never starts with a gap
+                    emit(1, (uint32_t)j); n_cols += j; j = 0; break;
+                }
                 const int jj = j - (banded ? (i - c - W) : 0);
                 if (jj < 0 || jj >= bw) { bad = true; break; }
                 const uint32_t f = (bits[(size_t)(i - i_lo - 1) * wpr + (jj >> 3)] >> (4 * (jj & 7))) & 15u;
                 if (st == 0) {
                     if (f & 1u) {
                         emit(0, 1u); ++n_cols;
-                        n_match += (RD.at(roff + (uint64_t)(j - 1)) == WN.at(woff + (uint64_t)(i - 1)));
+                        const bool eq = RD.at(roff + (uint64_t)(j - 1)) == WN.at(woff + (uint64_t)(i - 1));
+                        n_match += eq;
+                        rem -= eq ? tp.sc.match : tp.sc.mismatch;
                         --i; --j;
-                    } else if (f & 2u) st = 1;
-                    else st = 2;
+                    } else if (f & 2u) { st = 1; run = 0; }
+                    else { st = 2; run = 0; }
                 } else if (st == 1) {
-                    emit(2, 1u); ++n_cols;
-                    if (f & 4u) st = 0;
+                    emit(2, 1u); ++n_cols; ++run;
+                    if (f & 4u) { st = 0; rem += o + e * run; }
                     --i;
                 } else {
-                    emit(1, 1u); ++n_cols;
-                    if (f & 8u) st = 0;
+                    emit(1, 1u); ++n_cols; ++run;
+                    if (f & 8u) { st = 0; rem += o + e * run; }
                     --j;
                 }
             }
+            if (LOCAL && (rem != 0 || st != 0)) bad = true;
             ref_start = i;
+            read_start = j;
+            if (LOCAL && j > 0) emit(4, (uint32_t)j);       // leading soft clip
         }
     }
     emit(-2, 0u);                                          // flush the last run
     if (bad) { atomicOr(tp.err_flag, SDP_ERRF_TRACE); nops = min(nops, cap); }
-    tp.ref_start[p] = ref_start;
-    tp.read_start[p] = 0;
-    tp.read_end[p] = n - 1;
+    const bool none = LOCAL && tp.score[p] == 0;
+    tp.ref_start[p] = none ? 0 : ref_start;
+    tp.read_start[p] = none ? 0 : read_start;
+    tp.read_end[p] = none ? -1 : n - 1;
     tp.n_match[p] = n_match;
     tp.n_cols[p] = n_cols;
     tp.cigar_len[p] = nops;
-    tp.pass[p] = ((long long)n_match * 1000000LL >= tp.sc.min_sim_q * (long long)n_cols) ? 1 : 0;
+    // local: soft-clipped read bases count as columns that do not match, and an empty alignment never passes (R18)
+    const long long cols = LOCAL ? (long long)n_cols + (none ? n_full : read_start + (n_full - n)) : (long long)n_cols;
+    tp.pass[p] = ((!LOCAL || n_cols > 0) && (long long)n_match * 1000000LL >= tp.sc.min_sim_q * cols) ? 1 : 0;
 }
 
-void launch_traceback(int cls, const TraceParams& tp, cudaStream_t st)
+void launch_traceback(int cls, bool local, const TraceParams& tp, cudaStream_t st)
 {
     if (tp.count == 0) return;
     const uint32_t grid = (tp.count + 127) / 128;
+    if (local) { k_traceback<0, true><<<grid, 128, 0, st>>>(tp); return; }
     switch (cls) {
-        case 0: k_traceback<16><<<grid, 128, 0, st>>>(tp); break;
-        case 1: k_traceback<64><<<grid, 128, 0, st>>>(tp); break;
-        case 2: k_traceback<256><<<grid, 128, 0, st>>>(tp); break;
-        default: k_traceback<1032><<<grid, 128, 0, st>>>(tp); break;
+        case 0: k_traceback<16, false><<<grid, 128, 0, st>>>(tp); break;
+        case 1: k_traceback<64, false><<<grid, 128, 0, st>>>(tp); break;
+        case 2: k_traceback<256, false><<<grid, 128, 0, st>>>(tp); break;
+        case 3: k_traceback<1032, false><<<grid, 128, 0, st>>>(tp); break;
+        default: k_traceback<0, false><<<grid, 128, 0, st>>>(tp); break;
     }
 }
 

@@ -11,11 +11,11 @@ FIELDS = ["score", "ref_end", "ref_start", "read_start", "read_end", "n_match", 
           "cigar_off"]
 
 
-def run_oracle(batch, sc: OracleScoring, threads=None):
+def run_oracle(batch, sc: OracleScoring, threads=None, local=False):
     threads = threads or os.cpu_count() or 1
     return oracle.align_batch(batch.reads_packed, batch.read_off, batch.read_len, batch.wins_packed, batch.win_off,
                               batch.win_len, batch.pairs, sc, read_nmask=batch.read_nmask,
-                              win_nmask=batch.win_nmask, threads=threads)
+                              win_nmask=batch.win_nmask, threads=threads, local=local)
 
 
 def describe(batch, p, exp, got):
@@ -46,8 +46,9 @@ def assert_equal(batch, exp, got, what=""):
         raise AssertionError(f"{what}: cigar_ops differ; first:\n" + describe(batch, p, exp, got))
 
 
-def check_batch(ctx, batch, sc: OracleScoring, what="", host_path=True):
-    exp = run_oracle(batch, sc)
+def check_batch(ctx, batch, sc: OracleScoring, what="", host_path=True, local=False):
+    """`local` must match the mode the ctx was put in (Context.set_mode)."""
+    exp = run_oracle(batch, sc, local=local)
     db = ctx.upload(batch)
     got = ctx.fetch(ctx.align_batch(db))
     assert_equal(batch, exp, got, what + " [device path]")

@@ -47,7 +47,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(binding.sdp_scoring) == 24
     assert ctypes.sizeof(binding.sdp_batch) == 112
     assert ctypes.sizeof(binding.sdp_result) == 104
-    assert ctypes.sizeof(binding.sdp_stats) == 80
+    assert ctypes.sizeof(binding.sdp_stats) == 88
 
 
 def test_no_cpu_fallback_without_library(tmp_path):

@@ -323,6 +323,81 @@ def test_mixed_window_lengths_in_one_warp(ctx):
     parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "mixed m")
 
 
+@pytest.mark.parametrize("cfg,n_pairs", [(1, 1000), (2, 2500), (3, 1500), (4, 800), (5, 3000)])
+def test_local_mode_configs(cfg, n_pairs):
+    # the soft-clipping variant on all five configs; read_start / read_end are no longer constants
+    c = make_ctx(DEFAULT)
+    try:
+        c.set_mode(local=True)
+        b = W.make_config(cfg, n_pairs=n_pairs, ref_bases=2_000_000)
+        exp, got = parity.check_batch(c, b, DEFAULT, f"local cfg{cfg}", local=True)
+        n = b.read_len[b.pairs[:, 0]].astype(np.int64)
+        clipped = (got.read_start > 0) | (got.read_end < n - 1)
+        assert clipped.any() and (~clipped).any()
+        assert ((got.cigar_ops & 15) == 4).any()
+        c.set_mode(local=False)                                  # and back: the semi-global results are unchanged
+        parity.check_batch(c, b.subset(np.arange(min(300, b.n_pairs))), DEFAULT, f"semi-global after local cfg{cfg}",
+                           host_path=False)
+    finally:
+        c.destroy()
+
+
+def test_local_mode_edges():
+    rng = random.Random(61)
+    wins, reads = [], []
+    for _ in range(500):                                         # ties, empty alignments, N, tiny sizes
+        alpha = rng.choice(["A", "AC", "AC", "ACG", "ACGTN"])
+        wins.append("".join(rng.choice(alpha) for _ in range(rng.randint(1, 70))))
+        reads.append("".join(rng.choice(alpha) for _ in range(rng.randint(1, 40))))
+    wins += ["CCCC", "A", "ACGTACGTAC", "TTTTACGTACGTTTTT"]
+    reads += ["GGGG", "CACA", "GTAC", "GGGACGTACGGGG"]
+    for sc in (DEFAULT, OracleScoring(2, -1, 1, 1, 0.5), OracleScoring(3, -9, 1, 1, 0.6), OracleScoring(1, -4, 6, 1, 0.9)):
+        c = make_ctx(sc)
+        try:
+            c.set_mode(local=True)
+            exp, got = parity.check_batch(c, W.batch_from_strings(wins, reads), sc, f"local edges {sc}", local=True)
+            assert (got.score == 0).any() and (got.ref_end[got.score == 0] == -1).all()
+        finally:
+            c.destroy()
+
+
+def test_int32_lane(ctx):
+    # pairs outside the int16 kernels' domain are aligned on the int32 lane instead of being rejected:
+    # a 9,000-base and a 17,000-base window for a 100-base read, reads of 1,025 and 2,000 bases, mixed with ordinary pairs
+    rng = random.Random(62)
+
+    def rnd(k):
+        return "".join(rng.choice("ACGT") for _ in range(k))
+
+    def mutate(seq, subs, indel):
+        seq = list(seq)
+        for _ in range(subs):
+            seq[rng.randrange(len(seq))] = rng.choice("ACGT")
+        if indel:
+            k = rng.randrange(5, len(seq) - 5)
+            seq = seq[:k] + (list(rnd(indel)) if rng.random() < 0.5 else []) + seq[k + (0 if rng.random() < 0.5 else indel):]
+        return "".join(seq)
+
+    wins, reads = [], []
+    for m, n in ((9000, 100), (17000, 100), (20000, 250), (3000, 1025), (2500, 2000), (1500, 1200), (600, 100), (500, 100)):
+        for _ in range(3):
+            T = rnd(m)
+            s = rng.randrange(0, m - n + 1)
+            reads.append((mutate(T[s:s + n], rng.randint(0, n // 20), rng.choice([0, 0, 3, 12])) + rnd(n))[:n])
+            wins.append(T)
+    reads.append(rnd(1500)); wins.append(rnd(1800))              # an unplaceable long read: widest band
+    exp, got = parity.check_batch(ctx, W.batch_from_strings(wins, reads), DEFAULT, "int32 lane")
+    assert ctx.stats()["n_slow_words"] > 0
+    # a scoring whose constants alone leave the int16 domain for ordinary lengths
+    sc = OracleScoring(300, -400, 600, 200, 0.6)
+    c = make_ctx(sc)
+    try:
+        parity.check_batch(c, W.make_config(1, n_pairs=200, ref_bases=200_000), sc, "int32 lane, large scoring", host_path=False)
+        assert c.stats()["n_slow_words"] > 0
+    finally:
+        c.destroy()
+
+
 def test_errors(ctx):
     b = W.make_config(1, n_pairs=10, ref_bases=100_000)
     bad = W.Batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len,
@@ -330,17 +405,16 @@ def test_errors(ctx):
     with pytest.raises(SdpError) as e:
         ctx.align_batch(ctx.upload(bad))
     assert e.value.code == -1
-    # int16 range rule: 1*100 + 2*(100 + 17000 + 32) > 32000
-    long_win = "ACGT" * 4250
-    rb = W.batch_from_strings([long_win], ["ACGT" * 25])
+    # a sequence longer than SDP_MAX_SEQ_LEN is beyond even the int32 lane (lengths only: the bases are never read)
+    huge = W.Batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, np.array([0], dtype=np.uint64),
+                   np.array([1_000_001], dtype=np.uint32), np.array([[0, 0]], dtype=np.uint32), None, None)
+    db = ctx.upload(huge)
+    db.c.wins_bases = 2_000_000                                  # (pretend the buffer is that long; the call fails before reading it)
     with pytest.raises(SdpError) as e:
-        ctx.align_batch(ctx.upload(rb))
+        ctx.align_batch(db)
     assert e.value.code == -2
-    # read longer than SDP_MAX_READ_LEN
-    rb = W.batch_from_strings(["ACGT" * 300], ["ACGT" * 257])
-    with pytest.raises(SdpError) as e:
-        ctx.align_batch(ctx.upload(rb))
-    assert e.value.code == -2
+    with pytest.raises(SdpError):
+        ctx._check(ctx._lib.sdp_set_mode(ctx._h, 7))             # unknown mode
     with pytest.raises(SdpError):
         Context(match=1, mismatch=1)
     with pytest.raises(SdpError):
