@@ -64,6 +64,7 @@ struct sdp_ctx {
     int wide_ok = 0;                 // scoring fits the x8 tagged domain of the traceback DP kernel
     int wide_fits = 0;               // wide_ok before sdp_set_debug_route masked it
     int no_thin = 0;                 // sdp_set_debug_route: keep W >= 1 pairs off the narrow-band kernel
+    int thin_ok = 0;                 // scoring fits the x8 tagged int16 domain of thin_kernel.cu
     char err[512] = {0};
     bool timing = false;
     bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
@@ -82,17 +83,21 @@ struct sdp_ctx {
     cudaEvent_t fan_fork = nullptr, fan_join[SDP_FAN_STREAMS] = {};
     cudaStream_t side_stream2 = nullptr;  // the wider narrow bands (W >= THIN_SPLIT): few, long-running blocks
     cudaEvent_t side_done2 = nullptr;
+    cudaStream_t side_stream3 = nullptr;  // the middle band widths (THIN_SPLIT <= W < THIN_SPLIT2)
+    cudaEvent_t side_done3 = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     // fixed-size device buffers
-    uint32_t* hist[4] = {};          // forward, reverse, thin traceback, wide traceback
+    // what every call starts from zero sits in ONE block (one memset): counters, err_flag, the three histograms
+    void* zero_block = nullptr; size_t zero_bytes = 0;
+    uint32_t* hist[4] = {};          // forward, (unused), thin traceback, wide traceback + reverse pass
     uint32_t* bin_start[4] = {};
-    SlotInfo* slots[3] = {};         // forward, reverse, wide traceback
+    SlotInfo* slots[3] = {};         // forward, (unused), wide traceback + reverse pass
     uint32_t* task_prefix[3] = {};
     uint32_t* err_flag = nullptr;
     unsigned long long* counters = nullptr;
     uint64_t* totals = nullptr;
     // per-pair device buffers (grow only)
-    DevBuf keys, pn, pm, order, desc, order_rev, desc_rev, order_tb, keys_rev, keys_tb, tbW, rev_rows,
+    DevBuf keys, pn, pm, order, desc, desc_rev, order_tb, keys_tb, tbW, rev_rows,
         tb_rows, keys_wide, order_wide, desc_wide, wide_words, wide_off, wide_bits,
         bits_words, ops_cap, bits_off, ops_off,
         score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len,
@@ -247,6 +252,9 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         // and the match increment must stay an fp16 denormal bit pattern
         ctx->wide_ok = (qx >= 0 && qm < 2048 && sc8 * beta <= 32000) ? 1 : 0;
         ctx->wide_fits = ctx->wide_ok;
+        // narrow-band kernel: 8 (match - mismatch) must read as an fp16 value below 1.0, 8 beta must leave room
+        const int c = 2 * e + s->mismatch;
+        ctx->thin_ok = (sc8 * (s->match - s->mismatch) < 0x3C00 && sc8 * (beta + (c > 0 ? c : 0)) <= 32000) ? 1 : 0;
     }
     choose_geometry(ctx, 0);
 
@@ -268,6 +276,8 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaStreamCreateWithPriority(&ctx->side_stream, cudaStreamNonBlocking, prio_lo));
         CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
         CU(cudaStreamCreateWithPriority(&ctx->side_stream2, cudaStreamNonBlocking, prio_lo));
+        CU(cudaStreamCreateWithPriority(&ctx->side_stream3, cudaStreamNonBlocking, prio_lo));
+        CU(cudaEventCreateWithFlags(&ctx->side_done3, cudaEventDisableTiming));
         CU(cudaEventCreateWithFlags(&ctx->fan_fork, cudaEventDisableTiming));
         for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
             CU(cudaStreamCreateWithFlags(&ctx->fan_stream[k], cudaStreamNonBlocking));
@@ -275,16 +285,25 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         }
         CU(cudaEventCreateWithFlags(&ctx->side_done2, cudaEventDisableTiming));
         for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
+        {
+            const size_t hist_words = ((SDP_NBINS + 1 + 3) / 4) * 4;
+            ctx->zero_bytes = 8 * 8 + 16 + 3 * hist_words * 4;
+            CU(cudaMalloc(&ctx->zero_block, ctx->zero_bytes));
+            char* z = (char*)ctx->zero_block;
+            ctx->counters = (unsigned long long*)z;
+            ctx->err_flag = (uint32_t*)(z + 64);
+            uint32_t* h = (uint32_t*)(z + 80);
+            ctx->hist[0] = h; ctx->hist[2] = h + hist_words; ctx->hist[3] = h + 2 * hist_words;
+        }
         for (int i = 0; i < 4; ++i) {
-            CU(cudaMalloc(&ctx->hist[i], (SDP_NBINS + 1) * 4));
+            if (i == 1) continue;
             CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 4 + SDP_BIN_SCRATCH) * 4));
         }
         for (int i = 0; i < 3; ++i) {
+            if (i == 1) continue;
             CU(cudaMalloc(&ctx->slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
             CU(cudaMalloc(&ctx->task_prefix[i], (SDP_NSLOTS + 1) * 4));
         }
-        CU(cudaMalloc(&ctx->err_flag, 4));
-        CU(cudaMalloc(&ctx->counters, 8 * 8));
         CU(cudaMalloc(&ctx->totals, 4 * 8));
         return SDP_OK;
     };
@@ -299,8 +318,8 @@ void sdp_destroy(sdp_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     score_modules_destroy(&ctx->modules);
-    DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->order_rev, &ctx->desc_rev,
-                      &ctx->order_tb, &ctx->keys_rev, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
+    DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->desc_rev,
+                      &ctx->order_tb, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
                       &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local[0], &ctx->scan_local[1], &ctx->scan_local[2],
                       &ctx->scan_tiles[0], &ctx->scan_tiles[1], &ctx->scan_tiles[2], &ctx->scan_tile_base[0],
                       &ctx->scan_tile_base[1], &ctx->scan_tile_base[2], &ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start,
@@ -312,15 +331,17 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off, &ctx->slow_words, &ctx->slow_off, &ctx->slow_rows};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
-    for (int i = 0; i < 4; ++i) { cudaFree(ctx->hist[i]); cudaFree(ctx->bin_start[i]); }
+    for (int i = 0; i < 4; ++i) cudaFree(ctx->bin_start[i]);
     for (int i = 0; i < 3; ++i) { cudaFree(ctx->slots[i]); cudaFree(ctx->task_prefix[i]); }
-    cudaFree(ctx->err_flag); cudaFree(ctx->counters); cudaFree(ctx->totals);
+    cudaFree(ctx->zero_block); cudaFree(ctx->totals);
     cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K); cudaFree(ctx->d_slot_of_n);
     if (ctx->mb) cudaFreeHost(ctx->mb);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
     if (ctx->side_done) cudaEventDestroy(ctx->side_done);
     if (ctx->side_stream2) cudaStreamDestroy(ctx->side_stream2);
+    if (ctx->side_stream3) cudaStreamDestroy(ctx->side_stream3);
+    if (ctx->side_done3) cudaEventDestroy(ctx->side_done3);
     if (ctx->fan_fork) cudaEventDestroy(ctx->fan_fork);
     for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
         if (ctx->fan_stream[k]) cudaStreamDestroy(ctx->fan_stream[k]);
@@ -395,16 +416,17 @@ static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const
                               cudaStream_t st, uint32_t* nlaunch)
 {
     const bool rev = which == 1;
+    const int ti = which == 0 ? 0 : 2;                    // task table: the reverse pass runs on the wide-traceback buckets
     TraceDP td{};
     td.c = ctx->tconsts; td.bits = ctx->wide_bits.as<uint32_t>(); td.bits_off = ctx->wide_off.as<uint64_t>();
-    const uint32_t* tp = ctx->mb->task_prefix[which];
+    const uint32_t* tp = ctx->mb->task_prefix[ti];
     ScoreParams sp{};
     sp.reads_packed = b.reads_packed; sp.read_nmask = b.read_nmask;
     sp.wins_packed = b.wins_packed; sp.win_nmask = b.win_nmask;
     sp.wins_words = (b.wins_bases + 15) / 16; sp.win_nmask_words = (b.wins_bases + 31) / 32;
     sp.desc = desc;
-    sp.task_prefix = ctx->task_prefix[which];
-    sp.slots = ctx->slots[which];
+    sp.task_prefix = ctx->task_prefix[ti];
+    sp.slots = ctx->slots[ti];
     sp.c = ctx->consts;
     sp.score = ctx->score.as<int32_t>(); sp.ref_end = ctx->ref_end.as<int32_t>();
     sp.rev_rows = ctx->rev_rows.as<int32_t>(); sp.err_flag = ctx->err_flag;
@@ -469,8 +491,8 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     const size_t Pp = (size_t)(P ? P : 1);
     EN(keys, Pp * 4); EN(pn, Pp * 4); EN(pm, Pp * 4); EN(order, Pp * 4); EN(desc, Pp * sizeof(PairDesc));
-    EN(order_rev, Pp * 4); EN(desc_rev, Pp * sizeof(PairDesc)); EN(order_tb, Pp * 4);
-    EN(keys_rev, Pp * 4); EN(keys_tb, Pp * 4); EN(tbW, Pp * 4); EN(rev_rows, Pp * 4);
+    EN(desc_rev, Pp * sizeof(PairDesc)); EN(order_tb, Pp * 4);
+    EN(keys_tb, Pp * 4); EN(tbW, Pp * 4); EN(rev_rows, Pp * 4);
     EN(tb_rows, Pp * 4); EN(keys_wide, Pp * 4); EN(order_wide, Pp * 4); EN(desc_wide, Pp * sizeof(PairDesc));
     EN(wide_words, Pp * 4); EN(wide_off, Pp * 8);
     EN(bits_words, Pp * 4); EN(ops_cap, Pp * 4); EN(bits_off, Pp * 8); EN(ops_off, Pp * 8);
@@ -498,9 +520,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_START], st));
     // ---- a1 + a2
-    for (int i = 0; i < 4; ++i) CU(cudaMemsetAsync(ctx->hist[i], 0, (SDP_NBINS + 1) * 4, st));
-    CU(cudaMemsetAsync(ctx->err_flag, 0, 4, st));
-    CU(cudaMemsetAsync(ctx->counters, 0, 8 * 8, st));
+    CU(cudaMemsetAsync(ctx->zero_block, 0, ctx->zero_bytes, st));
     launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
                         ctx->hist[0], ctx->err_flag, ctx->counters + 3, (ctx->prefilter && !local) ? 1 : 0, ctx->score.as<int32_t>(),
                         ctx->ref_end.as<int32_t>(), ctx->counters + 4, local, ctx->slow_words.as<uint32_t>(), st);
@@ -576,28 +596,26 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     pp.b = b; pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
     pp.score = ctx->score.as<int32_t>(); pp.ref_end = ctx->ref_end.as<int32_t>();
     pp.tbW = ctx->tbW.as<int32_t>(); pp.tb_rows = ctx->tb_rows.as<int32_t>();
-    pp.keys_rev = ctx->keys_rev.as<uint32_t>(); pp.keys_tb = ctx->keys_tb.as<uint32_t>();
+    pp.keys_tb = ctx->keys_tb.as<uint32_t>();
     pp.keys_wide = ctx->keys_wide.as<uint32_t>();
-    pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin;
+    pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin; pp.thin_ok = ctx->thin_ok;
     pp.local = local; pp.slow_words = ctx->slow_words.as<uint32_t>(); pp.end_col = ctx->rev_rows.as<int32_t>();
     pp.err_flag = ctx->err_flag;
     pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
-    pp.hist_rev = ctx->hist[1]; pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
+    pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
     launch_post_forward(pp, st);
-    // The three bucket sorts and the three scratch-offset scans are short, latency-bound launch chains that
+    // The two bucket sorts and the three scratch-offset scans are short, latency-bound launch chains that
     // depend only on k_post_forward: they fan out over the helper streams and join before the mailbox kernel.
-    cudaStream_t f1 = ctx->fan_stream[1], f2 = ctx->fan_stream[2], f3 = ctx->fan_stream[3];
+    // (The reverse pass and the wide traceback serve the same pairs with the same key: one sort, one task table.)
+    cudaStream_t f2 = ctx->fan_stream[2], f3 = ctx->fan_stream[3];
     CU(cudaEventRecord(ctx->fan_fork, st));
     for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_stream[k], ctx->fan_fork, 0));
-    launch_sort_tail(ctx->keys_rev.as<uint32_t>(), P, ctx->hist[1], ctx->bin_start[1], ctx->order_rev.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[1], ctx->task_prefix[1],
-                     ctx->mb->task_prefix[1], &ctx->mb->bin_total[1], f1);
     launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
                      nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, f2);
     launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2],
                      ctx->mb->task_prefix[2], &ctx->mb->bin_total[3], st);
-    nl += 12;
+    nl += 8;
     // one region of direction nibbles per warp task of wide pairs (every slot of order_wide beyond the wide
     // pairs reads as a zero-size region)
     CU(cudaMemsetAsync(ctx->wide_words.p, 0, P * 4, st));
@@ -621,15 +639,15 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
                    ctx->mb->tb_bounds, ctx->mb->totals, ctx->mb->counters, st);
     ++nl;
     CU(cudaStreamSynchronize(st));
-    const uint32_t n_rev = ctx->mb->bin_total[1];
     const uint32_t n_wide = ctx->mb->bin_total[3];
+    const uint32_t n_rev = n_wide;
     EN(bits, (ctx->mb->totals[0] + 4) * 4);
     EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
     EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
     EN(wide_bits, (ctx->mb->totals[3] + 4) * 4);
 
     // ---- a4 reverse pass over the pairs whose score admits a gap
-    launch_fill_desc_rev(b, ctx->order_rev.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
+    launch_fill_desc_rev(b, ctx->order_wide.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
                          ctx->tbW.as<int32_t>(), ctx->desc_rev.as<PairDesc>(), st);
     ++nl;
     {
@@ -673,8 +691,9 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
     tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
     tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream2);
+    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream3, ctx->side_stream2);
     CU(cudaEventRecord(ctx->side_done2, ctx->side_stream2));
+    CU(cudaEventRecord(ctx->side_done3, ctx->side_stream3));
     for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
         tp.first = ctx->mb->tb_bounds[c];
         tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
@@ -686,6 +705,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 
     CU(cudaStreamWaitEvent(st, ctx->side_done, 0));
     CU(cudaStreamWaitEvent(st, ctx->side_done2, 0));
+    CU(cudaStreamWaitEvent(st, ctx->side_done3, 0));
     CU(cudaGetLastError());
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
 

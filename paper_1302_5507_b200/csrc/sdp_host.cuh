@@ -54,18 +54,18 @@ struct PostParams {
     const int32_t* score; const int32_t* ref_end;
     int32_t* tbW;                // gap-content bound W per pair
     int32_t* tb_rows;            // rows the traceback may need: min(i_end, n + W), 0 when W == 0
-    uint32_t* keys_rev;          // bucket key of the reverse pass (wide pairs only, else SKIP)
-    uint32_t* keys_wide;         // bucket key of the traceback DP kernel (wide pairs only, else SKIP)
+    uint32_t* keys_wide;         // bucket key of the reverse pass and the traceback DP kernel (wide pairs only, else SKIP)
     uint32_t* keys_tb;           // bucket key of the one-thread-per-pair traceback (everything else)
     int wide_ok;                 // scoring fits the x8 tagged domain of trace_kernel.cuh
     int no_thin;                 // debugging: keep W >= 1 pairs off the narrow-band kernel
+    int thin_ok;                 // scoring fits the x8 tagged int16 domain of thin_kernel.cu
     int local;                   // SDP_MODE_LOCAL
     const uint32_t* slow_words;  // != 0: the pair went through the int32 lane
     const int32_t* end_col;      // local: read column of the end cell
     uint32_t* err_flag;
     uint32_t* bits_words;        // direction-bit words the pair needs
     uint32_t* ops_cap;           // CIGAR run capacity the pair needs (2W + 1)
-    uint32_t* hist_rev; uint32_t* hist_tb; uint32_t* hist_wide;
+    uint32_t* hist_tb; uint32_t* hist_wide;
     unsigned long long* counters;   // [0] reverse cells, [1] traceback cells, [2] reverse pairs
 };
 void launch_post_forward(const PostParams& pp, cudaStream_t st);
@@ -113,10 +113,11 @@ void launch_forward_i32(const sdp_batch& b, const Scoring& sc, int local, const 
                         int32_t* rows, int32_t* score, int32_t* ref_end, int32_t* end_col, cudaStream_t st);
 // narrow bands (thin_kernel.cu): gap bound W in 0..THIN_NW-1, band rows <= THIN_MAXROWS
 constexpr int THIN_NW = 24;
-constexpr int THIN_SPLIT = 8;             // classes below / from here on run in two launches (register budgets differ)
+constexpr int THIN_SPLIT = 8;             // classes [0, SPLIT), [SPLIT, SPLIT2), [SPLIT2, NW) run in three launches
+constexpr int THIN_SPLIT2 = 16;           // (register budgets differ)
 constexpr uint32_t TB_KEY_STRIDE = 2048;  // traceback bucket key = class * TB_KEY_STRIDE + rows (rows, n < 2048)
 constexpr int THIN_MAXROWS = 336;
-int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st, cudaStream_t st_hi);   // returns kernels launched
+int launch_thin_all(const uint32_t* bounds, const TraceParams& tp, cudaStream_t st, cudaStream_t st_mid, cudaStream_t st_hi);   // returns kernels launched
 void launch_compact(uint64_t n_pairs, const uint64_t* ops_off, const uint32_t* ops_rev, const uint32_t* cigar_len,
                     const uint64_t* cigar_off, uint32_t* cigar_ops, cudaStream_t st);
 

@@ -46,7 +46,7 @@ __global__ void k_post_forward(const PostParams pp)
 {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = p < pp.n_pairs;
-    uint32_t krev = SDP_KEY_SKIP, ktb = SDP_KEY_SKIP, kwide = SDP_KEY_SKIP;
+    uint32_t ktb = SDP_KEY_SKIP, kwide = SDP_KEY_SKIP;
     unsigned long long c_rev = 0, c_tb = 0, n_rev = 0;
     bool too_big = false;
     if (valid) {
@@ -86,7 +86,9 @@ __global__ void k_post_forward(const PostParams pp)
         const long long vmax = (long long)pp.sc.match * n + (long long)pp.sc.gap_extend * (n + rows) +
                                3LL * pp.sc.gap_open + 8;
         if (slow && W == 0) { rows = min(i_end, n); bw = 1; }      // (the dynamic kernel walks a gapless pair through its band too)
-        const bool narrow = !slow && (W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && !pp.no_thin));
+        const int c_shift = 2 * pp.sc.gap_extend + pp.sc.mismatch;
+        const bool thin_fits = pp.thin_ok && vmax + (c_shift > 0 ? c_shift : 0) <= SDP_TB_MAX_VALUE;      // x8 tagged int16 lanes
+        const bool narrow = !slow && (W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && thin_fits && !pp.no_thin));
         const bool wide = !slow && !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
         if (narrow) {
             ktb = (uint32_t)W * TB_KEY_STRIDE + (uint32_t)min((int)TB_KEY_STRIDE - 1, W ? rows : n);
@@ -95,8 +97,7 @@ __global__ void k_post_forward(const PostParams pp)
             // 64 row classes per read length, scaled to the rows a read of this length can need (rows <= 2.5 n),
             // so that the pairs of one warp walk nearly the same number of rows
             const uint32_t rbin = (uint32_t)min(63, (rows * 64) / (5 * n / 2 + 1));
-            krev = (uint32_t)(n - 1) * 64u + rbin;
-            kwide = (uint32_t)(n - 1) * 64u + rbin;
+            kwide = (uint32_t)(n - 1) * 64u + rbin;         // the reverse pass and the traceback DP share this order
             c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
         } else {
             const int cls = slow ? TB_NCLASS - 1 : tb_class_of(bw);
@@ -106,14 +107,12 @@ __global__ void k_post_forward(const PostParams pp)
             c_tb = (unsigned long long)bw * rows;
             ktb = (uint32_t)(THIN_NW + cls) * TB_KEY_STRIDE + (uint32_t)min(bw, (int)TB_KEY_STRIDE - 1);
         }
-        pp.keys_rev[p] = krev;
         pp.keys_wide[p] = kwide;
         pp.keys_tb[p] = ktb;
         pp.bits_words[p] = words;
         pp.ops_cap[p] = 2u * (uint32_t)W + 5u;            // runs of a path with <= W gap bases, + flush slot + two soft clips
         if (too_big) atomicOr(pp.err_flag, SDP_ERRF_RANGE);
     }
-    hist_add(pp.hist_rev, krev, krev != SDP_KEY_SKIP);
     hist_add(pp.hist_tb, ktb, ktb != SDP_KEY_SKIP);
     hist_add(pp.hist_wide, kwide, kwide != SDP_KEY_SKIP);
     for (int o = 16; o > 0; o >>= 1) {
