@@ -226,6 +226,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (configs 1, 3, 4, 5 at full size)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--chunks", type=int, default=0, help="sdp_set_chunks: lanes per call (0 = the library's choice)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -251,6 +252,7 @@ def main():
                           seed=W.SEED_BASE + cfg + 1000 * rank)
     cells = batch.cells
     ctx = S.Context(device=local)
+    ctx.set_chunks(args.chunks)
     dbatch = ctx.upload(batch)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2

@@ -142,11 +142,19 @@ int sdp_create(const sdp_scoring* scoring, int cuda_device, sdp_ctx** out);
 #define SDP_ROUTE_FORCE_G(g) (((uint32_t)(g) & 0x3Fu) << 8)
 int sdp_set_debug_route(sdp_ctx* ctx, uint32_t flags);
 
-/* Align every pair of `batch` (DEVICE pointers). Work is enqueued on `cuda_stream`
- * (a cudaStream_t; NULL = default stream) and the call returns after the stream has completed
- * it (one internal synchronisation, needed to learn n_cigar_ops), so errors are synchronous.
+/* Align every pair of `batch` (DEVICE pointers). The call is ordered after everything already enqueued on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream), runs on the ctx's own streams, and returns after all of it
+ * has completed (the host needs sizes from the device between stages, and n_cigar_ops at the end), so errors are
+ * synchronous and the results are visible to any stream afterwards.
  * On error `out` is untouched. A CIGAR is produced for every pair, passing the filter or not. */
 int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp_result* out);
+
+/* Tuning hook; results never depend on it. A call splits its pair list into `chunks` contiguous ranges ("lanes") that
+ * run the path one after the other through the forward score kernel, while everything a lane does after its forward
+ * pass (bookkeeping, reverse pass, traceback) runs on higher-priority streams under the next lane's forward kernel.
+ * 0 (default) = the library's choice, which is 1 (no pipelining: on B200 the overlap costs the forward kernel more than
+ * it hides); at most 8. SDP_EINVAL outside 0..8. */
+int sdp_set_chunks(sdp_ctx* ctx, int chunks);
 
 /* Same operation with HOST pointers in `batch`: copies the inputs to the device through pinned
  * staging, runs sdp_align_batch's pipeline on an internal stream, and copies every result array

@@ -24,7 +24,7 @@ SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE = 1, 2
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
-           "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_set_mode", "sdp_mate_windows", "sdp_mate_pairs",
+           "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_set_mode", "sdp_set_chunks", "sdp_mate_windows", "sdp_mate_pairs",
            "sdp_proper_pairs"]
 
 
@@ -121,6 +121,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_set_mode.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_set_score_only.restype = ctypes.c_int
     lib.sdp_set_score_only.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    lib.sdp_set_chunks.restype = ctypes.c_int
+    lib.sdp_set_chunks.argtypes = [ctypes.c_void_p, ctypes.c_int]
     lib.sdp_get_stats.restype = ctypes.c_int
     lib.sdp_get_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_stats)]
     lib.sdp_set_timing.restype = ctypes.c_int
@@ -260,6 +262,10 @@ class Context:
     def set_mode(self, local: bool):
         """sdp_set_mode: False = the paper's semi-global formulation (default), True = local / soft-clipping variant."""
         self._check(self._lib.sdp_set_mode(self._h, 1 if local else 0))
+
+    def set_chunks(self, chunks: int):
+        """sdp_set_chunks: lanes one call's pair list is split into (0 = automatic, 1 = no pipelining)."""
+        self._check(self._lib.sdp_set_chunks(self._h, int(chunks)))
 
     def set_score_only(self, enabled: bool):
         self._lib.sdp_set_score_only(self._h, int(bool(enabled)))

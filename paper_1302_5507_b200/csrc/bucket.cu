@@ -275,11 +275,13 @@ __device__ __forceinline__ uint64_t block_exclusive_scan_1024_u64(uint64_t v, ui
     return base + x - v;
 }
 
+// base_in (may be null): the scan starts from *base_in instead of 0, and the total includes it
 __global__ void __launch_bounds__(1024) k_scan_tile_sums(const uint32_t* __restrict__ tile_sums, uint32_t ntiles,
-                                                         uint64_t* __restrict__ tile_base, uint64_t* __restrict__ total_out)
+                                                         uint64_t* __restrict__ tile_base, uint64_t* __restrict__ total_out,
+                                                         const uint64_t* __restrict__ base_in)
 {
     __shared__ uint64_t carry;
-    if (threadIdx.x == 0) carry = 0;
+    if (threadIdx.x == 0) carry = base_in ? *base_in : 0ull;
     __syncthreads();
     for (uint32_t start = 0; start < ntiles; start += 1024) {
         const uint32_t idx = start + threadIdx.x;
@@ -301,13 +303,13 @@ __global__ void k_scan_add(const uint32_t* __restrict__ local, const uint64_t* _
     if (i < n) out[i] = tile_base[i / SCAN_TILE] + local[i];
 }
 
-void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev,
+void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev, const uint64_t* base_dev,
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
                             cudaStream_t st, uint32_t* launches)
 {
     const uint32_t ntiles = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (n) k_scan_tiles<<<ntiles, 1024, 0, st>>>(in, n, tmp_local, tmp_tiles);
-    k_scan_tile_sums<<<1, 1024, 0, st>>>(tmp_tiles, ntiles, tmp_tile_base, total_dev);
+    k_scan_tile_sums<<<1, 1024, 0, st>>>(tmp_tiles, ntiles, tmp_tile_base, total_dev, base_dev);
     if (n) k_scan_add<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(tmp_local, tmp_tile_base, n, out);
     *launches += n ? 3 : 1;
 }

@@ -180,15 +180,18 @@ __device__ __forceinline__ uint32_t reverse_bits16(uint32_t x) { return __brev(x
 struct RingGeom {
     int chunk, ring, stride_w, mirror;
 };
-__device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups, int skew) {
+__device__ __forceinline__ RingGeom ring_geometry(int G, int ngroups, int skew, bool short_chunks = false) {
     RingGeom r;
     r.mirror = skew * (G - 1) > 32 ? 64 : 32;             // (64 only when one group fills the warp)
     if (G == 1)      { r.chunk = 32; r.stride_w = 49; }
     else if (G == 2) { r.chunk = 32; r.stride_w = 50; }
     else {
-        r.chunk = 128;
+        // short_chunks (reverse pass): its early-exit test runs once per chunk. A chunk must still cover the
+        // skew * (G - 1) <= 62 rows the group's last thread trails behind (the ring keeps one chunk of history).
+        r.chunk = short_chunks ? 64 : 128;
         const int want = (32 / ngroups) & 31;             // bank offset between neighbouring groups
-        r.stride_w = 144 + ((want - 144) & 31);           // >= (256 + 32) / 2 words, == want (mod 32)
+        const int base = r.chunk + 16;                    // >= (2 * chunk + 32) / 2 words
+        r.stride_w = base + ((want - base) & 31);         // == want (mod 32)
     }
     r.ring = 2 * r.chunk;
     return r;
@@ -339,7 +342,7 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
 
     // ---- window-row selector ring of this group
     constexpr int SKEW = SDP_SCORE_SKEW;
-    const RingGeom rg = ring_geometry(G, ngroups, SKEW);
+    const RingGeom rg = ring_geometry(G, ngroups, SKEW, REV);
     uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
     const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - SKEW * g;
 
@@ -493,6 +496,9 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
     // window is longer.
     const int lead = SKEW * (G - 1);
     const int fast_end = Mmin + lead, all_end = Mmax + lead;
+    int rows_done = Mmax;
+    // (the exit test adds up to n*match + e*SKEW*G to a stored value: only where that still fits 16 bits)
+    const bool can_exit = REV && 2 * P.c.match * max(nA, nB) + P.c.e * (max(nA, nB) + Mmax + SKEW * G + 2) + P.c.beta <= 32000;
     for (int s0 = 0; s0 < all_end; s0 += rg.chunk) {
         fill_ring(s0);
         __syncwarp();
@@ -520,12 +526,47 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
         for (; s <= fe; ++s, ++rp) row_step1(s - SKEW * g, rp, std::false_type{});
 #pragma unroll 1
         for (; s <= send; ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
+        rows_done = send - lead;
+        if (REV && can_exit && send < all_end) {
+            // Early exit of the reverse pass. The pass looks for the LAST row whose M(i,n) equals the forward score S
+            // (dA.aux), so it may stop as soon as no later row can reach S. Any path to a later cell of column n leaves
+            // the cells computed so far through a cell on their staircase frontier -- a thread's current row, the cell left
+            // of it that the thread's next row takes as its diagonal neighbour, the last column of one of its two most
+            // recent rows (the right neighbour trails by SKEW rows), or the closed-form boundary column 0 -- and gains at
+            // most `match` per read base it still has to consume:
+            //     M(i2, n) <= max over frontier cells (i,j) of  M(i,j) + (n - j) * match.
+            // In drift form (stored X' = X + e(i+j) + beta, this thread at row s - SKEW*g):
+            //     alive  <=>  X' + (n-j)*match - e*j + e*SKEW*g  >=  S + beta + e*s.
+            const int M = P.c.match, e = P.c.e;
+            const int jA = startA + 1, jB = startB + 1;             // 1-based column of H[0]
+            uint32_t c = sdp_pack_lo_hi((nA - jA) * M - e * jA + e * SKEW * g, (nB - jB) * M - e * jB + e * SKEW * g);
+            const uint32_t dstep = sdp_pack2(-(M + e));
+            uint32_t acc = 0x80008000u;
+#pragma unroll
+            for (int k = 0; k < K; ++k) { acc = __viaddmax_s16x2(H[k], c, acc); c = __vadd2(c, dstep); }
+            {   // the lane's true last column, one row back: one more e of allowance covers both rows in flight
+                const int lA = startA + realA, lB = startB + realB;
+                const uint32_t cl = sdp_pack_lo_hi((nA - lA) * M - e * lA + e * SKEW * g + e, (nB - lB) * M - e * lB + e * SKEW * g + e);
+                acc = __viaddmax_s16x2(houtA, cl, acc);
+                if (SKEW == 2) acc = __viaddmax_s16x2(houtB, cl, acc);
+            }
+            if (is_first) acc = __viaddmax_s16x2(fv, sdp_pack_lo_hi(nA * M, nB * M), acc);   // boundary column 0
+            else {
+                // the diagonal neighbour of this thread's next cell: M(current row, column left of H[0]), still to be used
+                acc = __viaddmax_s16x2(hdiag, sdp_pack_lo_hi((nA - jA + 1) * M - e * (jA - 1) + e * SKEW * g,
+                                                             (nB - jB + 1) * M - e * (jB - 1) + e * SKEW * g), acc);
+            }
+            const int tA = dA.aux + P.c.beta + e * send, tB = dB.aux + P.c.beta + e * send;
+            const bool alive = (hasA && (int)(int16_t)(acc & 0xFFFFu) >= tA) || (hasB && (int)(int16_t)(acc >> 16) >= tB);
+            if (!__any_sync(0xffffffffu, alive)) break;
+        }
     }
 
     if (is_last) {
-        // best = H'(idx,n) + e*(Mmax - idx) = H(idx,n) + e*(n + Mmax) + beta
+        // best = H'(idx,n) + e*(rows_done - idx) = H(idx,n) + e*(n + rows_done) + beta, rows_done = rows this thread
+        // went through (Mmax unless the reverse pass stopped early)
         const int bA = (int)(int16_t)(best & 0xFFFFu), bB = (int)(int16_t)(best >> 16);
-        const int sA = bA - P.c.beta - P.c.e * (nA + Mmax), sB = bB - P.c.beta - P.c.e * (nB + Mmax);
+        const int sA = bA - P.c.beta - P.c.e * (nA + rows_done), sB = bB - P.c.beta - P.c.e * (nB + rows_done);
         if (REV) {
             // idx = rows of the reversed window consumed by the longest alignment scoring S;
             // the lowest co-optimal start is s_lo = ref_end + 1 - idx

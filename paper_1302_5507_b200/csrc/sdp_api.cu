@@ -37,8 +37,8 @@ struct DevBuf {
 };
 
 struct Mailbox {                    // pinned host memory the device results land in
-    uint32_t task_prefix[3][SDP_NSLOTS + 1];   // forward, reverse, traceback DP
-    uint32_t bin_total[4];                     // forward, reverse, thin traceback, wide traceback
+    uint32_t task_prefix[3][SDP_NSLOTS + 1];   // forward, (unused), traceback DP + reverse pass
+    uint32_t bin_total[4];                     // forward, (unused), thin traceback, wide traceback
     uint32_t tb_bounds[THIN_NW + TB_NCLASS + 1];   // narrow-band launches (one per W), then the generic band classes
     uint32_t err_flag;
     uint64_t totals[4];             // [0] thin direction-bit words, [1] run capacity, [2] CIGAR runs, [3] wide nibble words
@@ -48,8 +48,44 @@ struct Mailbox {                    // pinned host memory the device results lan
 };
 
 constexpr int SDP_FAN_STREAMS = 4;
+constexpr int SDP_MAX_LANES = 8;
 
-enum { EV_START, EV_BUCKET, EV_FORWARD, EV_REVERSE, EV_TRACE, EV_END, EV_COUNT };
+enum { LEV_A0, LEV_A1, LEV_F0, LEV_F1, LEV_REV, LEV_TRACE, LEV_END, LEV_COUNT };
+
+// One chunk of a call's pair list (a "lane"): a contiguous range of caller pairs that runs the whole path a1..a7 with
+// its own scratch. Lanes are software-pipelined (sdp_align_batch): all forward kernels go back to back on one
+// low-priority stream, and everything a lane does after its forward pass -- latency-bound bookkeeping, two host
+// round trips, the reverse pass and the traceback kernels -- runs on higher-priority streams UNDER the next lane's
+// forward kernel instead of after it.
+struct Lane {
+    Mailbox* mb = nullptr;
+    cudaStream_t st = nullptr;       // this lane's stream (high priority): everything but the forward kernels
+    cudaEvent_t evA = nullptr, evB = nullptr, evC = nullptr, evD = nullptr;   // end of the four phases
+    cudaEvent_t ev_desc = nullptr, ev_fwd = nullptr;
+    cudaEvent_t fan_fork = nullptr, fan_join[SDP_FAN_STREAMS] = {};
+    cudaEvent_t side_done[3] = {};
+    cudaEvent_t tev[LEV_COUNT] = {};
+    // what every call starts from zero sits in ONE block (one memset): counters, err_flag, the three histograms
+    void* zero_block = nullptr; size_t zero_bytes = 0;
+    uint32_t* hist[4] = {};          // forward, (unused), thin traceback, wide traceback + reverse pass
+    uint32_t* bin_start[4] = {};
+    SlotInfo* slots[3] = {};         // forward, (unused), wide traceback + reverse pass
+    uint32_t* task_prefix[3] = {};
+    uint32_t* err_flag = nullptr;
+    unsigned long long* counters = nullptr;
+    uint64_t* totals = nullptr;
+    // per-pair device buffers (grow only), indexed by the pair's position inside the lane
+    DevBuf keys, pn, pm, order, desc, desc_rev, order_tb, keys_tb, tbW, rev_rows,
+        tb_rows, keys_wide, order_wide, desc_wide, wide_words, wide_off, wide_bits,
+        bits_words, ops_cap, bits_off, ops_off, bits, ops_rev;
+    DevBuf scan_local[3], scan_tiles[3], scan_tile_base[3];   // one set per concurrent scan
+    DevBuf slow_words, slow_off, slow_rows;   // int32 lane (slow_lane.cu): per-pair row-array words, their offsets, the arrays
+    // this call
+    uint64_t p0 = 0, P = 0;          // caller pair range [p0, p0 + P)
+    sdp_batch b{};                   // the caller's batch restricted to that range
+    uint32_t nl = 0, fwd_launches = 0;
+    uint32_t n_wide = 0;
+};
 
 }  // namespace
 
@@ -70,46 +106,30 @@ struct sdp_ctx {
     bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
     bool score_only = false;         // sdp_set_score_only: stop after the forward pass
     int mode = SDP_MODE_SEMIGLOBAL;  // sdp_set_mode
+    int chunks = 0;                  // sdp_set_chunks: lanes per call, 0 = chosen from the pair count
     sdp_stats stats{};
     uint16_t h_slot_n[SDP_NSLOTS], h_slot_G[SDP_NSLOTS], h_slot_K[SDP_NSLOTS];
     uint32_t cls_begin[2 * SDP_MAX_K + 3];   // first slot of class c = 2K + padded; [c+1] ends it
     uint16_t h_slot_of_n[SDP_NSLOTS];        // read length - 1 -> slot
     uint16_t *d_slot_n = nullptr, *d_slot_G = nullptr, *d_slot_K = nullptr, *d_slot_of_n = nullptr;
-    Mailbox* mb = nullptr;
-    cudaStream_t own_stream = nullptr;
-    cudaStream_t side_stream = nullptr;   // narrow-band traceback runs here, beside the wide path on the caller's stream
-    cudaEvent_t side_done = nullptr;
-    cudaStream_t fan_stream[SDP_FAN_STREAMS] = {};   // [0] unused: the caller's stream takes that turn
-    cudaEvent_t fan_fork = nullptr, fan_join[SDP_FAN_STREAMS] = {};
-    cudaStream_t side_stream2 = nullptr;  // the wider narrow bands (W >= THIN_SPLIT): few, long-running blocks
-    cudaEvent_t side_done2 = nullptr;
-    cudaStream_t side_stream3 = nullptr;  // the middle band widths (THIN_SPLIT <= W < THIN_SPLIT2)
-    cudaEvent_t side_done3 = nullptr;
-    cudaEvent_t ev[EV_COUNT] = {};
-    // fixed-size device buffers
-    // what every call starts from zero sits in ONE block (one memset): counters, err_flag, the three histograms
-    void* zero_block = nullptr; size_t zero_bytes = 0;
-    uint32_t* hist[4] = {};          // forward, (unused), thin traceback, wide traceback + reverse pass
-    uint32_t* bin_start[4] = {};
-    SlotInfo* slots[3] = {};         // forward, (unused), wide traceback + reverse pass
-    uint32_t* task_prefix[3] = {};
-    uint32_t* err_flag = nullptr;
-    unsigned long long* counters = nullptr;
-    uint64_t* totals = nullptr;
-    // per-pair device buffers (grow only)
-    DevBuf keys, pn, pm, order, desc, desc_rev, order_tb, keys_tb, tbW, rev_rows,
-        tb_rows, keys_wide, order_wide, desc_wide, wide_words, wide_off, wide_bits,
-        bits_words, ops_cap, bits_off, ops_off,
-        score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len,
-        bits, ops_rev, cigar_ops;
-    DevBuf scan_local[3], scan_tiles[3], scan_tile_base[3];   // one set per concurrent scan
+    int prio_lo = 0, prio_hi = 0;
+    Lane lane[SDP_MAX_LANES];
+    int lanes_ready = 0;                  // lanes whose streams, events and fixed-size buffers exist
+    cudaStream_t own_stream = nullptr;    // sdp_align_batch_host
+    cudaStream_t fwd_stream = nullptr;    // every lane's forward score kernels, lowest priority
+    cudaStream_t fan_fwd[SDP_FAN_STREAMS] = {};    // [0] unused; forward / reverse / trace launches of several K classes
+    cudaStream_t fan_post[SDP_FAN_STREAMS] = {};   // [0] unused; the short sort and scan chains after the forward pass
+    cudaStream_t side_stream[3] = {};     // narrow-band traceback (three register classes), beside the wide path
+    cudaEvent_t ev_start = nullptr, ev_end = nullptr, ev_cig[SDP_MAX_LANES] = {};
+    uint64_t* cig_total = nullptr;        // [SDP_MAX_LANES + 1] running CIGAR run totals across lanes; [0] = 0
+    // results, caller pair order, shared by the lanes
+    DevBuf score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len, cigar_ops;
     // sdp_align_batch_host: device copies of the inputs and pinned host copies of the outputs
     DevBuf in_reads, in_read_off, in_read_len, in_read_nmask, in_wins, in_win_off, in_win_len, in_win_nmask, in_pairs;
     DevBuf h_out;                    // one pinned slab, carved per call
     // sdp_best_per_read
     DevBuf rb_key, rb_pair, rb_score, rb_second, rb_ncand;
     DevBuf mp_flag, mp_off;          // sdp_mate_pairs
-    DevBuf slow_words, slow_off, slow_rows;   // int32 lane (slow_lane.cu): per-pair row-array words, their offsets, the arrays
     const uint32_t* last_pairs = nullptr;   // pair list of the last successful align call (to match results to it)
     uint64_t last_n_pairs = 0;
     uint32_t last_n_reads = 0;
@@ -157,6 +177,70 @@ int ensure_pinned(sdp_ctx* ctx, DevBuf& b, size_t bytes) {
         int rc_ = ensure(ctx, ctx->buf, (size_t)(bytes));      \
         if (rc_ != SDP_OK) return rc_;                         \
     } while (0)
+#define LEN(buf, bytes)                                        \
+    do {                                                       \
+        int rc_ = ensure(ctx, L.buf, (size_t)(bytes));         \
+        if (rc_ != SDP_OK) return rc_;                         \
+    } while (0)
+
+// streams, events and fixed-size buffers of lanes [ctx->lanes_ready, want)
+int lanes_init(sdp_ctx* ctx, int want)
+{
+    for (int li = ctx->lanes_ready; li < want; ++li) {
+        Lane& L = ctx->lane[li];
+        CU(cudaMallocHost(&L.mb, sizeof(Mailbox)));
+        memset(L.mb, 0, sizeof(Mailbox));
+        CU(cudaStreamCreateWithPriority(&L.st, cudaStreamNonBlocking, ctx->prio_hi));
+        cudaEvent_t* evs[] = {&L.evA, &L.evB, &L.evC, &L.evD, &L.ev_desc, &L.ev_fwd, &L.fan_fork, &L.side_done[0],
+                              &L.side_done[1], &L.side_done[2]};
+        for (cudaEvent_t* e : evs) CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+        for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaEventCreateWithFlags(&L.fan_join[k], cudaEventDisableTiming));
+        for (int k = 0; k < LEV_COUNT; ++k) CU(cudaEventCreate(&L.tev[k]));
+        {
+            const size_t hist_words = ((SDP_NBINS + 1 + 3) / 4) * 4;
+            L.zero_bytes = 8 * 8 + 16 + 3 * hist_words * 4;
+            CU(cudaMalloc(&L.zero_block, L.zero_bytes));
+            char* z = (char*)L.zero_block;
+            L.counters = (unsigned long long*)z;
+            L.err_flag = (uint32_t*)(z + 64);
+            uint32_t* h = (uint32_t*)(z + 80);
+            L.hist[0] = h; L.hist[2] = h + hist_words; L.hist[3] = h + 2 * hist_words;
+        }
+        for (int i = 0; i < 4; ++i) {
+            if (i == 1) continue;
+            CU(cudaMalloc(&L.bin_start[i], (SDP_NBINS + 4 + SDP_BIN_SCRATCH) * 4));
+        }
+        for (int i = 0; i < 3; ++i) {
+            if (i == 1) continue;
+            CU(cudaMalloc(&L.slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
+            CU(cudaMalloc(&L.task_prefix[i], (SDP_NSLOTS + 1) * 4));
+        }
+        CU(cudaMalloc(&L.totals, 4 * 8));
+        ctx->lanes_ready = li + 1;
+    }
+    return SDP_OK;
+}
+
+void lane_destroy(Lane& L)
+{
+    DevBuf* bufs[] = {&L.keys, &L.pn, &L.pm, &L.order, &L.desc, &L.desc_rev, &L.order_tb, &L.keys_tb, &L.tbW, &L.rev_rows,
+                      &L.tb_rows, &L.keys_wide, &L.order_wide, &L.desc_wide, &L.wide_words, &L.wide_off, &L.wide_bits,
+                      &L.bits_words, &L.ops_cap, &L.bits_off, &L.ops_off, &L.bits, &L.ops_rev, &L.scan_local[0],
+                      &L.scan_local[1], &L.scan_local[2], &L.scan_tiles[0], &L.scan_tiles[1], &L.scan_tiles[2],
+                      &L.scan_tile_base[0], &L.scan_tile_base[1], &L.scan_tile_base[2], &L.slow_words, &L.slow_off,
+                      &L.slow_rows};
+    for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
+    for (int i = 0; i < 4; ++i) cudaFree(L.bin_start[i]);
+    for (int i = 0; i < 3; ++i) { cudaFree(L.slots[i]); cudaFree(L.task_prefix[i]); }
+    cudaFree(L.zero_block); cudaFree(L.totals);
+    if (L.mb) cudaFreeHost(L.mb);
+    if (L.st) cudaStreamDestroy(L.st);
+    cudaEvent_t evs[] = {L.evA, L.evB, L.evC, L.evD, L.ev_desc, L.ev_fwd, L.fan_fork, L.side_done[0], L.side_done[1],
+                         L.side_done[2]};
+    for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e);
+    for (int k = 1; k < SDP_FAN_STREAMS; ++k) if (L.fan_join[k]) cudaEventDestroy(L.fan_join[k]);
+    for (int k = 0; k < LEV_COUNT; ++k) if (L.tev[k]) cudaEventDestroy(L.tev[k]);
+}
 
 // (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. A warp runs 2*floor(32/G) pairs
 // for (m + G - 1) steps, and a step costs what the (K, padded) kernel variant was MEASURED to cost on B200
@@ -233,7 +317,7 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         score_modules_init(&ctx->modules);
         ctx->consts.beta2 = sdp_pack2(beta_s);
         ctx->consts.betaMinusO2 = sdp_pack2(beta_s - o);
-        ctx->consts.e = e; ctx->consts.beta = beta_s;
+        ctx->consts.e = e; ctx->consts.beta = beta_s; ctx->consts.match = s->match;
     }
     {   // traceback DP kernel: x8 scaled values with tags in the low three bits (trace_kernel.cuh)
         const int sc8 = SDP_TB_SCALE;
@@ -268,44 +352,25 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaMemcpy(ctx->d_slot_K, ctx->h_slot_K, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
         CU(cudaMalloc(&ctx->d_slot_of_n, SDP_NSLOTS * 2));
         CU(cudaMemcpy(ctx->d_slot_of_n, ctx->h_slot_of_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
-        CU(cudaMallocHost(&ctx->mb, sizeof(Mailbox)));
-        memset(ctx->mb, 0, sizeof(Mailbox));
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
-        int prio_lo = 0, prio_hi = 0;                 // narrow-band work fills the gaps of the (critical) wide path
-        CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
-        CU(cudaStreamCreateWithPriority(&ctx->side_stream, cudaStreamNonBlocking, prio_lo));
-        CU(cudaEventCreateWithFlags(&ctx->side_done, cudaEventDisableTiming));
-        CU(cudaStreamCreateWithPriority(&ctx->side_stream2, cudaStreamNonBlocking, prio_lo));
-        CU(cudaStreamCreateWithPriority(&ctx->side_stream3, cudaStreamNonBlocking, prio_lo));
-        CU(cudaEventCreateWithFlags(&ctx->side_done3, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&ctx->fan_fork, cudaEventDisableTiming));
+        // Three priority levels (numerically lower = higher priority): the forward kernels of all lanes at the lowest,
+        // the narrow-band traceback kernels in the middle, each lane's own stream (bookkeeping, reverse pass, wide
+        // traceback: the lane's critical path) at the highest, so that a lane's tail runs under the next lane's
+        // forward kernel instead of queueing behind its thousands of CTAs.
+        CU(cudaDeviceGetStreamPriorityRange(&ctx->prio_lo, &ctx->prio_hi));
+        const int prio_mid = (ctx->prio_lo + ctx->prio_hi) / 2;
+        CU(cudaStreamCreateWithPriority(&ctx->fwd_stream, cudaStreamNonBlocking, ctx->prio_lo));
+        for (int k = 0; k < 3; ++k) CU(cudaStreamCreateWithPriority(&ctx->side_stream[k], cudaStreamNonBlocking, prio_mid));
         for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
-            CU(cudaStreamCreateWithFlags(&ctx->fan_stream[k], cudaStreamNonBlocking));
-            CU(cudaEventCreateWithFlags(&ctx->fan_join[k], cudaEventDisableTiming));
+            CU(cudaStreamCreateWithPriority(&ctx->fan_fwd[k], cudaStreamNonBlocking, ctx->prio_lo));
+            CU(cudaStreamCreateWithPriority(&ctx->fan_post[k], cudaStreamNonBlocking, ctx->prio_hi));
         }
-        CU(cudaEventCreateWithFlags(&ctx->side_done2, cudaEventDisableTiming));
-        for (int i = 0; i < EV_COUNT; ++i) CU(cudaEventCreate(&ctx->ev[i]));
-        {
-            const size_t hist_words = ((SDP_NBINS + 1 + 3) / 4) * 4;
-            ctx->zero_bytes = 8 * 8 + 16 + 3 * hist_words * 4;
-            CU(cudaMalloc(&ctx->zero_block, ctx->zero_bytes));
-            char* z = (char*)ctx->zero_block;
-            ctx->counters = (unsigned long long*)z;
-            ctx->err_flag = (uint32_t*)(z + 64);
-            uint32_t* h = (uint32_t*)(z + 80);
-            ctx->hist[0] = h; ctx->hist[2] = h + hist_words; ctx->hist[3] = h + 2 * hist_words;
-        }
-        for (int i = 0; i < 4; ++i) {
-            if (i == 1) continue;
-            CU(cudaMalloc(&ctx->bin_start[i], (SDP_NBINS + 4 + SDP_BIN_SCRATCH) * 4));
-        }
-        for (int i = 0; i < 3; ++i) {
-            if (i == 1) continue;
-            CU(cudaMalloc(&ctx->slots[i], SDP_NSLOTS * sizeof(SlotInfo)));
-            CU(cudaMalloc(&ctx->task_prefix[i], (SDP_NSLOTS + 1) * 4));
-        }
-        CU(cudaMalloc(&ctx->totals, 4 * 8));
-        return SDP_OK;
+        CU(cudaEventCreate(&ctx->ev_start));
+        CU(cudaEventCreate(&ctx->ev_end));
+        for (int k = 0; k < SDP_MAX_LANES; ++k) CU(cudaEventCreateWithFlags(&ctx->ev_cig[k], cudaEventDisableTiming));
+        CU(cudaMalloc(&ctx->cig_total, (SDP_MAX_LANES + 1) * 8));
+        CU(cudaMemset(ctx->cig_total, 0, (SDP_MAX_LANES + 1) * 8));
+        return lanes_init(ctx, 1);
     };
     int rc = init();
     if (rc != SDP_OK) { sdp_destroy(ctx); return rc; }
@@ -317,38 +382,28 @@ void sdp_destroy(sdp_ctx* ctx)
 {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
     score_modules_destroy(&ctx->modules);
-    DevBuf* bufs[] = {&ctx->keys, &ctx->pn, &ctx->pm, &ctx->order, &ctx->desc, &ctx->desc_rev,
-                      &ctx->order_tb, &ctx->keys_tb, &ctx->tbW, &ctx->rev_rows, &ctx->bits_words,
-                      &ctx->ops_cap, &ctx->bits_off, &ctx->ops_off, &ctx->scan_local[0], &ctx->scan_local[1], &ctx->scan_local[2],
-                      &ctx->scan_tiles[0], &ctx->scan_tiles[1], &ctx->scan_tiles[2], &ctx->scan_tile_base[0],
-                      &ctx->scan_tile_base[1], &ctx->scan_tile_base[2], &ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start,
-                      &ctx->read_end, &ctx->pass, &ctx->n_match, &ctx->n_cols, &ctx->cigar_off, &ctx->cigar_len,
-                      &ctx->bits, &ctx->ops_rev, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
+    for (int li = 0; li < SDP_MAX_LANES; ++li) if (ctx->lane[li].mb) lane_destroy(ctx->lane[li]);
+    DevBuf* bufs[] = {&ctx->score, &ctx->ref_start, &ctx->ref_end, &ctx->read_start, &ctx->read_end, &ctx->pass, &ctx->n_match,
+                      &ctx->n_cols, &ctx->cigar_off, &ctx->cigar_len, &ctx->cigar_ops, &ctx->in_reads, &ctx->in_read_off,
                       &ctx->in_read_len, &ctx->in_read_nmask, &ctx->in_wins, &ctx->in_win_off, &ctx->in_win_len,
-                      &ctx->in_win_nmask, &ctx->in_pairs, &ctx->tb_rows, &ctx->keys_wide, &ctx->order_wide,
-                      &ctx->desc_wide, &ctx->wide_words, &ctx->wide_off, &ctx->wide_bits,
-                      &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second, &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off, &ctx->slow_words, &ctx->slow_off, &ctx->slow_rows};
+                      &ctx->in_win_nmask, &ctx->in_pairs, &ctx->rb_key, &ctx->rb_pair, &ctx->rb_score, &ctx->rb_second,
+                      &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
-    for (int i = 0; i < 4; ++i) cudaFree(ctx->bin_start[i]);
-    for (int i = 0; i < 3; ++i) { cudaFree(ctx->slots[i]); cudaFree(ctx->task_prefix[i]); }
-    cudaFree(ctx->zero_block); cudaFree(ctx->totals);
+    cudaFree(ctx->cig_total);
     cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K); cudaFree(ctx->d_slot_of_n);
-    if (ctx->mb) cudaFreeHost(ctx->mb);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
-    if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
-    if (ctx->side_done) cudaEventDestroy(ctx->side_done);
-    if (ctx->side_stream2) cudaStreamDestroy(ctx->side_stream2);
-    if (ctx->side_stream3) cudaStreamDestroy(ctx->side_stream3);
-    if (ctx->side_done3) cudaEventDestroy(ctx->side_done3);
-    if (ctx->fan_fork) cudaEventDestroy(ctx->fan_fork);
+    if (ctx->fwd_stream) cudaStreamDestroy(ctx->fwd_stream);
+    for (int k = 0; k < 3; ++k) if (ctx->side_stream[k]) cudaStreamDestroy(ctx->side_stream[k]);
     for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
-        if (ctx->fan_stream[k]) cudaStreamDestroy(ctx->fan_stream[k]);
-        if (ctx->fan_join[k]) cudaEventDestroy(ctx->fan_join[k]);
+        if (ctx->fan_fwd[k]) cudaStreamDestroy(ctx->fan_fwd[k]);
+        if (ctx->fan_post[k]) cudaStreamDestroy(ctx->fan_post[k]);
     }
-    if (ctx->side_done2) cudaEventDestroy(ctx->side_done2);
-    for (int i = 0; i < EV_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
+    if (ctx->ev_end) cudaEventDestroy(ctx->ev_end);
+    for (int k = 0; k < SDP_MAX_LANES; ++k) if (ctx->ev_cig[k]) cudaEventDestroy(ctx->ev_cig[k]);
     delete ctx;
 }
 
@@ -411,37 +466,46 @@ int sdp_measure_dpx_rate(int cuda_device, double* rate, int32_t* sms, double* mh
     return measure_dpx_rate(cuda_device, rate, sms, mhz);
 }
 
-// which: 0 forward, 1 reverse, 2 traceback DP (trace_kernel)
-static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const PairDesc* desc,
-                              cudaStream_t st, uint32_t* nlaunch)
+int sdp_set_chunks(sdp_ctx* ctx, int chunks)
+{
+    if (!ctx) return SDP_EINVAL;
+    ctx->err[0] = 0;
+    if (chunks < 0 || chunks > SDP_MAX_LANES) return fail(ctx, SDP_EINVAL, "chunks must be 0 (automatic) .. %d", SDP_MAX_LANES);
+    ctx->chunks = chunks;
+    return SDP_OK;
+}
+
+// which: 0 forward, 1 reverse, 2 traceback DP (trace_kernel). Launches on `st`; with several column-count classes
+// (mixed read lengths) the launches go round-robin over `st` and the helper streams fan[1..], forked from and
+// joined back into `st` with the lane's events, so that one class's tail overlaps the next class's start.
+static int launch_score_stage(sdp_ctx* ctx, Lane& L, int which, const PairDesc* desc, cudaStream_t st,
+                              cudaStream_t* fan, uint32_t* nlaunch)
 {
     const bool rev = which == 1;
     const int ti = which == 0 ? 0 : 2;                    // task table: the reverse pass runs on the wide-traceback buckets
+    const sdp_batch& b = L.b;
     TraceDP td{};
-    td.c = ctx->tconsts; td.bits = ctx->wide_bits.as<uint32_t>(); td.bits_off = ctx->wide_off.as<uint64_t>();
-    const uint32_t* tp = ctx->mb->task_prefix[ti];
+    td.c = ctx->tconsts; td.bits = L.wide_bits.as<uint32_t>(); td.bits_off = L.wide_off.as<uint64_t>();
+    const uint32_t* tp = L.mb->task_prefix[ti];
     ScoreParams sp{};
     sp.reads_packed = b.reads_packed; sp.read_nmask = b.read_nmask;
     sp.wins_packed = b.wins_packed; sp.win_nmask = b.win_nmask;
     sp.wins_words = (b.wins_bases + 15) / 16; sp.win_nmask_words = (b.wins_bases + 31) / 32;
     sp.desc = desc;
-    sp.task_prefix = ctx->task_prefix[ti];
-    sp.slots = ctx->slots[ti];
+    sp.task_prefix = L.task_prefix[ti];
+    sp.slots = L.slots[ti];
     sp.c = ctx->consts;
-    sp.score = ctx->score.as<int32_t>(); sp.ref_end = ctx->ref_end.as<int32_t>();
-    sp.rev_rows = ctx->rev_rows.as<int32_t>(); sp.err_flag = ctx->err_flag;
-    // One launch per column-count class in use. With several classes (mixed read lengths) the launches go
-    // round-robin over the caller's stream and SDP_FAN_STREAMS - 1 helper streams, forked from and joined
-    // back into the caller's stream with events, so that one class's tail overlaps the next class's start.
+    sp.score = ctx->score.as<int32_t>() + L.p0; sp.ref_end = ctx->ref_end.as<int32_t>() + L.p0;
+    sp.rev_rows = L.rev_rows.as<int32_t>(); sp.err_flag = L.err_flag;
     int classes = 0;
     for (int cls = 2; cls <= 2 * SDP_MAX_K + 1; ++cls) {
         const uint32_t s0 = ctx->cls_begin[cls], s1 = ctx->cls_begin[cls + 1];
         if (s1 > s0 && tp[s1] > tp[s0]) ++classes;
     }
-    const bool fan = classes > 1;
-    if (fan) {
-        CU(cudaEventRecord(ctx->fan_fork, st));
-        for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_stream[k], ctx->fan_fork, 0));
+    const bool do_fan = classes > 1;
+    if (do_fan) {
+        CU(cudaEventRecord(L.fan_fork, st));
+        for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(fan[k], L.fan_fork, 0));
     }
     int turn = 0;
     for (int cls = 2 * SDP_MAX_K + 1; cls >= 2; --cls) {                 // largest K (longest reads) first
@@ -450,7 +514,7 @@ static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const
         const uint32_t t0 = tp[s0], t1 = tp[s1];
         if (t1 <= t0) continue;
         sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
-        cudaStream_t ls = (fan && (turn % SDP_FAN_STREAMS)) ? ctx->fan_stream[turn % SDP_FAN_STREAMS] : st;
+        cudaStream_t ls = (do_fan && (turn % SDP_FAN_STREAMS)) ? fan[turn % SDP_FAN_STREAMS] : st;
         ++turn;
         if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, ls);
         else {
@@ -460,15 +524,257 @@ static int launch_score_stage(sdp_ctx* ctx, int which, const sdp_batch& b, const
         }
         ++*nlaunch;
     }
-    if (fan) {
+    if (do_fan) {
         for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
-            CU(cudaEventRecord(ctx->fan_join[k], ctx->fan_stream[k]));
-            CU(cudaStreamWaitEvent(st, ctx->fan_join[k], 0));
+            CU(cudaEventRecord(L.fan_join[k], fan[k]));
+            CU(cudaStreamWaitEvent(st, L.fan_join[k], 0));
         }
     }
     CU(cudaGetLastError());
     return SDP_OK;
 }
+
+namespace {
+
+// wait until nothing of this ctx is in flight any more (error paths: a later call must not meet leftover work)
+void drain(sdp_ctx* ctx)
+{
+    cudaStreamSynchronize(ctx->fwd_stream);
+    for (int k = 0; k < 3; ++k) cudaStreamSynchronize(ctx->side_stream[k]);
+    for (int k = 1; k < SDP_FAN_STREAMS; ++k) { cudaStreamSynchronize(ctx->fan_fwd[k]); cudaStreamSynchronize(ctx->fan_post[k]); }
+    for (int li = 0; li < ctx->lanes_ready; ++li) cudaStreamSynchronize(ctx->lane[li].st);
+}
+
+// ---- phase A: a1 + a2 of one lane (validate, key, histogram, scan, scatter, task table), enqueued on the lane's stream
+int lane_phase_a(sdp_ctx* ctx, Lane& L, const int local)
+{
+    const sdp_batch& b = L.b;
+    const uint64_t P = L.P;
+    const size_t Pp = (size_t)(P ? P : 1);
+    LEN(keys, Pp * 4); LEN(pn, Pp * 4); LEN(pm, Pp * 4); LEN(order, Pp * 4); LEN(desc, Pp * sizeof(PairDesc));
+    LEN(desc_rev, Pp * sizeof(PairDesc)); LEN(order_tb, Pp * 4);
+    LEN(keys_tb, Pp * 4); LEN(tbW, Pp * 4); LEN(rev_rows, Pp * 4);
+    LEN(tb_rows, Pp * 4); LEN(keys_wide, Pp * 4); LEN(order_wide, Pp * 4); LEN(desc_wide, Pp * sizeof(PairDesc));
+    LEN(wide_words, Pp * 4); LEN(wide_off, Pp * 8);
+    LEN(bits_words, Pp * 4); LEN(ops_cap, Pp * 4); LEN(bits_off, Pp * 8); LEN(ops_off, Pp * 8);
+    for (int k = 0; k < 3; ++k) { LEN(scan_local[k], Pp * 4); LEN(scan_tiles[k], (Pp / 4096 + 2) * 4); LEN(scan_tile_base[k], (Pp / 4096 + 2) * 8); }
+    LEN(slow_words, Pp * 4); LEN(slow_off, Pp * 8);
+    cudaStream_t st = L.st;
+    L.nl = 0; L.fwd_launches = 0; L.n_wide = 0;
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A0], st));
+    CU(cudaMemsetAsync(L.zero_block, 0, L.zero_bytes, st));
+    launch_validate_key(b, ctx->sc, L.keys.as<uint32_t>(), L.pn.as<uint32_t>(), L.pm.as<uint32_t>(),
+                        L.hist[0], L.err_flag, L.counters + 3, (ctx->prefilter && !local) ? 1 : 0,
+                        ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0, L.counters + 4, local,
+                        L.slow_words.as<uint32_t>(), st);
+    // row arrays of the int32 lane: offsets now, so that the arrays can be allocated after the host has seen the total
+    exclusive_scan_u32_u64(L.slow_words.as<uint32_t>(), P, L.slow_off.as<uint64_t>(), L.totals + 0, nullptr,
+                           L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
+                           L.scan_tile_base[0].as<uint64_t>(), st, &L.nl);
+    CU(cudaMemcpyAsync(&L.mb->slow_total, L.totals + 0, 8, cudaMemcpyDeviceToHost, st));
+    launch_sort_tail(L.keys.as<uint32_t>(), P, L.hist[0], L.bin_start[0], L.order.as<uint32_t>(),
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, L.slots[0], L.task_prefix[0],
+                     L.mb->task_prefix[0], &L.mb->bin_total[0], st);
+    L.nl += 5;
+    CU(cudaMemcpyAsync(&L.mb->err_flag, L.err_flag, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaEventRecord(L.evA, st));
+    return SDP_OK;
+}
+
+// ---- phase B: a3 on the shared forward stream, then (on the lane's stream) the gap bound W, the keys of the later
+// stages, their bucket sorts and the scratch-size scans
+int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
+{
+    const sdp_batch& b = L.b;
+    const uint64_t P = L.P;
+    cudaStream_t st = L.st, fs = ctx->fwd_stream;
+    // (with the ungapped pre-pass on, fewer than P pairs are in the forward buckets)
+    launch_fill_desc_fwd(b, L.order.as<uint32_t>(), L.mb->bin_total[0], L.desc.as<PairDesc>(), st);
+    ++L.nl;
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A1], st));
+    CU(cudaEventRecord(L.ev_desc, st));
+    CU(cudaStreamWaitEvent(fs, L.ev_desc, 0));
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_F0], fs));
+    {
+        uint32_t before = L.nl;
+        int rc = launch_score_stage(ctx, L, 0, L.desc.as<PairDesc>(), fs, ctx->fan_fwd, &L.nl);
+        if (rc != SDP_OK) return rc;
+        L.fwd_launches = L.nl - before;
+    }
+    if (L.mb->slow_total) {
+        // the int32 lane: pairs outside the int16 kernels' domain, and every pair in local mode (slow_lane.cu)
+        LEN(slow_rows, (L.mb->slow_total + 4) * 4);
+        launch_forward_i32(b, ctx->sc, local, L.slow_words.as<uint32_t>(), L.slow_off.as<uint64_t>(),
+                           L.slow_rows.as<int32_t>(), ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0,
+                           L.rev_rows.as<int32_t>(), fs);
+        ++L.nl;
+    }
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_F1], fs));
+    CU(cudaEventRecord(L.ev_fwd, fs));
+    CU(cudaStreamWaitEvent(st, L.ev_fwd, 0));
+
+    if (ctx->score_only) {
+        // candidate screening (step-3 shape): score and ref_end only; everything the traceback would fill reads
+        // as "no alignment" (ref_start -1, no CIGAR, pass 0)
+        CU(cudaMemsetAsync(ctx->ref_start.as<int32_t>() + L.p0, 0xFF, P * 4, st));
+        CU(cudaMemsetAsync(ctx->read_start.as<int32_t>() + L.p0, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->read_end.as<int32_t>() + L.p0, 0xFF, P * 4, st));
+        CU(cudaMemsetAsync(ctx->pass.as<uint8_t>() + L.p0, 0, P, st));
+        CU(cudaMemsetAsync(ctx->n_match.as<int32_t>() + L.p0, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->n_cols.as<int32_t>() + L.p0, 0, P * 4, st));
+        CU(cudaMemsetAsync(ctx->cigar_off.as<uint64_t>() + L.p0, 0, P * 8, st));
+        CU(cudaMemsetAsync(ctx->cigar_len.as<uint32_t>() + L.p0, 0, P * 4, st));
+        CU(cudaMemcpyAsync(L.mb->counters + 3, L.counters + 3, 16, cudaMemcpyDeviceToHost, st));
+        if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_END], st));
+        CU(cudaEventRecord(L.evB, st));
+        return SDP_OK;
+    }
+
+    PostParams pp{};
+    pp.b = b; pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = L.pn.as<uint32_t>(); pp.pm = L.pm.as<uint32_t>();
+    pp.score = ctx->score.as<int32_t>() + L.p0; pp.ref_end = ctx->ref_end.as<int32_t>() + L.p0;
+    pp.tbW = L.tbW.as<int32_t>(); pp.tb_rows = L.tb_rows.as<int32_t>();
+    pp.keys_tb = L.keys_tb.as<uint32_t>();
+    pp.keys_wide = L.keys_wide.as<uint32_t>();
+    pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin; pp.thin_ok = ctx->thin_ok;
+    pp.local = local; pp.slow_words = L.slow_words.as<uint32_t>(); pp.end_col = L.rev_rows.as<int32_t>();
+    pp.err_flag = L.err_flag;
+    pp.bits_words = L.bits_words.as<uint32_t>(); pp.ops_cap = L.ops_cap.as<uint32_t>();
+    pp.hist_tb = L.hist[2]; pp.hist_wide = L.hist[3]; pp.counters = L.counters;
+    launch_post_forward(pp, st);
+    // The two bucket sorts and the three scratch-offset scans are short, latency-bound launch chains that
+    // depend only on k_post_forward: they fan out over the helper streams and join before the mailbox kernel.
+    // (The reverse pass and the wide traceback serve the same pairs with the same key: one sort, one task table.)
+    cudaStream_t f2 = ctx->fan_post[2], f3 = ctx->fan_post[3];
+    CU(cudaEventRecord(L.fan_fork, st));
+    for (int k = 2; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_post[k], L.fan_fork, 0));
+    launch_sort_tail(L.keys_tb.as<uint32_t>(), P, L.hist[2], L.bin_start[2], L.order_tb.as<uint32_t>(),
+                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, f2);
+    launch_sort_tail(L.keys_wide.as<uint32_t>(), P, L.hist[3], L.bin_start[3], L.order_wide.as<uint32_t>(),
+                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, L.slots[2], L.task_prefix[2],
+                     L.mb->task_prefix[2], &L.mb->bin_total[3], st);
+    L.nl += 8;
+    // one region of direction nibbles per warp task of wide pairs (every slot of order_wide beyond the wide
+    // pairs reads as a zero-size region)
+    CU(cudaMemsetAsync(L.wide_words.p, 0, P * 4, st));
+    launch_wide_regions(L.order_wide.as<uint32_t>(), (uint32_t)P, L.bin_start[3] + SDP_NBINS, L.pn.as<uint32_t>(),
+                        L.tb_rows.as<int32_t>(), ctx->d_slot_of_n, L.slots[2], L.wide_words.as<uint32_t>(), st);
+    ++L.nl;
+    exclusive_scan_u32_u64(L.wide_words.as<uint32_t>(), P, L.wide_off.as<uint64_t>(), L.totals + 3, nullptr,
+                           L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
+                           L.scan_tile_base[0].as<uint64_t>(), st, &L.nl);
+    exclusive_scan_u32_u64(L.bits_words.as<uint32_t>(), P, L.bits_off.as<uint64_t>(), L.totals + 0, nullptr,
+                           L.scan_local[1].as<uint32_t>(), L.scan_tiles[1].as<uint32_t>(),
+                           L.scan_tile_base[1].as<uint64_t>(), f2, &L.nl);
+    exclusive_scan_u32_u64(L.ops_cap.as<uint32_t>(), P, L.ops_off.as<uint64_t>(), L.totals + 1, nullptr,
+                           L.scan_local[2].as<uint32_t>(), L.scan_tiles[2].as<uint32_t>(),
+                           L.scan_tile_base[2].as<uint64_t>(), f3, &L.nl);
+    for (int k = 2; k < SDP_FAN_STREAMS; ++k) {
+        CU(cudaEventRecord(L.fan_join[k], ctx->fan_post[k]));
+        CU(cudaStreamWaitEvent(st, L.fan_join[k], 0));
+    }
+    launch_mailbox(L.bin_start[2], TB_KEY_STRIDE, THIN_NW + TB_NCLASS + 1, L.totals, L.counters,
+                   L.mb->tb_bounds, L.mb->totals, L.mb->counters, st);
+    ++L.nl;
+    CU(cudaEventRecord(L.evB, st));
+    return SDP_OK;
+}
+
+// ---- phase C: a4 reverse pass, a5 + a6 traceback (wide path on the lane's stream, narrow bands on the side streams)
+int lane_phase_c(sdp_ctx* ctx, Lane& L, const int local)
+{
+    const sdp_batch& b = L.b;
+    cudaStream_t st = L.st;
+    const uint32_t n_wide = L.mb->bin_total[3];
+    L.n_wide = n_wide;
+    LEN(bits, (L.mb->totals[0] + 4) * 4);
+    LEN(ops_rev, (L.mb->totals[1] + 4) * 4);
+    LEN(wide_bits, (L.mb->totals[3] + 4) * 4);
+    int32_t* score = ctx->score.as<int32_t>() + L.p0;
+    int32_t* ref_end = ctx->ref_end.as<int32_t>() + L.p0;
+
+    // ---- a4 reverse pass over the wide pairs (same buckets and task table as their traceback DP)
+    launch_fill_desc_rev(b, L.order_wide.as<uint32_t>(), n_wide, score, ref_end, L.tbW.as<int32_t>(),
+                         L.desc_rev.as<PairDesc>(), st);
+    ++L.nl;
+    {
+        int rc = launch_score_stage(ctx, L, 1, L.desc_rev.as<PairDesc>(), st, ctx->fan_post, &L.nl);
+        if (rc != SDP_OK) return rc;
+    }
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_REV], st));
+
+    // ---- a5 + a6: wide pairs: rectangle DP that leaves four direction bits per cell, then the walk
+    if (n_wide) {
+        launch_fill_desc_tb(b, L.order_wide.as<uint32_t>(), n_wide, score, ref_end, L.rev_rows.as<int32_t>(),
+                            L.desc_wide.as<PairDesc>(), st);
+        ++L.nl;
+        int rc = launch_score_stage(ctx, L, 2, L.desc_wide.as<PairDesc>(), st, ctx->fan_post, &L.nl);
+        if (rc != SDP_OK) return rc;
+        WalkParams wp{};
+        wp.b = b; wp.sc = ctx->sc; wp.desc = L.desc_wide.as<PairDesc>(); wp.count = n_wide;
+        wp.slots = L.slots[2]; wp.slot_of_n = ctx->d_slot_of_n;
+        wp.bits = L.wide_bits.as<uint32_t>(); wp.bits_off = L.wide_off.as<uint64_t>();
+        wp.ref_end = ref_end; wp.tbW = L.tbW.as<int32_t>();
+        wp.ops_off = L.ops_off.as<uint64_t>(); wp.ops_rev = L.ops_rev.as<uint32_t>();
+        wp.ref_start = ctx->ref_start.as<int32_t>() + L.p0; wp.read_start = ctx->read_start.as<int32_t>() + L.p0;
+        wp.read_end = ctx->read_end.as<int32_t>() + L.p0; wp.pass = ctx->pass.as<uint8_t>() + L.p0;
+        wp.n_match = ctx->n_match.as<int32_t>() + L.p0; wp.n_cols = ctx->n_cols.as<int32_t>() + L.p0;
+        wp.cigar_len = ctx->cigar_len.as<uint32_t>() + L.p0; wp.err_flag = L.err_flag;
+        launch_walk(wp, st);
+        ++L.nl;
+    }
+    // ---- a5 + a6, narrow bands (W < THIN_NW: two pairs per thread, band in registers) and the generic band kernel.
+    // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on side streams
+    // beside it (the host has waited for the lane's phase B, which produced everything they read).
+    TraceParams tp{};
+    tp.b = b; tp.sc = ctx->sc; tp.order = L.order_tb.as<uint32_t>();
+    tp.score = score; tp.ref_end = ref_end; tp.tbW = L.tbW.as<int32_t>();
+    tp.rev_rows = nullptr; tp.end_col = L.rev_rows.as<int32_t>();
+    tp.bits_off = L.bits_off.as<uint64_t>(); tp.bits = L.bits.as<uint32_t>();
+    tp.ops_off = L.ops_off.as<uint64_t>(); tp.ops_rev = L.ops_rev.as<uint32_t>();
+    tp.ref_start = ctx->ref_start.as<int32_t>() + L.p0; tp.read_start = ctx->read_start.as<int32_t>() + L.p0;
+    tp.read_end = ctx->read_end.as<int32_t>() + L.p0; tp.pass = ctx->pass.as<uint8_t>() + L.p0;
+    tp.n_match = ctx->n_match.as<int32_t>() + L.p0; tp.n_cols = ctx->n_cols.as<int32_t>() + L.p0;
+    tp.cigar_len = ctx->cigar_len.as<uint32_t>() + L.p0; tp.err_flag = L.err_flag;
+    L.nl += (uint32_t)launch_thin_all(L.mb->tb_bounds, tp, ctx->side_stream[0], ctx->side_stream[1], ctx->side_stream[2]);
+    for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
+        tp.first = L.mb->tb_bounds[c];
+        tp.count = L.mb->tb_bounds[c + 1] - tp.first;
+        if (!tp.count) continue;
+        launch_traceback(c - THIN_NW, local != 0, tp, ctx->side_stream[0]);
+        ++L.nl;
+    }
+    for (int k = 0; k < 3; ++k) {
+        CU(cudaEventRecord(L.side_done[k], ctx->side_stream[k]));
+        CU(cudaStreamWaitEvent(st, L.side_done[k], 0));
+    }
+    CU(cudaGetLastError());
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_TRACE], st));
+    CU(cudaEventRecord(L.evC, st));
+    return SDP_OK;
+}
+
+// ---- phase D: a7 compaction in caller pair order; the lane's run offsets start at the previous lanes' total
+int lane_phase_d(sdp_ctx* ctx, Lane& L, const int li)
+{
+    cudaStream_t st = L.st;
+    const uint64_t P = L.P;
+    if (li > 0) CU(cudaStreamWaitEvent(st, ctx->ev_cig[li - 1], 0));
+    exclusive_scan_u32_u64(ctx->cigar_len.as<uint32_t>() + L.p0, P, ctx->cigar_off.as<uint64_t>() + L.p0, ctx->cig_total + li + 1,
+                           ctx->cig_total + li, L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
+                           L.scan_tile_base[0].as<uint64_t>(), st, &L.nl);
+    CU(cudaEventRecord(ctx->ev_cig[li], st));
+    launch_compact(P, L.ops_off.as<uint64_t>(), L.ops_rev.as<uint32_t>(), ctx->cigar_len.as<uint32_t>() + L.p0,
+                   ctx->cigar_off.as<uint64_t>() + L.p0, ctx->cigar_ops.as<uint32_t>(), st);
+    ++L.nl;
+    CU(cudaMemcpyAsync(&L.mb->totals[2], ctx->cig_total + li + 1, 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&L.mb->err_flag, L.err_flag, 4, cudaMemcpyDeviceToHost, st));
+    if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_END], st));
+    CU(cudaEventRecord(L.evD, st));
+    return SDP_OK;
+}
+
+}  // namespace
 
 int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp_result* out)
 {
@@ -487,19 +793,10 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     ctx->last_pairs = nullptr; ctx->last_n_pairs = 0; ctx->last_n_reads = 0;
     sdp_stats stats{};
     stats.n_pairs = P;
-    uint32_t nl = 0;
 
     const size_t Pp = (size_t)(P ? P : 1);
-    EN(keys, Pp * 4); EN(pn, Pp * 4); EN(pm, Pp * 4); EN(order, Pp * 4); EN(desc, Pp * sizeof(PairDesc));
-    EN(desc_rev, Pp * sizeof(PairDesc)); EN(order_tb, Pp * 4);
-    EN(keys_tb, Pp * 4); EN(tbW, Pp * 4); EN(rev_rows, Pp * 4);
-    EN(tb_rows, Pp * 4); EN(keys_wide, Pp * 4); EN(order_wide, Pp * 4); EN(desc_wide, Pp * sizeof(PairDesc));
-    EN(wide_words, Pp * 4); EN(wide_off, Pp * 8);
-    EN(bits_words, Pp * 4); EN(ops_cap, Pp * 4); EN(bits_off, Pp * 8); EN(ops_off, Pp * 8);
-    for (int k = 0; k < 3; ++k) { EN(scan_local[k], Pp * 4); EN(scan_tiles[k], (Pp / 4096 + 2) * 4); EN(scan_tile_base[k], (Pp / 4096 + 2) * 8); }
     EN(score, Pp * 4); EN(ref_start, Pp * 4); EN(ref_end, Pp * 4); EN(read_start, Pp * 4); EN(read_end, Pp * 4);
     EN(pass, Pp); EN(n_match, Pp * 4); EN(n_cols, Pp * 4); EN(cigar_off, Pp * 8); EN(cigar_len, Pp * 4);
-    EN(slow_words, Pp * 4); EN(slow_off, Pp * 8);
     const int local = ctx->mode == SDP_MODE_LOCAL ? 1 : 0;
 
     auto finish = [&](uint64_t n_ops) {
@@ -518,232 +815,109 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         return SDP_OK;
     }
 
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_START], st));
-    // ---- a1 + a2
-    CU(cudaMemsetAsync(ctx->zero_block, 0, ctx->zero_bytes, st));
-    launch_validate_key(b, ctx->sc, ctx->keys.as<uint32_t>(), ctx->pn.as<uint32_t>(), ctx->pm.as<uint32_t>(),
-                        ctx->hist[0], ctx->err_flag, ctx->counters + 3, (ctx->prefilter && !local) ? 1 : 0, ctx->score.as<int32_t>(),
-                        ctx->ref_end.as<int32_t>(), ctx->counters + 4, local, ctx->slow_words.as<uint32_t>(), st);
-    // row arrays of the int32 lane: offsets now, so that the arrays can be allocated after the synchronisation below
-    exclusive_scan_u32_u64(ctx->slow_words.as<uint32_t>(), P, ctx->slow_off.as<uint64_t>(), ctx->totals + 0,
-                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
-                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
-    CU(cudaMemcpyAsync(&ctx->mb->slow_total, ctx->totals + 0, 8, cudaMemcpyDeviceToHost, st));
-    launch_sort_tail(ctx->keys.as<uint32_t>(), P, ctx->hist[0], ctx->bin_start[0], ctx->order.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[0], ctx->task_prefix[0],
-                     ctx->mb->task_prefix[0], &ctx->mb->bin_total[0], st);
-    nl += 5;
-    CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    if (ctx->mb->err_flag & SDP_ERRF_INDEX)
-        return fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)");
-    if (ctx->mb->err_flag & SDP_ERRF_RANGE)
-        return fail(ctx, SDP_ERANGE, "a sequence is longer than SDP_MAX_SEQ_LEN (see sdp.h)");
-    // (with the ungapped pre-pass on, fewer than P pairs are in the forward buckets)
-    launch_fill_desc_fwd(b, ctx->order.as<uint32_t>(), ctx->mb->bin_total[0], ctx->desc.as<PairDesc>(), st);
-    ++nl;
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_BUCKET], st));
-
-    // ---- a3 forward score pass
+    // ---- lanes: contiguous ranges of the pair list, software-pipelined (see Lane)
+    int NL = ctx->chunks;
+    if (NL <= 0) NL = 1;      // measured on B200: a lane's latency-bound tail under the next forward kernel costs that kernel
+                              // more than it hides, so pipelining stays opt-in
+    if ((uint64_t)NL > P) NL = (int)P;
     {
-        uint32_t before = nl;
-        int rc = launch_score_stage(ctx, 0, b, ctx->desc.as<PairDesc>(), st, &nl);
+        const int rc = lanes_init(ctx, NL);
         if (rc != SDP_OK) return rc;
-        stats.forward_launches = nl - before;
     }
-    stats.n_slow_words = ctx->mb->slow_total;
-    if (ctx->mb->slow_total) {
-        // the int32 lane: pairs outside the int16 kernels' domain, and every pair in local mode (slow_lane.cu)
-        EN(slow_rows, (ctx->mb->slow_total + 4) * 4);
-        launch_forward_i32(b, ctx->sc, local, ctx->slow_words.as<uint32_t>(), ctx->slow_off.as<uint64_t>(),
-                           ctx->slow_rows.as<int32_t>(), ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
-                           ctx->rev_rows.as<int32_t>(), st);
-        ++nl;
+    CU(cudaEventRecord(ctx->ev_start, st));
+    CU(cudaStreamWaitEvent(ctx->fwd_stream, ctx->ev_start, 0));
+    for (int li = 0; li < NL; ++li) {
+        Lane& L = ctx->lane[li];
+        L.p0 = P * (uint64_t)li / (uint64_t)NL;
+        L.P = P * (uint64_t)(li + 1) / (uint64_t)NL - L.p0;
+        L.b = b; L.b.pairs = b.pairs + 2 * L.p0; L.b.n_pairs = L.P;
+        CU(cudaStreamWaitEvent(L.st, ctx->ev_start, 0));
     }
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_FORWARD], st));
+    auto bail = [&](int rc) { drain(ctx); return rc; };
 
-    if (ctx->score_only) {
-        // candidate screening (step-3 shape): score and ref_end only; everything the traceback would fill reads
-        // as "no alignment" (ref_start -1, no CIGAR, pass 0)
-        EN(cigar_ops, 16);
-        CU(cudaMemsetAsync(ctx->ref_start.p, 0xFF, P * 4, st));
-        CU(cudaMemsetAsync(ctx->read_start.p, 0, P * 4, st));
-        CU(cudaMemsetAsync(ctx->read_end.p, 0xFF, P * 4, st));
-        CU(cudaMemsetAsync(ctx->pass.p, 0, P, st));
-        CU(cudaMemsetAsync(ctx->n_match.p, 0, P * 4, st));
-        CU(cudaMemsetAsync(ctx->n_cols.p, 0, P * 4, st));
-        CU(cudaMemsetAsync(ctx->cigar_off.p, 0, P * 8, st));
-        CU(cudaMemsetAsync(ctx->cigar_len.p, 0, P * 4, st));
-        CU(cudaMemcpyAsync(ctx->mb->counters + 3, ctx->counters + 3, 16, cudaMemcpyDeviceToHost, st));
-        if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
-        CU(cudaStreamSynchronize(st));
-        stats.cells_forward = ctx->mb->counters[3];
-        stats.cells_prefiltered = ctx->mb->counters[4];
-        stats.kernel_launches = nl;
-        if (ctx->timing) {
-            cudaEventElapsedTime(&stats.ms_total, ctx->ev[EV_START], ctx->ev[EV_END]);
-            cudaEventElapsedTime(&stats.ms_bucket, ctx->ev[EV_START], ctx->ev[EV_BUCKET]);
-            cudaEventElapsedTime(&stats.ms_forward, ctx->ev[EV_BUCKET], ctx->ev[EV_FORWARD]);
+    for (int li = 0; li < NL; ++li) {
+        const int rc = lane_phase_a(ctx, ctx->lane[li], local);
+        if (rc != SDP_OK) return bail(rc);
+    }
+    for (int li = 0; li < NL; ++li) {
+        Lane& L = ctx->lane[li];
+        CU(cudaEventSynchronize(L.evA));
+        if (L.mb->err_flag & SDP_ERRF_INDEX)
+            return bail(fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)"));
+        if (L.mb->err_flag & SDP_ERRF_RANGE)
+            return bail(fail(ctx, SDP_ERANGE, "a sequence is longer than SDP_MAX_SEQ_LEN (see sdp.h)"));
+    }
+    for (int li = 0; li < NL; ++li) {
+        const int rc = lane_phase_b(ctx, ctx->lane[li], local);
+        if (rc != SDP_OK) return bail(rc);
+    }
+    uint64_t n_ops = 0;
+    if (!ctx->score_only) {
+        uint64_t ops_capacity = 0;
+        for (int li = 0; li < NL; ++li) {
+            Lane& L = ctx->lane[li];
+            CU(cudaEventSynchronize(L.evB));
+            ops_capacity += L.mb->totals[1];
+            const int rc = lane_phase_c(ctx, L, local);
+            if (rc != SDP_OK) return bail(rc);
         }
-        ctx->stats = stats;
-        ctx->last_pairs = b.pairs; ctx->last_n_pairs = P; ctx->last_n_reads = b.n_reads;
-        finish(0);
-        return SDP_OK;
+        {
+            const int rc = ensure(ctx, ctx->cigar_ops, (ops_capacity + 4) * 4);
+            if (rc != SDP_OK) return bail(rc);
+        }
+        for (int li = 0; li < NL; ++li) {
+            const int rc = lane_phase_d(ctx, ctx->lane[li], li);
+            if (rc != SDP_OK) return bail(rc);
+        }
+        for (int li = 0; li < NL; ++li) CU(cudaStreamWaitEvent(st, ctx->lane[li].evD, 0));
+    } else {
+        const int rc = ensure(ctx, ctx->cigar_ops, 16);
+        if (rc != SDP_OK) return bail(rc);
+        for (int li = 0; li < NL; ++li) CU(cudaStreamWaitEvent(st, ctx->lane[li].evB, 0));
     }
-
-    // ---- gap bound W, keys of the two later stages, scratch sizes
-    PostParams pp{};
-    pp.b = b; pp.n_pairs = P; pp.sc = ctx->sc; pp.pn = ctx->pn.as<uint32_t>(); pp.pm = ctx->pm.as<uint32_t>();
-    pp.score = ctx->score.as<int32_t>(); pp.ref_end = ctx->ref_end.as<int32_t>();
-    pp.tbW = ctx->tbW.as<int32_t>(); pp.tb_rows = ctx->tb_rows.as<int32_t>();
-    pp.keys_tb = ctx->keys_tb.as<uint32_t>();
-    pp.keys_wide = ctx->keys_wide.as<uint32_t>();
-    pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin; pp.thin_ok = ctx->thin_ok;
-    pp.local = local; pp.slow_words = ctx->slow_words.as<uint32_t>(); pp.end_col = ctx->rev_rows.as<int32_t>();
-    pp.err_flag = ctx->err_flag;
-    pp.bits_words = ctx->bits_words.as<uint32_t>(); pp.ops_cap = ctx->ops_cap.as<uint32_t>();
-    pp.hist_tb = ctx->hist[2]; pp.hist_wide = ctx->hist[3]; pp.counters = ctx->counters;
-    launch_post_forward(pp, st);
-    // The two bucket sorts and the three scratch-offset scans are short, latency-bound launch chains that
-    // depend only on k_post_forward: they fan out over the helper streams and join before the mailbox kernel.
-    // (The reverse pass and the wide traceback serve the same pairs with the same key: one sort, one task table.)
-    cudaStream_t f2 = ctx->fan_stream[2], f3 = ctx->fan_stream[3];
-    CU(cudaEventRecord(ctx->fan_fork, st));
-    for (int k = 1; k < SDP_FAN_STREAMS; ++k) CU(cudaStreamWaitEvent(ctx->fan_stream[k], ctx->fan_fork, 0));
-    launch_sort_tail(ctx->keys_tb.as<uint32_t>(), P, ctx->hist[2], ctx->bin_start[2], ctx->order_tb.as<uint32_t>(),
-                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, f2);
-    launch_sort_tail(ctx->keys_wide.as<uint32_t>(), P, ctx->hist[3], ctx->bin_start[3], ctx->order_wide.as<uint32_t>(),
-                     ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, ctx->slots[2], ctx->task_prefix[2],
-                     ctx->mb->task_prefix[2], &ctx->mb->bin_total[3], st);
-    nl += 8;
-    // one region of direction nibbles per warp task of wide pairs (every slot of order_wide beyond the wide
-    // pairs reads as a zero-size region)
-    CU(cudaMemsetAsync(ctx->wide_words.p, 0, P * 4, st));
-    launch_wide_regions(ctx->order_wide.as<uint32_t>(), (uint32_t)P, ctx->bin_start[3] + SDP_NBINS, ctx->pn.as<uint32_t>(),
-                        ctx->tb_rows.as<int32_t>(), ctx->d_slot_of_n, ctx->slots[2], ctx->wide_words.as<uint32_t>(), st);
-    ++nl;
-    exclusive_scan_u32_u64(ctx->wide_words.as<uint32_t>(), P, ctx->wide_off.as<uint64_t>(), ctx->totals + 3,
-                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
-                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
-    exclusive_scan_u32_u64(ctx->bits_words.as<uint32_t>(), P, ctx->bits_off.as<uint64_t>(), ctx->totals + 0,
-                           ctx->scan_local[1].as<uint32_t>(), ctx->scan_tiles[1].as<uint32_t>(),
-                           ctx->scan_tile_base[1].as<uint64_t>(), f2, &nl);
-    exclusive_scan_u32_u64(ctx->ops_cap.as<uint32_t>(), P, ctx->ops_off.as<uint64_t>(), ctx->totals + 1,
-                           ctx->scan_local[2].as<uint32_t>(), ctx->scan_tiles[2].as<uint32_t>(),
-                           ctx->scan_tile_base[2].as<uint64_t>(), f3, &nl);
-    for (int k = 1; k < SDP_FAN_STREAMS; ++k) {
-        CU(cudaEventRecord(ctx->fan_join[k], ctx->fan_stream[k]));
-        CU(cudaStreamWaitEvent(st, ctx->fan_join[k], 0));
-    }
-    launch_mailbox(ctx->bin_start[2], TB_KEY_STRIDE, THIN_NW + TB_NCLASS + 1, ctx->totals, ctx->counters,
-                   ctx->mb->tb_bounds, ctx->mb->totals, ctx->mb->counters, st);
-    ++nl;
-    CU(cudaStreamSynchronize(st));
-    const uint32_t n_wide = ctx->mb->bin_total[3];
-    const uint32_t n_rev = n_wide;
-    EN(bits, (ctx->mb->totals[0] + 4) * 4);
-    EN(ops_rev, (ctx->mb->totals[1] + 4) * 4);
-    EN(cigar_ops, (ctx->mb->totals[1] + 4) * 4);
-    EN(wide_bits, (ctx->mb->totals[3] + 4) * 4);
-
-    // ---- a4 reverse pass over the pairs whose score admits a gap
-    launch_fill_desc_rev(b, ctx->order_wide.as<uint32_t>(), n_rev, ctx->score.as<int32_t>(), ctx->ref_end.as<int32_t>(),
-                         ctx->tbW.as<int32_t>(), ctx->desc_rev.as<PairDesc>(), st);
-    ++nl;
-    {
-        int rc = launch_score_stage(ctx, 1, b, ctx->desc_rev.as<PairDesc>(), st, &nl);
-        if (rc != SDP_OK) return rc;
-    }
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_REVERSE], st));
-
-    // ---- a5 + a6 traceback, CIGAR runs, similarity filter
-    // wide pairs: rectangle DP that leaves four direction bits per cell, then the walk
-    if (n_wide) {
-        launch_fill_desc_tb(b, ctx->order_wide.as<uint32_t>(), n_wide, ctx->score.as<int32_t>(),
-                            ctx->ref_end.as<int32_t>(), ctx->rev_rows.as<int32_t>(), ctx->desc_wide.as<PairDesc>(), st);
-        ++nl;
-        int rc = launch_score_stage(ctx, 2, b, ctx->desc_wide.as<PairDesc>(), st, &nl);
-        if (rc != SDP_OK) return rc;
-        WalkParams wp{};
-        wp.b = b; wp.sc = ctx->sc; wp.desc = ctx->desc_wide.as<PairDesc>(); wp.count = n_wide;
-        wp.slots = ctx->slots[2]; wp.slot_of_n = ctx->d_slot_of_n;
-        wp.bits = ctx->wide_bits.as<uint32_t>(); wp.bits_off = ctx->wide_off.as<uint64_t>();
-        wp.ref_end = ctx->ref_end.as<int32_t>(); wp.tbW = ctx->tbW.as<int32_t>();
-        wp.ops_off = ctx->ops_off.as<uint64_t>(); wp.ops_rev = ctx->ops_rev.as<uint32_t>();
-        wp.ref_start = ctx->ref_start.as<int32_t>(); wp.read_start = ctx->read_start.as<int32_t>();
-        wp.read_end = ctx->read_end.as<int32_t>(); wp.pass = ctx->pass.as<uint8_t>();
-        wp.n_match = ctx->n_match.as<int32_t>(); wp.n_cols = ctx->n_cols.as<int32_t>();
-        wp.cigar_len = ctx->cigar_len.as<uint32_t>(); wp.err_flag = ctx->err_flag;
-        launch_walk(wp, st);
-        ++nl;
-    }
-    // ---- a5 + a6, narrow bands (W < THIN_NW: one thread per pair, band in registers) and the generic band kernel.
-    // They need nothing from the reverse pass and touch other pairs than the wide path, so they run on a
-    // side stream beside it (the stream synchronisation above has completed everything they read).
-    cudaStream_t ss = ctx->side_stream;
-    TraceParams tp{};
-    tp.b = b; tp.sc = ctx->sc; tp.order = ctx->order_tb.as<uint32_t>();
-    tp.score = ctx->score.as<int32_t>(); tp.ref_end = ctx->ref_end.as<int32_t>(); tp.tbW = ctx->tbW.as<int32_t>();
-    tp.rev_rows = nullptr; tp.end_col = ctx->rev_rows.as<int32_t>();
-    tp.bits_off = ctx->bits_off.as<uint64_t>(); tp.bits = ctx->bits.as<uint32_t>();
-    tp.ops_off = ctx->ops_off.as<uint64_t>(); tp.ops_rev = ctx->ops_rev.as<uint32_t>();
-    tp.ref_start = ctx->ref_start.as<int32_t>(); tp.read_start = ctx->read_start.as<int32_t>();
-    tp.read_end = ctx->read_end.as<int32_t>(); tp.pass = ctx->pass.as<uint8_t>();
-    tp.n_match = ctx->n_match.as<int32_t>(); tp.n_cols = ctx->n_cols.as<int32_t>();
-    tp.cigar_len = ctx->cigar_len.as<uint32_t>(); tp.err_flag = ctx->err_flag;
-    nl += (uint32_t)launch_thin_all(ctx->mb->tb_bounds, tp, ss, ctx->side_stream3, ctx->side_stream2);
-    CU(cudaEventRecord(ctx->side_done2, ctx->side_stream2));
-    CU(cudaEventRecord(ctx->side_done3, ctx->side_stream3));
-    for (int c = THIN_NW; c < THIN_NW + TB_NCLASS; ++c) {
-        tp.first = ctx->mb->tb_bounds[c];
-        tp.count = ctx->mb->tb_bounds[c + 1] - tp.first;
-        if (!tp.count) continue;
-        launch_traceback(c - THIN_NW, local != 0, tp, ss);
-        ++nl;
-    }
-    CU(cudaEventRecord(ctx->side_done, ss));
-
-    CU(cudaStreamWaitEvent(st, ctx->side_done, 0));
-    CU(cudaStreamWaitEvent(st, ctx->side_done2, 0));
-    CU(cudaStreamWaitEvent(st, ctx->side_done3, 0));
-    CU(cudaGetLastError());
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_TRACE], st));
-
-    // ---- a7 compaction in caller pair order
-    exclusive_scan_u32_u64(ctx->cigar_len.as<uint32_t>(), P, ctx->cigar_off.as<uint64_t>(), ctx->totals + 2,
-                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
-                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
-    launch_compact(P, ctx->ops_off.as<uint64_t>(), ctx->ops_rev.as<uint32_t>(), ctx->cigar_len.as<uint32_t>(),
-                   ctx->cigar_off.as<uint64_t>(), ctx->cigar_ops.as<uint32_t>(), st);
-    ++nl;
-    CU(cudaMemcpyAsync(&ctx->mb->totals[2], ctx->totals + 2, 8, cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(&ctx->mb->err_flag, ctx->err_flag, 4, cudaMemcpyDeviceToHost, st));
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[EV_END], st));
+    CU(cudaEventRecord(ctx->ev_end, st));
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
-    if (ctx->mb->err_flag & SDP_ERRF_RANGE)
-        return fail(ctx, SDP_ERANGE, "the traceback scratch of one pair exceeds 16 GiB (see sdp.h)");
-    if (ctx->mb->err_flag & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
-        return fail(ctx, SDP_ECUDA, "internal consistency check failed (flags 0x%x): reverse pass or traceback "
-                    "disagrees with the forward score", ctx->mb->err_flag);
+    uint32_t errf = 0;
+    for (int li = 0; li < NL; ++li) errf |= ctx->lane[li].mb->err_flag;
+    if (!ctx->score_only) {
+        if (errf & SDP_ERRF_RANGE)
+            return bail(fail(ctx, SDP_ERANGE, "the traceback scratch of one pair exceeds 16 GiB (see sdp.h)"));
+        if (errf & (SDP_ERRF_REVERSE | SDP_ERRF_TRACE))
+            return bail(fail(ctx, SDP_ECUDA, "internal consistency check failed (flags 0x%x): reverse pass or traceback "
+                             "disagrees with the forward score", errf));
+        n_ops = ctx->lane[NL - 1].mb->totals[2];
+    }
 
-    stats.cells_forward = ctx->mb->counters[3];
-    stats.cells_prefiltered = ctx->mb->counters[4];
-    stats.cells_reverse = ctx->mb->counters[0];
-    stats.cells_traceback = ctx->mb->counters[1];
-    stats.n_reverse_pairs = ctx->mb->counters[2];
-    stats.kernel_launches = nl;
-    if (ctx->timing) {
-        cudaEventElapsedTime(&stats.ms_total, ctx->ev[EV_START], ctx->ev[EV_END]);
-        cudaEventElapsedTime(&stats.ms_bucket, ctx->ev[EV_START], ctx->ev[EV_BUCKET]);
-        cudaEventElapsedTime(&stats.ms_forward, ctx->ev[EV_BUCKET], ctx->ev[EV_FORWARD]);
-        cudaEventElapsedTime(&stats.ms_reverse, ctx->ev[EV_FORWARD], ctx->ev[EV_REVERSE]);
-        cudaEventElapsedTime(&stats.ms_traceback, ctx->ev[EV_REVERSE], ctx->ev[EV_TRACE]);
-        cudaEventElapsedTime(&stats.ms_compact, ctx->ev[EV_TRACE], ctx->ev[EV_END]);
+    if (ctx->timing) cudaEventElapsedTime(&stats.ms_total, ctx->ev_start, ctx->ev_end);
+    for (int li = 0; li < NL; ++li) {
+        Lane& L = ctx->lane[li];
+        stats.cells_forward += L.mb->counters[3];
+        stats.cells_prefiltered += L.mb->counters[4];
+        stats.n_slow_words += L.mb->slow_total;
+        stats.kernel_launches += L.nl;
+        stats.forward_launches += L.fwd_launches;
+        if (!ctx->score_only) {
+            stats.cells_reverse += L.mb->counters[0];
+            stats.cells_traceback += L.mb->counters[1];
+            stats.n_reverse_pairs += L.mb->counters[2];
+        }
+        if (ctx->timing) {
+            // per-stage times are summed over the lanes; with more than one lane the stages of different lanes overlap,
+            // so the sum of the parts exceeds ms_total (ms_forward: the forward kernels run back to back on one stream)
+            float t = 0.f;
+            cudaEventElapsedTime(&t, L.tev[LEV_A0], L.tev[LEV_A1]); stats.ms_bucket += t;
+            cudaEventElapsedTime(&t, L.tev[LEV_F0], L.tev[LEV_F1]); stats.ms_forward += t;
+            if (!ctx->score_only) {
+                cudaEventElapsedTime(&t, L.tev[LEV_F1], L.tev[LEV_REV]); stats.ms_reverse += t;
+                cudaEventElapsedTime(&t, L.tev[LEV_REV], L.tev[LEV_TRACE]); stats.ms_traceback += t;
+                cudaEventElapsedTime(&t, L.tev[LEV_TRACE], L.tev[LEV_END]); stats.ms_compact += t;
+            }
+        }
     }
     ctx->stats = stats;
     ctx->last_pairs = b.pairs; ctx->last_n_pairs = P; ctx->last_n_reads = b.n_reads;
-    finish(ctx->mb->totals[2]);
+    finish(n_ops);
     return SDP_OK;
 }
 
@@ -797,18 +971,19 @@ int sdp_mate_pairs(sdp_ctx* ctx, const uint32_t* win_len, uint64_t n, void* cuda
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CU(cudaSetDevice(ctx->device));
     const size_t N = (size_t)(n ? n : 1);
+    Lane& L = ctx->lane[0];                    // scan scratch and mailbox of the first lane (no align call is in flight)
     EN(mp_flag, N * 4); EN(mp_off, N * 8);
-    EN(scan_local[0], N * 4); EN(scan_tiles[0], (N / 4096 + 2) * 4); EN(scan_tile_base[0], (N / 4096 + 2) * 8);
+    LEN(scan_local[0], N * 4); LEN(scan_tiles[0], (N / 4096 + 2) * 4); LEN(scan_tile_base[0], (N / 4096 + 2) * 8);
     uint32_t nl = 0;
     launch_mate_flags(win_len, n, ctx->mp_flag.as<uint32_t>(), st);
-    exclusive_scan_u32_u64(ctx->mp_flag.as<uint32_t>(), n, ctx->mp_off.as<uint64_t>(), ctx->totals + 2,
-                           ctx->scan_local[0].as<uint32_t>(), ctx->scan_tiles[0].as<uint32_t>(),
-                           ctx->scan_tile_base[0].as<uint64_t>(), st, &nl);
+    exclusive_scan_u32_u64(ctx->mp_flag.as<uint32_t>(), n, ctx->mp_off.as<uint64_t>(), L.totals + 2, nullptr,
+                           L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
+                           L.scan_tile_base[0].as<uint64_t>(), st, &nl);
     launch_mate_pairs(ctx->mp_flag.as<uint32_t>(), ctx->mp_off.as<uint64_t>(), n, pairs, pair_of_rescue, st);
-    CU(cudaMemcpyAsync(&ctx->mb->totals[2], ctx->totals + 2, 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&L.mb->totals[2], L.totals + 2, 8, cudaMemcpyDeviceToHost, st));
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(st));
-    *n_pairs = ctx->mb->totals[2];
+    *n_pairs = L.mb->totals[2];
     return SDP_OK;
 }
 

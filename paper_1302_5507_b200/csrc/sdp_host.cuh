@@ -23,7 +23,8 @@ void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbou
                     const unsigned long long* counters, uint32_t* host_bounds, uint64_t* host_totals,
                     unsigned long long* host_counters, cudaStream_t st);
 void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st);
-void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev,
+// exclusive scan of n 32-bit values into 64-bit offsets starting at *base_dev (0 when null); *total_dev = base + sum
+void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev, const uint64_t* base_dev,
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
                             cudaStream_t st, uint32_t* launches);
 

@@ -49,6 +49,7 @@ struct ScoreConsts {           // what the score kernels take as arguments; the 
     uint32_t beta2;            // packed int16x2 beta
     uint32_t betaMinusO2;      // packed beta - o
     int32_t  e, beta;          // scalars
+    int32_t  match;            // reverse pass: early-exit bound
 };
 
 struct ScoreParams {
@@ -91,6 +92,9 @@ struct TraceDP {
 };
 
 // packed helpers
+__host__ __device__ constexpr static inline uint32_t sdp_pack_lo_hi(int lo, int hi) {
+    return ((uint32_t)(uint16_t)(int16_t)lo) | (((uint32_t)(uint16_t)(int16_t)hi) << 16);
+}
 __host__ __device__ constexpr static inline uint32_t sdp_pack2(int v) {
     return ((uint32_t)(uint16_t)(int16_t)v) | (((uint32_t)(uint16_t)(int16_t)v) << 16);
 }

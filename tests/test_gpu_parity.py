@@ -57,6 +57,22 @@ def test_ragged_counts(ctx):
         parity.check_batch(ctx, full.subset(np.arange(cnt)), DEFAULT, f"count={cnt}", host_path=False)
 
 
+@pytest.mark.parametrize("chunks", [1, 2, 3, 5, 8])
+def test_chunked_lanes(chunks):
+    # sdp_set_chunks: the pair list split into pipelined lanes; every output array (the CIGAR offsets run across the
+    # lanes) must be what the unsplit call gives. Also a batch with fewer pairs than lanes, and mixed read lengths.
+    c = make_ctx(DEFAULT)
+    try:
+        c.set_chunks(chunks)
+        for cfg, n_pairs in ((2, 3001), (5, 4000), (4, 700), (1, 3)):
+            b = W.make_config(cfg, n_pairs=n_pairs, ref_bases=1_000_000)
+            parity.check_batch(c, b, DEFAULT, f"cfg{cfg} in {chunks} lanes")
+        with pytest.raises(SdpError):
+            c.set_chunks(9)
+    finally:
+        c.destroy()
+
+
 def test_empty_batch(ctx):
     full = W.make_config(1, n_pairs=4, ref_bases=100_000)
     b = full.subset(np.arange(0))
