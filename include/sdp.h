@@ -156,9 +156,11 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
  * it hides); at most 8. SDP_EINVAL outside 0..8. */
 int sdp_set_chunks(sdp_ctx* ctx, int chunks);
 
-/* Same operation with HOST pointers in `batch`: copies the inputs to the device through pinned
- * staging, runs sdp_align_batch's pipeline on an internal stream, and copies every result array
- * back; `out` then holds pinned HOST pointers owned by the ctx. */
+/* Same operation with HOST pointers in `batch`: copies the inputs into device buffers owned by the ctx
+ * (cudaMemcpyAsync on an internal stream, straight from the caller's arrays: pass page-locked memory for full PCIe
+ * speed; pageable memory is accepted, the driver then stages the copies and they run synchronously), runs
+ * sdp_align_batch's pipeline, and copies every result array back into one pinned slab; `out` then holds pinned HOST
+ * pointers owned by the ctx, valid until the next call on this ctx. */
 int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* batch, sdp_result* out);
 
 /*

@@ -303,10 +303,32 @@ __global__ void k_scan_add(const uint32_t* __restrict__ local, const uint64_t* _
     if (i < n) out[i] = tile_base[i / SCAN_TILE] + local[i];
 }
 
+// n <= SCAN_TILE: the three phases in one block, 64-bit throughout (small batches are launch-bound: one launch
+// instead of three)
+__global__ void __launch_bounds__(1024) k_scan_small(const uint32_t* __restrict__ in, uint32_t n, uint64_t* __restrict__ out,
+                                                     uint64_t* __restrict__ total_out, const uint64_t* __restrict__ base_in)
+{
+    const uint32_t base = threadIdx.x * SCAN_PER;
+    uint32_t v[SCAN_PER];
+    uint64_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_PER; ++k) { v[k] = (base + k < n) ? in[base + k] : 0u; sum += v[k]; }
+    uint64_t total;
+    uint64_t run = block_exclusive_scan_1024_u64(sum, &total) + (base_in ? *base_in : 0ull);
+#pragma unroll
+    for (int k = 0; k < SCAN_PER; ++k) { if (base + k < n) out[base + k] = run; run += v[k]; }
+    if (threadIdx.x == 0) *total_out = total + (base_in ? *base_in : 0ull);
+}
+
 void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev, const uint64_t* base_dev,
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
                             cudaStream_t st, uint32_t* launches)
 {
+    if (n <= (uint64_t)SCAN_TILE) {
+        k_scan_small<<<1, 1024, 0, st>>>(in, (uint32_t)n, out, total_dev, base_dev);
+        *launches += 1;
+        return;
+    }
     const uint32_t ntiles = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (n) k_scan_tiles<<<ntiles, 1024, 0, st>>>(in, n, tmp_local, tmp_tiles);
     k_scan_tile_sums<<<1, 1024, 0, st>>>(tmp_tiles, ntiles, tmp_tile_base, total_dev, base_dev);

@@ -244,11 +244,11 @@ void lane_destroy(Lane& L)
 
 // (G, K) per read length: G threads share the read, K = ceil(n / G) columns each. A warp runs 2*floor(32/G) pairs
 // for (m + G - 1) steps, and a step costs what the (K, padded) kernel variant was MEASURED to cost on B200
-// (200,000 pairs, m = n + 300, G = 4; relative units; K = 1 extrapolated). A table, not a formula, because the
-// per-variant cost depends on how ptxas happened to allocate registers for that K (e.g. K = 21 exact is 6 %
-// slower than K = 21 padded), which no smooth model captures; DESIGN.md "Score kernel".
-static const double kStepCostExact[SDP_MAX_K] = {6.7, 8.4, 10.0, 12.1, 13.8, 15.7, 17.5, 19.5, 21.1, 23.4, 25.0, 27.0, 29.4, 31.3, 33.8, 34.5, 36.2, 40.1, 41.0, 44.0, 48.3, 45.9, 47.7, 49.1, 50.5, 56.6, 58.4, 60.4, 61.4, 65.5, 70.1, 67.6};
-static const double kStepCostPadded[SDP_MAX_K] = {7.5, 9.2, 11.0, 12.8, 14.7, 16.5, 18.4, 20.0, 22.1, 23.8, 26.4, 27.1, 30.3, 31.2, 33.8, 36.0, 39.4, 43.3, 41.6, 43.2, 45.4, 49.4, 49.2, 50.4, 53.4, 57.5, 60.4, 59.2, 65.3, 66.0, 64.7, 66.7};
+// (200,000 pairs, m = n + 300, G = 4; relative units; re-measured in round 2 for the two-row-skew, immediate-operand
+// kernel, whose cost is close to 0.24 + 0.103 K: the per-K irregularities of the round-1 kernel are gone).
+// A table, not a formula, so that it can follow ptxas's register allocation per K; DESIGN.md "Score kernel".
+static const double kStepCostExact[SDP_MAX_K] = {3.49, 4.5, 5.37, 6.48, 7.47, 8.4, 9.46, 10.54, 11.39, 12.37, 13.52, 14.63, 15.56, 16.46, 17.57, 18.49, 19.65, 20.48, 21.6, 22.87, 23.79, 24.95, 26.21, 26.9, 28.09, 29.27, 30.13, 30.86, 32.22, 33.02, 33.24, 35.01};
+static const double kStepCostPadded[SDP_MAX_K] = {3.91, 4.97, 5.97, 6.82, 7.75, 8.78, 9.97, 10.81, 11.85, 12.73, 13.85, 14.93, 16.17, 17.29, 17.78, 19.11, 19.97, 21.1, 22.09, 23.51, 24.22, 25.32, 26.67, 27.58, 28.59, 29.44, 30.79, 31.82, 32.64, 33.59, 34.75, 35.57};
 
 void choose_geometry(sdp_ctx* c, int force_g) {      // force_g: sdp_set_debug_route (geometry experiments), 0 = off
     struct Ent { uint16_t n, G, K, pad; };
@@ -262,7 +262,7 @@ void choose_geometry(sdp_ctx* c, int force_g) {      // force_g: sdp_set_debug_r
             if (force_g && G != force_g && (n + force_g - 1) / force_g <= SDP_MAX_K &&
                 force_g * ((n + force_g - 1) / force_g) - n < force_g) continue;
             double ppw = 2.0 * (32 / G);
-            double rows = (double)n + 300.0 + G - 1;
+            double rows = (double)n + 300.0 + 2.0 * (G - 1);        // two rows of skew per thread
             double thr = ppw / (rows * (G * K != n ? kStepCostPadded[K - 1] : kStepCostExact[K - 1]));
             if (thr > best) { best = thr; bG = G; bK = K; }
         }
