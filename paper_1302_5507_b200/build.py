@@ -3,7 +3,7 @@
 ``python -m paper_1302_5507_b200.build`` or ``build()`` from ``__graft_entry__``. Objects are
 compiled in parallel; the score and traceback-DP kernels are instantiated for 32 column counts x
 {forward, reverse, traceback} x {exact, padded}, split over sixteen K ranges by ``-DSDP_K_LO/-DSDP_K_HI``.
-The score kernels (``score_cubin.cu``) are compiled to cubins whose scoring constants are sentinel immediates;
+They (``score_cubin.cu``) are compiled to cubins whose scoring constants are sentinel immediates;
 the cubins are embedded in the library as data (``.incbin``) and patched per context at load time
 (``score_modules.cu``). The build checks that every sentinel sits only where the loader looks for it.
 """
@@ -44,7 +44,8 @@ def _deps_hash(extra: str) -> str:
     return h.hexdigest()
 
 
-SENTINELS = {"negOc": 0x5D1A37C2, "negO": 0x2B6E4A91, "c2": 0x63C5195D, "Cd": 0x39E2746B, "e2": 0x1F83528E}   # score_kernel.cuh
+SENTINELS = {"negOc": 0x5D1A37C2, "negO": 0x2B6E4A91, "c2": 0x63C5195D, "Cd": 0x39E2746B, "e2": 0x1F83528E,   # score_kernel.cuh
+             "t_negOf": 0x4E2B7D13, "t_negOe": 0x2D9C51E6, "t_c8": 0x35A8C6F1, "t_Cd8": 0x3B5E92A7}              # trace_kernel.cuh
 
 
 def _units():
@@ -52,8 +53,6 @@ def _units():
              ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("mate", "mate.cu", []),
              ("score_modules", "score_modules.cu", []), ("slow_lane", "slow_lane.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
-        units.append((f"score_r{r}", "score_inst.cu",
-                      [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}", f"-DSDP_T_FN=launch_trace_r{r}"]))
         units.append((f"cubin_r{r}", "score_cubin.cu", [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}"]))
     return units
 

@@ -250,15 +250,6 @@ __device__ __forceinline__ void fill_ring_rows(const ScoreParams& P, const RingG
 #define SDP_ROWS_UNROLL 8
 #endif
 
-// Rows between neighbouring threads of a group: thread g works on row s - SDP_SCORE_SKEW*g at step s. With 1 the
-// H'/E' a thread receives at step s were finished by its left neighbour at the very end of step s-1, so the serial
-// chains of consecutive steps cannot overlap and a warp waits out the ALU latency between dependent chain
-// instructions (measured: a third of the issue slots idle). With 2 they were finished at step s-2: the chains of two
-// consecutive steps are independent (row i+1 only trails row i by a column inside the thread) and ptxas interleaves them.
-#ifndef SDP_SCORE_SKEW
-#define SDP_SCORE_SKEW 2
-#endif
-
 // resident CTAs per SM the register budget is sized for: 128 registers up to K = 21, 168 above
 #ifndef SDP_SCORE_MIN_CTAS
 #define SDP_SCORE_MIN_CTAS(K) ((K) <= 21 ? 4 : 3)

@@ -12,7 +12,7 @@
 #include <string.h>
 
 #include "sdp_host.cuh"
-#include "score_kernel.cuh"
+#include "trace_kernel.cuh"
 
 #define SDP_UNIT_SYMS(r) extern "C" const unsigned char sdp_cubin_r##r##_start[], sdp_cubin_r##r##_end[];
 SDP_UNIT_SYMS(0) SDP_UNIT_SYMS(1) SDP_UNIT_SYMS(2) SDP_UNIT_SYMS(3) SDP_UNIT_SYMS(4) SDP_UNIT_SYMS(5) SDP_UNIT_SYMS(6)
@@ -47,8 +47,9 @@ constexpr uint64_t kShfExecinstr = 4;
 // in hits[], or false when the image is not a well-formed ELF64.
 bool patch_score_image(unsigned char* img, size_t len, const ScorePatch& pv, uint32_t hits[SDP_N_SENTINELS])
 {
-    static const uint32_t sent[SDP_N_SENTINELS] = {SDP_SENT_NEGOC, SDP_SENT_NEGO, SDP_SENT_C2, SDP_SENT_CD, SDP_SENT_E2};
-    const uint32_t val[SDP_N_SENTINELS] = {pv.negOc, pv.negO, pv.c2, pv.Cd, pv.e2};
+    static const uint32_t sent[SDP_N_SENTINELS] = {SDP_SENT_NEGOC, SDP_SENT_NEGO, SDP_SENT_C2, SDP_SENT_CD, SDP_SENT_E2,
+                                                   SDP_SENT_T_NEGOF, SDP_SENT_T_NEGOE, SDP_SENT_T_C8, SDP_SENT_T_CD8};
+    const uint32_t val[SDP_N_SENTINELS] = {pv.negOc, pv.negO, pv.c2, pv.Cd, pv.e2, pv.t_negOf, pv.t_negOe, pv.t_c8, pv.t_Cd8};
     for (int k = 0; k < SDP_N_SENTINELS; ++k) hits[k] = 0;
     if (len < sizeof(Elf64Hdr) || memcmp(img, "\177ELF", 4) != 0 || img[4] != 2 || img[5] != 1) return false;
     Elf64Hdr eh; memcpy(&eh, img, sizeof(eh));
@@ -98,6 +99,16 @@ static int load_unit(ScoreModules* m, const ScorePatch& pv, int r, char* err, si
     }
     m->loaded[r] = 1;
     for (int K = 2 * r + 1; K <= 2 * r + 2; ++K)
+        for (int pad = 0; pad < 2; ++pad) {
+            char name[64];
+            snprintf(name, sizeof(name), "sdp_trace_k%d_%c", K, pad ? 'p' : 'e');
+            const cudaError_t g = cudaLibraryGetKernel(&m->kern_trace[K][pad], m->lib[r], name);
+            if (g != cudaSuccess) {
+                snprintf(err, errlen, "cudaLibraryGetKernel(%s): %s", name, cudaGetErrorString(g));
+                return SDP_ECUDA;
+            }
+        }
+    for (int K = 2 * r + 1; K <= 2 * r + 2; ++K)
         for (int rev = 0; rev < 2; ++rev)
             for (int pad = 0; pad < 2; ++pad) {
                 char name[64];
@@ -112,7 +123,7 @@ static int load_unit(ScoreModules* m, const ScorePatch& pv, int r, char* err, si
 }
 
 int score_modules_launch(ScoreModules* m, const ScorePatch& pv, int K, bool pad, bool rev, const ScoreParams& p,
-                         cudaStream_t st, char* err, size_t errlen)
+                         const TraceDP* td, cudaStream_t st, char* err, size_t errlen)
 {
     const uint32_t ntasks = p.task_end - p.task_begin;
     if (ntasks == 0) return SDP_OK;
@@ -124,9 +135,10 @@ int score_modules_launch(ScoreModules* m, const ScorePatch& pv, int K, bool pad,
     }
     const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
     ScoreParams arg = p;
-    void* args[1] = {&arg};
-    const cudaError_t e = cudaLaunchKernel((const void*)m->kern[K][rev ? 1 : 0][pad ? 1 : 0], dim3(grid), dim3(SDP_SCORE_THREADS),
-                                           args, 0, st);
+    TraceDP targ = td ? *td : TraceDP{};
+    void* args[2] = {&arg, &targ};
+    const cudaKernel_t kern = td ? m->kern_trace[K][pad ? 1 : 0] : m->kern[K][rev ? 1 : 0][pad ? 1 : 0];
+    const cudaError_t e = cudaLaunchKernel((const void*)kern, dim3(grid), dim3(SDP_SCORE_THREADS), args, 0, st);
     if (e != cudaSuccess) { snprintf(err, errlen, "score kernel launch (K = %d): %s", K, cudaGetErrorString(e)); return SDP_ECUDA; }
     return SDP_OK;
 }

@@ -17,18 +17,6 @@
 
 using namespace sdp;
 
-namespace sdp {
-#define SDP_SCORE_UNITS(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15)
-#define SDP_DECL(r) bool launch_trace_r##r(int, bool, const ScoreParams&, const TraceDP&, cudaStream_t);
-SDP_SCORE_UNITS(SDP_DECL)
-#undef SDP_DECL
-void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st) {
-#define SDP_TRY(r) if (launch_trace_r##r(K, pad, p, t, st)) return;
-    SDP_SCORE_UNITS(SDP_TRY)
-#undef SDP_TRY
-}
-}  // namespace sdp
-
 namespace {
 
 struct DevBuf {
@@ -313,32 +301,29 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
     {   // score kernel (score_kernel.cuh): c = 2e + mismatch; F~ = F' - c starts at 0 = "minus infinity", which needs
         // beta >= 2o + c
         const int c = 2 * e + s->mismatch, beta_s = 3 * o + 8 + (c > 0 ? c : 0);
-        ctx->patch = ScorePatch{sdp_pack2(-(o + c)), sdp_pack2(-o), sdp_pack2(c), sdp_pack2(s->match - s->mismatch), sdp_pack2(e)};
+        ctx->patch.negOc = sdp_pack2(-(o + c)); ctx->patch.negO = sdp_pack2(-o); ctx->patch.c2 = sdp_pack2(c);
+        ctx->patch.Cd = sdp_pack2(s->match - s->mismatch); ctx->patch.e2 = sdp_pack2(e);
         score_modules_init(&ctx->modules);
         ctx->consts.beta2 = sdp_pack2(beta_s);
         ctx->consts.betaMinusO2 = sdp_pack2(beta_s - o);
         ctx->consts.e = e; ctx->consts.beta = beta_s; ctx->consts.match = s->match;
     }
-    {   // traceback DP kernel: x8 scaled values with tags in the low three bits (trace_kernel.cuh)
-        const int sc8 = SDP_TB_SCALE;
-        const int qm = sc8 * (2 * e + s->match) + 7, qx = sc8 * (2 * e + s->mismatch) + 7;
+    {   // traceback DP kernels (trace_kernel.cuh, thin_kernel.cu): x8 scaled values with tags in the low three bits,
+        // F and u shifted by c = 2e + mismatch as in the score kernel
+        const int sc8 = SDP_TB_SCALE, c = 2 * e + s->mismatch, beta_t = 3 * o + 8 + (c > 0 ? c : 0);
         TraceConsts& t = ctx->tconsts;
-        t.m4 = 0x00040004u; t.cm1 = 0xFFFFFFFFu;
-        t.negO_e = sdp_pack2(-sc8 * o + 1);
-        t.negO_f = sdp_pack2(-sc8 * o + 6);
-        t.qx = sdp_pack2(qx);
-        t.Cd8 = sdp_pack2(sc8 * (s->match - s->mismatch));
         t.e2 = sdp_pack2(sc8 * e);
-        t.beta2 = sdp_pack2(sc8 * beta);
-        t.betaMinusO2 = sdp_pack2(sc8 * (beta - o));
-        t.e = e; t.beta = beta;
-        // the diagonal increment is added with a 32-bit IMAD: it must be non-negative in both lanes,
-        // and the match increment must stay an fp16 denormal bit pattern
-        ctx->wide_ok = (qx >= 0 && qm < 2048 && sc8 * beta <= 32000) ? 1 : 0;
+        t.beta2 = sdp_pack2(sc8 * beta_t + 7);
+        t.betaMinusO2 = sdp_pack2(sc8 * (beta_t - o) + 7);
+        t.e = e; t.beta = beta_t;
+        ctx->patch.t_negOf = sdp_pack2(sc8 * (-o - c) - 1);
+        ctx->patch.t_negOe = sdp_pack2(-sc8 * o - 6);
+        ctx->patch.t_c8 = sdp_pack2(sc8 * c);
+        ctx->patch.t_Cd8 = sdp_pack2(sc8 * (s->match - s->mismatch));
+        // 8 (match - mismatch) must read as an fp16 value below 1.0, and 8 beta must leave room in 16 bits
+        ctx->thin_ok = (sc8 * (s->match - s->mismatch) < 0x3C00 && sc8 * beta_t <= 32000) ? 1 : 0;
+        ctx->wide_ok = ctx->thin_ok;
         ctx->wide_fits = ctx->wide_ok;
-        // narrow-band kernel: 8 (match - mismatch) must read as an fp16 value below 1.0, 8 beta must leave room
-        const int c = 2 * e + s->mismatch;
-        ctx->thin_ok = (sc8 * (s->match - s->mismatch) < 0x3C00 && sc8 * (beta + (c > 0 ? c : 0)) <= 32000) ? 1 : 0;
     }
     choose_geometry(ctx, 0);
 
@@ -516,10 +501,9 @@ static int launch_score_stage(sdp_ctx* ctx, Lane& L, int which, const PairDesc* 
         sp.slot_lo = s0; sp.slot_hi = s1; sp.task_begin = t0; sp.task_end = t1;
         cudaStream_t ls = (do_fan && (turn % SDP_FAN_STREAMS)) ? fan[turn % SDP_FAN_STREAMS] : st;
         ++turn;
-        if (which == 2) launch_trace(cls >> 1, (cls & 1) != 0, sp, td, ls);
-        else {
-            const int rc = score_modules_launch(&ctx->modules, ctx->patch, cls >> 1, (cls & 1) != 0, rev, sp, ls, ctx->err,
-                                                sizeof(ctx->err));
+        {
+            const int rc = score_modules_launch(&ctx->modules, ctx->patch, cls >> 1, (cls & 1) != 0, rev, sp,
+                                                which == 2 ? &td : nullptr, ls, ctx->err, sizeof(ctx->err));
             if (rc != SDP_OK) return rc;
         }
         ++*nlaunch;

@@ -30,21 +30,23 @@ void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint6
 
 // ---- score_modules.cu: the score kernels, loaded per context with the scoring patched into their immediates
 constexpr int SDP_SCORE_UNITS_N = 16;     // cubins, two column counts each (K = 2r+1, 2r+2)
-constexpr int SDP_N_SENTINELS = 5;
-struct ScorePatch { uint32_t negOc, negO, c2, Cd, e2; };       // packed int16x2 values, see score_kernel.cuh
+constexpr int SDP_N_SENTINELS = 9;
+struct ScorePatch {                                            // packed int16x2 values
+    uint32_t negOc, negO, c2, Cd, e2;                          // score kernels, see score_kernel.cuh
+    uint32_t t_negOf, t_negOe, t_c8, t_Cd8;                    // traceback DP kernels, see trace_kernel.cuh
+};
 struct ScoreModules {
     cudaLibrary_t lib[SDP_SCORE_UNITS_N];
     unsigned char loaded[SDP_SCORE_UNITS_N];
     cudaKernel_t kern[SDP_MAX_K + 1][2][2];                     // [K][reverse][padded]
+    cudaKernel_t kern_trace[SDP_MAX_K + 1][2];                  // [K][padded]
 };
 void score_modules_init(ScoreModules* m);
 void score_modules_destroy(ScoreModules* m);
 bool patch_score_image(unsigned char* img, size_t len, const ScorePatch& pv, uint32_t hits[SDP_N_SENTINELS]);
+// td == nullptr: the score kernel (forward, or reverse with rev); else the traceback DP kernel
 int score_modules_launch(ScoreModules* m, const ScorePatch& pv, int K, bool pad, bool rev, const ScoreParams& p,
-                         cudaStream_t st, char* err, size_t errlen);
-
-// ---- score_inst.cu (compiled once per K range): the traceback DP kernels
-void launch_trace(int K, bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st);
+                         const TraceDP* td, cudaStream_t st, char* err, size_t errlen);
 
 // ---- traceback.cu
 struct PostParams {

@@ -14,6 +14,16 @@
 #define SDP_RING_WORDS 1792     // shared-memory words per warp for the window-row selector rings
 #define SDP_KEY_SKIP 0xFFFFFFFFu
 
+// Rows between neighbouring threads of a group: thread g works on row s - SDP_SCORE_SKEW*g at step s. With 1 the
+// H'/E' a thread receives at step s were finished by its left neighbour at the very end of step s-1, so the serial
+// chains of consecutive steps cannot overlap and a warp waits out the ALU latency between dependent chain
+// instructions (measured: a third of the issue slots idle). With 2 they were finished at step s-2: the chains of two
+// consecutive steps are independent (row i+1 only trails row i by a column inside the thread) and ptxas interleaves them.
+#ifndef SDP_SCORE_SKEW
+#define SDP_SCORE_SKEW 2
+#endif
+
+
 // device-side error flag bits
 #define SDP_ERRF_INDEX   1u     // pair index / offset out of range, empty sequence
 #define SDP_ERRF_REVERSE 2u     // reverse pass did not reproduce the forward score (internal)
@@ -74,15 +84,12 @@ struct ScoreParams {
 // carry "which operand won" tags. All fields are packed int16x2 unless noted.
 #define SDP_TB_SCALE 8
 #define SDP_TB_MAX_VALUE 4090   // largest unscaled drift-form value: 8 * 4090 + 7 <= 32767
-struct TraceConsts {
-    uint32_t cm1;                  // 0xFFFFFFFF (-1), opaque multiplier: subtractions as IMAD on the FMA pipe
-    uint32_t m4;                   // 0x00040004, opaque so that the tag select stays one LOP3
-    uint32_t negO_e;               // 8 * (-o) + 1 : "I opened here" candidate (tag bit 0)
-    uint32_t negO_f;               // 8 * (-o) + 6 : "D opened here" candidate (tag bit 2); D extended carries tag 2
-    uint32_t qx;                   // 8 * (2e + mismatch) + 7 : diagonal increment of a mismatch, tag 7
-    uint32_t Cd8;                  // fp16 denormal whose bits are 8 * (match - mismatch)
-    uint32_t e2, beta2, betaMinusO2;   // 8e, 8 beta, 8 (beta - o)
-    int32_t  e, beta;              // unscaled
+struct TraceConsts {            // arguments of the traceback DP kernels; the constants of their column loop are patched
+                                // instruction immediates like the score kernels' (trace_kernel.cuh, ScorePatch)
+    uint32_t e2;                   // packed 8 e
+    uint32_t beta2;                // packed 8 beta + 7          : H7(i_lo, 0)
+    uint32_t betaMinusO2;          // packed 8 (beta - o) + 7    : H7(i_lo, j >= 1)
+    int32_t  e, beta;              // unscaled; beta = 3o + 8 + max(2e + mismatch, 0)
 };
 
 struct TraceDP {

@@ -3,8 +3,9 @@
 // The paper backtracks through tables D and M kept in global memory. Here no table
 // survives the forward pass; instead the rectangle of window rows (i_lo, i_end] x all n read
 // columns that contains every co-optimal path is recomputed with the same register-resident
-// anti-diagonal wavefront as the score kernel (score_kernel.cuh), and each cell leaves FOUR BITS
-// behind instead of two table entries:
+// anti-diagonal wavefront as the score kernel (score_kernel.cuh: two rows of skew per thread, two rows per pass,
+// scoring constants as patched instruction immediates), and each cell leaves FOUR BITS behind instead of two
+// table entries:
 //     bits 1..0  where M(i,j) came from: 3 = diagonal, 2 = D(i,j), 0/1 = I(i,j)   (diag > D > I)
 //     bit  2     D(i,j) was opened from M(i-1,j)   (else extended from D(i-1,j))
 //     bit  3     I(i,j) was opened from M(i,j-1)   (else extended from I(i,j-1))
@@ -13,43 +14,69 @@
 // The bits are free by-products of the max instructions: every value is stored x8 and the three
 // low bits of a candidate are a tag chosen so that (a) ties between candidates of equal value are
 // won by the candidate the tie rule prefers (diag 7 > D opened 6 > D extended 2 > I opened 1 >
-// I extended 0) and (b) the winner's tag survives in the low bits of the result:
-//     Et = max(Hc(i,j-1) - 8o + 1, Ec(i,j-1))             VIADDMNMX   tag bit 0 = opened
-//     Ft = max(Hc(i-1,j) - 8o + 6, Fc(i-1,j) [= 8v+2])    VIADDMNMX   tag bit 2 = opened
-//     u  = max(Hc(i-1,j-1) + q8, Ft)                      VIADDMNMX   q8 = 8(2e+delta)+7, exact (fp16 pipe,
-//     Ht = max(u, Et)                                     VIMNMX           as in score_kernel.cuh)
-//     Ec = Et & ~1, Fc = Ft & ~4, Hc = Ht & ~7            3 LOP3      clean values for the next cell
-//     v  = Ht & ~4 | Ft & 4                               1 LOP3
+// I extended 0) and (b) the winner's tag survives in the low bits of the result. With c = 2e + mismatch,
+// q' = delta - mismatch, F~ = F' - c as in the score kernel, and H kept as H7 = H | 7 (the diagonal tag rides on it):
+//     Ft = max(H7(i-1,j) + 8(-o-c) - 1, Fc(i-1,j))      VIADDMNMX    Fc = Ft & ~4 (tag 2)       LOP3
+//     u  = max(H7(i-1,j-1) + 8q', Ft)                   VIADDMNMX    8q' exact from the fp16 pipe (HADD2 + HFMA2.RELU)
+//     Et = max(H7(i,j-1) - 8o - 6, Ec(i,j-1))           VIADDMNMX    Ec = Et & ~1               LOP3
+//     Ht = max(u + 8c, Et)                              VIADDMNMX    H7 = Ht | 7                LOP3
+//     v  = Ht & ~4 | Ft & 4                                                                     LOP3
 // Eight ALU-pipe instructions per two cells (two pairs share the int16x2 lanes) against four in
-// the score kernel. The nibble (v - Hc) + 8 (Et - Ec) and its packing run on the FMA pipe: the two
-// subtractions are 32-bit IMADs (an IMAD costs two HFMA2 slots on sm_100a, but masking the tags out with
-// two more LOP3 instead loads the ALU pipe, which is this kernel's bottleneck: measured 6 % slower), then fp16
-// FMAs on the small integers as DENORMALS (t = eb*8 + nib, byte = t0*16 + t1: exact below 2048),
-// and one PRMT per four cells joins two bytes. Nibbles are left-aligned, four cells per 16-bit
-// lane (cell kk of a word in bits 4*(3 - kk)), and stored row by row:
+// the score kernel. The nibble (H7 - v) + 8 (Et - Ec) -- the three low bits COMPLEMENTED, the walk undoes that -- and
+// its packing run on the FMA pipe: two integer subtractions, then fp16 FMAs on the small integers as DENORMALS
+// (t = eb*8 + x, byte = t0*16 + t1: exact below 2048), and one PRMT per four cells joins two bytes. Nibbles are
+// left-aligned, four cells per 16-bit lane (cell kk of a word in bits 4*(3 - kk)), and stored step by step:
 //     word((i, w, lane)) = task region + ((s-1) * ceil(K/4) + w) * 32 + lane,   low half = first pair of the two,
-// where s = i + g is the STEP at which thread g of its group works on row i: the threads of a warp are on
-// different rows at any one time (anti-diagonal wavefront), so only a step-major layout makes a warp-wide
-// store one 128-byte line. One region of (rows + G - 1) steps per warp task.
+// where s = i + SDP_SCORE_SKEW*g is the STEP at which thread g of its group works on row i: the threads of a warp are
+// on different rows at any one time (anti-diagonal wavefront), so only a step-major layout makes a warp-wide
+// store one 128-byte line. One region of (rows + SKEW*(G - 1)) steps per warp task.
 #pragma once
 #include "score_kernel.cuh"
 
 namespace sdp {
 
-// bitwise (mask ? b : a) in one LOP3 (mask kept in a register: a LOP3 takes one immediate at most)
-__device__ __forceinline__ uint32_t imad_u(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t r; asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c)); return r;
+// sentinel immediates of the traceback DP kernels (patched like the score kernels', score_modules.cu)
+#define SDP_SENT_T_NEGOF 0x4E2B7D13u    // packed 8 (-o - c) - 1
+#define SDP_SENT_T_NEGOE 0x2D9C51E6u    // packed -8 o - 6
+#define SDP_SENT_T_C8    0x35A8C6F1u    // packed 8 c
+#define SDP_SENT_T_CD8   0x3B5E92A7u    // packed 8 (match - mismatch), read as an fp16 pair
+
+__device__ __forceinline__ uint32_t sub_u32(uint32_t a, uint32_t b) {
+    uint32_t r; asm("sub.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b)); return r;
 }
+// bitwise (mask ? b : a) in one LOP3
 __device__ __forceinline__ uint32_t lop3_select(uint32_t a, uint32_t b, uint32_t mask) {
     uint32_t r; asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(r) : "r"(a), "r"(b), "r"(mask)); return r;
 }
 
+// nibble packer of one row: four cells -> one 32-bit word (16 bits per int16 lane)
+struct NibblePack {
+    uint32_t t0, b0, b1;
+    __device__ __forceinline__ void reset() { t0 = 0u; b0 = 0u; b1 = 0u; }
+    // returns true when `word` is complete (after cell k with k % 4 == 3 or k == last)
+    template <int K>
+    __device__ __forceinline__ bool add(const int k, const uint32_t t, uint32_t& word) {
+        constexpr uint32_t H2_16 = 0x4C004C00u;            // fp16 16.0, both lanes
+        if ((k & 1) == 0) t0 = t;
+        if ((k & 1) == 1 || k == K - 1) {
+            const uint32_t byte = (k & 1) ? hfma2_u(t0, H2_16, t) : hfma2_u(t0, H2_16, 0u);
+            if ((k & 3) < 2) b0 = byte; else b1 = byte;
+        }
+        if ((k & 3) == 3 || k == K - 1) {
+            if ((k & 3) < 2) b1 = 0u;
+            word = __byte_perm(b1, b0, 0x6240);
+            return true;
+        }
+        return false;
+    }
+};
+
 template <int K, bool PAD>
-__global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))
-trace_kernel(const ScoreParams P, const TraceDP T)
+__device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& T, uint32_t (*ring_mem)[SDP_RING_WORDS])
 {
-    __shared__ uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];
     constexpr int NW = (K + 3) / 4;
+    constexpr int SKEW = SDP_SCORE_SKEW;
+    static_assert(SKEW == 2, "the row-pair pass below assumes two rows of skew");
     const int lane = threadIdx.x & 31;
     const uint32_t task = P.task_begin + blockIdx.x * SDP_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (task >= P.task_end) return;                       // warp-uniform
@@ -91,7 +118,7 @@ trace_kernel(const ScoreParams P, const TraceDP T)
     const uint32_t skipmask = (skipA ? 0x0000FFFFu : 0u) | (skipB ? 0xFFFF0000u : 0u);
 
     uint32_t rh[K], H[K], F[K];
-    const uint32_t h_row0 = T.c.betaMinusO2;              // 8 (H'(0,j)) = 8 (beta - o) for j >= 1
+    const uint32_t h_row0 = T.c.betaMinusO2;              // H7(0,j) = 8 (beta - o) + 7 for j >= 1
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         uint32_t cA = SDP_CODE_READ_N, cB = SDP_CODE_READ_N;
@@ -102,25 +129,43 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         F[k] = 0x00020002u;                               // D(0,j) = -inf, carrying the "extended" tag
     }
 
-    const RingGeom rg = ring_geometry(G, ngroups, 1);
+    const RingGeom rg = ring_geometry(G, ngroups, SKEW);
     uint32_t* const ring_w = ring_mem[threadIdx.x >> 5] + q * rg.stride_w;
-    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - g;
+    const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - SKEW * g;
 
     const bool st_ok = hasA;                              // hasB implies hasA
     constexpr uint32_t rowstride = 32u * NW;              // word (step, w, lane): a warp-wide store is one 128-byte line
     uint32_t* wp = T.bits + T.bits_off[first] + (uint32_t)lane;
 
-    const uint32_t m4 = T.c.m4, Cd8 = T.c.Cd8, cm1 = T.c.cm1;
-    const uint32_t negOe = T.c.negO_e, negOf = T.c.negO_f, qx = T.c.qx, e2 = T.c.e2;
-    constexpr uint32_t H2_8 = 0x48004800u, H2_16 = 0x4C004C00u;        // fp16 8.0 and 16.0, both lanes
-    const uint32_t notfirst = opaque_u32(is_first ? 0u : 0xFFFFFFFFu);   // a mask, not a predicate: one LOP3 per use
-    uint32_t fv = is_first ? T.c.beta2 : 0u;              // 8 H'(i,0) = 8 (beta + e i): free start
-    const uint32_t fstep = is_first ? e2 : 0u;
-    uint32_t hout = h_row0, eout = 0u;
+    constexpr uint32_t negOf = SDP_SENT_T_NEGOF, negOe = SDP_SENT_T_NEGOE, c8 = SDP_SENT_T_C8, Cd8 = SDP_SENT_T_CD8;
+    constexpr uint32_t H2_8 = 0x48004800u;                // fp16 8.0, both lanes
+    const uint32_t notfirst = opaque_u32(is_first ? 0u : 1u);            // multiplier: the select stays on the FMA pipe
+    uint32_t fv = is_first ? T.c.beta2 : 0u;              // H7(i,0) = 8 (beta + e i) + 7: free start
+    const uint32_t fstep = is_first ? T.c.e2 : 0u;
+    uint32_t houtA = h_row0, eoutA = 0u, houtB = h_row0, eoutB = 0u;     // the two rows in flight towards the right neighbour
     uint32_t hdiag = is_first ? T.c.beta2 : h_row0;
-    uint32_t fin = 0u;                                    // 8 H'(m, n) per lane, caught on the lane's last row
+    uint32_t fin = 0u;                                    // H7(m, n) per lane, caught on the lane's last row
 
-    auto row_step = [&](const int i, const uint16_t* rp, auto slow_tag, const uint32_t (&Hs)[K], uint32_t (&Hn)[K]) {
+    // one cell of two pairs: updates F (tag 2), E (tag 0), Hl (H7); returns the packed nibble value as an fp16 denormal
+    auto cell = [&](const uint32_t hd, const uint32_t hup, uint32_t& Fk, const uint32_t nt, const uint32_t rcode,
+                    uint32_t& Hl, uint32_t& E) -> uint32_t {
+        const uint32_t qv = hfma2_relu_negsq(hsub2_u(nt, rcode), Cd8);
+        const uint32_t Ft = __viaddmax_s16x2(hup, negOf, Fk);
+        const uint32_t u = __viaddmax_s16x2(hd, qv, Ft);
+        const uint32_t Et = __viaddmax_s16x2(Hl, negOe, E);
+        const uint32_t Ht = __viaddmax_s16x2(u, c8, Et);
+        Fk = Ft & 0xFFFBFFFBu;
+        E = Et & 0xFFFEFFFEu;
+        Hl = Ht | 0x00070007u;
+        const uint32_t v = lop3_select(Ht, Ft, 0x00040004u);
+        const uint32_t x = sub_u32(Hl, v);                // 7 - (Ht&3 | Ft&4) per lane, no borrow (Hl >= v per lane)
+        const uint32_t eb = sub_u32(Et, E);               // Et & 1 per lane
+        return hfma2_u(eb, H2_8, x);                      // x + 8 eb as fp16 denormals: exact
+    };
+
+    // One DP row of this thread's K columns (fill, drain and odd rows). Hs = H7(i-1, .) is only read, Hn receives H7(i, .).
+    auto row_step = [&](const int i, const uint16_t* rp, auto slow_tag, const uint32_t (&Hs)[K], uint32_t (&Hn)[K],
+                        uint32_t& hout, uint32_t& eout) {
         constexpr bool SLOW = decltype(slow_tag)::value;
         uint32_t hin = __shfl_up_sync(0xffffffffu, hout, 1);
         uint32_t ein = __shfl_up_sync(0xffffffffu, eout, 1);
@@ -131,44 +176,24 @@ trace_kernel(const ScoreParams P, const TraceDP T)
             return;
         }
         fv = __vadd2(fv, fstep);
-        hin = (hin & notfirst) | fv;
-        ein = ein & notfirst;
+        hin = imad_sel(hin, notfirst, fv);
+        ein = imad_sel(ein, notfirst, 0u);
         const uint32_t nt = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)*rp);
-        // (thread g runs G-1-g rows past Mmin inside the steady-state loop: always test the row)
+        // (thread g runs SKEW*(G-1-g) rows past Mmin inside the steady-state loop: always test the row)
         const bool do_store = st_ok && i <= Rpp;
 
         uint32_t Hl = hin, E = ein;
         uint32_t Hsk = hin, Esk = ein;
         uint32_t hd = hdiag;
         hdiag = hin;
-        uint32_t b0 = 0u, b1 = 0u, t0 = 0u;              // high byte, low byte of the current word; first nibble of a byte
+        NibblePack np; np.reset();
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const uint32_t q8 = hfma2_u(hfma2_is_zero(hsub2_u(nt, rh[k])), Cd8, qx);
-            const uint32_t Ft = __viaddmax_s16x2(Hs[k], negOf, F[k]);
-            F[k] = Ft & 0xFFFBFFFBu;
-            const uint32_t u = __viaddmax_s16x2(hd, q8, Ft);
+            const uint32_t t = cell(hd, Hs[k], F[k], nt, rh[k], Hl, E);
             hd = Hs[k];
-            const uint32_t Et = __viaddmax_s16x2(Hl, negOe, E);
-            E = Et & 0xFFFEFFFEu;
-            const uint32_t Ht = __vmaxs2(u, Et);
-            Hl = Ht & 0xFFF8FFF8u;
             Hn[k] = Hl;
-            const uint32_t v = lop3_select(Ht, Ft, m4);
-            // v - Hc and Et - Ec as 32-bit IMADs (no borrow crosses the lanes: Hc <= v, Ec <= Et per lane). An IMAD
-            // costs two FMA-pipe slots, but the ALU pipe is this kernel's bottleneck and the FMA pipe has room.
-            const uint32_t nib = imad_u(Hl, cm1, v);      // bits 2..0
-            const uint32_t eb = imad_u(E, cm1, Et);       // 0 or 1
-            const uint32_t t = hfma2_u(eb, H2_8, nib);    // nib + 8 eb as fp16 denormals: exact
-            if ((k & 1) == 0) t0 = t;
-            if ((k & 1) == 1 || k == K - 1) {
-                const uint32_t byte = (k & 1) ? hfma2_u(t0, H2_16, t) : hfma2_u(t0, H2_16, 0u);
-                if ((k & 3) < 2) b0 = byte; else b1 = byte;
-            }
-            if ((k & 3) == 3 || k == K - 1) {
-                if ((k & 3) < 2) b1 = 0u;
-                if (do_store) wp[(k >> 2) * 32] = __byte_perm(b1, b0, 0x6240);
-            }
+            uint32_t word;
+            if (np.template add<K>(k, t, word)) { if (do_store) wp[(k >> 2) * 32] = word; }
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }
         wp += rowstride;
@@ -179,14 +204,73 @@ trace_kernel(const ScoreParams P, const TraceDP T)
             if (i == mB) fin = (fin & 0x0000FFFFu) | (Hl & 0xFFFF0000u);
         }
     };
+    // Two consecutive steps of the steady state (rows ia and ia + 1 of this thread) as ONE skewed pass, as in the score
+    // kernel: column k of the first row, then column k-1 of the second, whose "row above" is the first row's chain value.
+    auto row_pair = [&](const int ia, const uint16_t* rp) {
+        uint32_t hinA = __shfl_up_sync(0xffffffffu, houtA, 1);
+        uint32_t einA = __shfl_up_sync(0xffffffffu, eoutA, 1);
+        uint32_t hinB = __shfl_up_sync(0xffffffffu, houtB, 1);
+        uint32_t einB = __shfl_up_sync(0xffffffffu, eoutB, 1);
+        fv = __vadd2(fv, fstep);
+        hinA = imad_sel(hinA, notfirst, fv);
+        einA = imad_sel(einA, notfirst, 0u);
+        fv = __vadd2(fv, fstep);
+        hinB = imad_sel(hinB, notfirst, fv);
+        einB = imad_sel(einB, notfirst, 0u);
+        const uint32_t ntA = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[0]);
+        const uint32_t ntB = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[1]);
+        const bool storeA = st_ok && ia <= Rpp, storeB = st_ok && ia + 1 <= Rpp;
+
+        uint32_t HlA = hinA, EA = einA, HlB = hinB, EB = einB;
+        uint32_t hdA = hdiag, hdB = hinA;                 // H7(ia-1, left), H7(ia, left)
+        hdiag = hinB;
+        uint32_t HskA = hinA, EskA = einA, HskB = hinB, EskB = einB;
+        uint32_t prevA = hinA;                            // H7(ia, k-1)
+        NibblePack npA, npB; npA.reset(); npB.reset();
+#pragma unroll
+        for (int k = 0; k <= K; ++k) {
+            const uint32_t upB = prevA;                   // H7(ia, k-1): the second row's "row above" at column k-1
+            if (k < K) {                                  // first row, column k
+                const uint32_t t = cell(hdA, H[k], F[k], ntA, rh[k], HlA, EA);
+                hdA = H[k];
+                prevA = HlA;
+                uint32_t word;
+                if (npA.template add<K>(k, t, word)) { if (storeA) wp[(k >> 2) * 32] = word; }
+                if (PAD && k == K - 2) { HskA = HlA; EskA = EA; }
+            }
+            if (k >= 1) {                                 // second row, column k-1
+                const uint32_t t = cell(hdB, upB, F[k - 1], ntB, rh[k - 1], HlB, EB);
+                hdB = upB;
+                H[k - 1] = HlB;
+                uint32_t word;
+                if (npB.template add<K>(k - 1, t, word)) { if (storeB) wp[rowstride + ((k - 1) >> 2) * 32] = word; }
+                if (PAD && k - 1 == K - 2) { HskB = HlB; EskB = EB; }
+            }
+        }
+        wp += 2 * rowstride;
+        if (PAD) {
+            houtA = blend(skipmask, HskA, HlA); eoutA = blend(skipmask, EskA, EA);
+            houtB = blend(skipmask, HskB, HlB); eoutB = blend(skipmask, EskB, EB);
+        } else { houtA = HlA; eoutA = EA; houtB = HlB; eoutB = EB; }
+        if (is_last) {
+            if (ia == mA) fin = (fin & 0xFFFF0000u) | (HlA & 0x0000FFFFu);
+            if (ia == mB) fin = (fin & 0x0000FFFFu) | (HlA & 0xFFFF0000u);
+            if (ia + 1 == mA) fin = (fin & 0xFFFF0000u) | (HlB & 0x0000FFFFu);
+            if (ia + 1 == mB) fin = (fin & 0x0000FFFFu) | (HlB & 0xFFFF0000u);
+        }
+    };
+    // one step outside the paired loop; the two output sets trade places afterwards
     auto row_step1 = [&](const int i, const uint16_t* rp, auto slow_tag) {
         uint32_t H2[K];
-        row_step(i, rp, slow_tag, H, H2);
+        row_step(i, rp, slow_tag, H, H2, houtA, eoutA);
 #pragma unroll
         for (int k = 0; k < K; ++k) H[k] = H2[k];
+        const uint32_t th = houtA, te = eoutA;
+        houtA = houtB; eoutA = eoutB; houtB = th; eoutB = te;
     };
 
-    const int fast_end = Mmin + G - 1, all_end = Mmax + G - 1;
+    const int lead = SKEW * (G - 1);
+    const int fast_end = Mmin + lead, all_end = Mmax + lead;
     for (int s0 = 0; s0 < all_end; s0 += rg.chunk) {
         if (in_group) fill_ring_rows<false>(P, rg, ring_w, g, G, s0, dA.woff, mA, dB.woff, mB);
         __syncwarp();
@@ -194,34 +278,22 @@ trace_kernel(const ScoreParams P, const TraceDP T)
         const uint16_t* rp = rp0 + (s0 & (rg.ring - 1));
         int s = s0 + 1;
 #pragma unroll 1
-        for (; s <= min(send, G - 1); ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+        for (; s <= min(send, lead); ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
         const int fe = min(send, fast_end);
 #pragma unroll 1
-        for (; s + 1 <= fe; s += 2, rp += 2) {
-            uint32_t H2[K];
-            row_step(s - g, rp, std::false_type{}, H, H2);
-            row_step(s + 1 - g, rp + 1, std::false_type{}, H2, H);
-        }
-        if (s <= fe) { row_step1(s - g, rp, std::false_type{}); ++s; ++rp; }
+        for (; s + 1 <= fe; s += 2, rp += 2) row_pair(s - SKEW * g, rp);     // (four rows per iteration: measured slower)
 #pragma unroll 1
-        for (; s <= send; ++s, ++rp) row_step1(s - g, rp, std::true_type{});
+        for (; s <= fe; ++s, ++rp) row_step1(s - SKEW * g, rp, std::false_type{});
+#pragma unroll 1
+        for (; s <= send; ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
     }
 
     if (is_last) {
-        // the restricted DP must end on the forward score: 8 H'(m,n) = 8 (S + e (m + n) + beta)
+        // the restricted DP must end on the forward score: H7(m, n) = 8 (S + e (m + n) + beta) + 7
         const int fA = (int)(fin & 0xFFFFu) >> 3, fB = (int)(fin >> 16) >> 3;
         if (hasA && fA - T.c.beta - T.c.e * (nA + mA) != dA.aux) atomicOr(P.err_flag, SDP_ERRF_TRACE);
         if (hasB && fB - T.c.beta - T.c.e * (nB + mB) != dB.aux) atomicOr(P.err_flag, SDP_ERRF_TRACE);
     }
-}
-
-template <int K>
-static void launch_trace_K(bool pad, const ScoreParams& p, const TraceDP& t, cudaStream_t st) {
-    const uint32_t ntasks = p.task_end - p.task_begin;
-    if (ntasks == 0) return;
-    const uint32_t grid = (ntasks + SDP_WARPS_PER_CTA - 1) / SDP_WARPS_PER_CTA;
-    if (pad) trace_kernel<K, true><<<grid, SDP_SCORE_THREADS, 0, st>>>(p, t);
-    else     trace_kernel<K, false><<<grid, SDP_SCORE_THREADS, 0, st>>>(p, t);
 }
 
 }  // namespace sdp

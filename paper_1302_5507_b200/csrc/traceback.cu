@@ -89,7 +89,7 @@ __global__ void k_post_forward(const PostParams pp)
         const int c_shift = 2 * pp.sc.gap_extend + pp.sc.mismatch;
         const bool thin_fits = pp.thin_ok && vmax + (c_shift > 0 ? c_shift : 0) <= SDP_TB_MAX_VALUE;      // x8 tagged int16 lanes
         const bool narrow = !slow && (W == 0 || (W < THIN_NW && 2 * W + 1 < n + 1 && rows <= THIN_MAXROWS && thin_fits && !pp.no_thin));
-        const bool wide = !slow && !narrow && pp.wide_ok && vmax <= SDP_TB_MAX_VALUE;
+        const bool wide = !slow && !narrow && pp.wide_ok && vmax + (c_shift > 0 ? c_shift : 0) <= SDP_TB_MAX_VALUE;
         if (narrow) {
             ktb = (uint32_t)W * TB_KEY_STRIDE + (uint32_t)min((int)TB_KEY_STRIDE - 1, W ? rows : n);
             c_tb = (unsigned long long)bw * rows;
@@ -344,7 +344,7 @@ __global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_
     if (local % ppw == 0) {                               // first pair of a task owns the task's region
         int rows = 0;
         for (uint32_t t = 0; t < ppw && local + t < si.count; ++t) rows = max(rows, tb_rows[order[k + t]]);
-        w = (uint32_t)(rows + si.G - 1) * 32u * (uint32_t)((si.K + 3) / 4);   // one line set per wavefront step
+        w = (uint32_t)(rows + SDP_SCORE_SKEW * (si.G - 1)) * 32u * (uint32_t)((si.K + 3) / 4);   // one line set per wavefront step
     }
     words[k] = w;
 }
@@ -428,8 +428,8 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
         else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
         const int w = kk >> 2;
-        const uint32_t word = __ldg(region + ((size_t)(i - 1 + g) * NW + w) * 32u + lane0 + (uint32_t)g);   // step i + g
-        const uint32_t f = (word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u;
+        const uint32_t word = __ldg(region + ((size_t)(i - 1 + SDP_SCORE_SKEW * g) * NW + w) * 32u + lane0 + (uint32_t)g);   // step i + SKEW g
+        const uint32_t f = ((word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u) ^ 7u;   // low three bits are stored complemented
         if (st == 0) {
             if ((f & 3u) == 3u) {
                 emit(0, 1u); ++n_cols;
