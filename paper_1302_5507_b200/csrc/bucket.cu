@@ -110,14 +110,35 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
         slow_words[p] = slow;
     }
     if (err) atomicOr(err_flag, err);
-    // warp-aggregated histogram: one atomic per distinct key per warp
-    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
-    if (key != SDP_KEY_SKIP) {
-        const uint32_t peers = __match_any_sync(active, key);
-        if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
+    // histogram: the key of the block's first thread is counted per block (a uniform batch would otherwise serialise
+    // one atomic per warp on a single bin, see k_scatter), every other key per warp
+    {
+        __shared__ uint32_t s_key;
+        if (threadIdx.x == 0) s_key = key;
+        __syncthreads();
+        const uint32_t bkey = s_key;
+        const bool same = key == bkey && key != SDP_KEY_SKIP;
+        const int n_same = __syncthreads_count(same ? 1 : 0);
+        if (threadIdx.x == 0 && n_same) atomicAdd(hist + bkey, (uint32_t)n_same);
+        const bool other = !same && key != SDP_KEY_SKIP;
+        const uint32_t active = __ballot_sync(0xffffffffu, other);
+        if (other) {
+            const uint32_t peers = __match_any_sync(active, key);
+            if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
+        }
     }
-    for (int o = 16; o > 0; o >>= 1) my_cells += __shfl_down_sync(0xffffffffu, my_cells, o);
-    if ((threadIdx.x & 31) == 0 && my_cells) atomicAdd(cells, my_cells);
+    // cells: one atomic per block
+    {
+        __shared__ unsigned long long s_cells[8];
+        for (int o = 16; o > 0; o >>= 1) my_cells += __shfl_down_sync(0xffffffffu, my_cells, o);
+        if ((threadIdx.x & 31) == 0) s_cells[threadIdx.x >> 5] = my_cells;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long t = 0;
+            for (int k = 0; k < (int)(blockDim.x >> 5); ++k) t += s_cells[k];
+            if (t) atomicAdd(cells, t);
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -178,19 +199,46 @@ __global__ void __launch_bounds__(1024) k_scan_bins_finish(uint32_t* __restrict_
 
 // scatter pair indices into bucket order (order inside one bin is not deterministic; no result
 // depends on it because every pair is aligned independently and written back by caller index)
-__global__ void k_scatter(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ cursor,
-                          uint32_t* __restrict__ order)
+// A batch of one read length and one window length puts every pair into ONE bin: a warp-aggregated atomic per warp
+// then serialises on that bin's cursor (31,250 atomics on one address for a million pairs: 75 us). So the key of the
+// block's first thread is handled per BLOCK (one atomic for all threads that share it, positions from a ballot /
+// warp-count scan); every other key takes the warp-aggregated path.
+__global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ cursor,
+                                                 uint32_t* __restrict__ order)
 {
+    __shared__ uint32_t s_key, s_base, s_wcnt[8];
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t key = p < n ? keys[p] : SDP_KEY_SKIP;
-    const uint32_t active = __ballot_sync(0xffffffffu, key != SDP_KEY_SKIP);
-    if (key != SDP_KEY_SKIP) {
+    const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_key = key;
+    __syncthreads();
+    const uint32_t bkey = s_key;
+    const bool same = key == bkey && key != SDP_KEY_SKIP;
+    const uint32_t same_mask = __ballot_sync(0xffffffffu, same);
+    if (lane == 0) s_wcnt[w] = (uint32_t)__popc(same_mask);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t total = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) total += s_wcnt[k];
+        s_base = total ? atomicAdd(cursor + bkey, total) : 0u;
+    }
+    __syncthreads();
+    if (same) {
+        uint32_t pre = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) pre += (k < (int)w) ? s_wcnt[k] : 0u;
+        order[s_base + pre + (uint32_t)__popc(same_mask & ((1u << lane) - 1u))] = (uint32_t)p;
+    }
+    const bool other = !same && key != SDP_KEY_SKIP;
+    const uint32_t active = __ballot_sync(0xffffffffu, other);
+    if (other) {
         const uint32_t peers = __match_any_sync(active, key);
         const int leader = __ffs(peers) - 1;
         uint32_t base = 0;
-        if ((threadIdx.x & 31) == (uint32_t)leader) base = atomicAdd(cursor + key, (uint32_t)__popc(peers));
+        if (lane == (uint32_t)leader) base = atomicAdd(cursor + key, (uint32_t)__popc(peers));
         base = __shfl_sync(peers, base, leader);
-        order[base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u))] = (uint32_t)p;
+        order[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)p;
     }
 }
 

@@ -34,9 +34,21 @@ __device__ __forceinline__ int tb_class_of(int bw) {
 }
 static_assert((THIN_NW + TB_NCLASS) * TB_KEY_STRIDE <= SDP_NBINS && SDP_MAX_READ_LEN < TB_KEY_STRIDE, "thin keys must fit the bucket-sort key space");
 
+// Histogram add for every thread of the block (call from uniform control flow). The key of the block's first thread
+// is counted once per block -- half of a typical batch shares one key (the gapless class), and one atomic per warp
+// would serialise on that bin -- every other key once per warp.
 __device__ __forceinline__ void hist_add(uint32_t* hist, uint32_t key, bool valid) {
-    const uint32_t active = __ballot_sync(0xffffffffu, valid);
-    if (valid) {
+    __shared__ uint32_t s_key;
+    __syncthreads();
+    if (threadIdx.x == 0) s_key = valid ? key : SDP_KEY_SKIP;
+    __syncthreads();
+    const uint32_t bkey = s_key;
+    const bool same = valid && key == bkey;
+    const int n_same = __syncthreads_count(same ? 1 : 0);
+    if (threadIdx.x == 0 && n_same) atomicAdd(hist + bkey, (uint32_t)n_same);
+    const bool other = valid && !same;
+    const uint32_t active = __ballot_sync(0xffffffffu, other);
+    if (other) {
         const uint32_t peers = __match_any_sync(active, key);
         if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
     }
