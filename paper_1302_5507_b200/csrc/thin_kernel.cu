@@ -128,6 +128,7 @@ __device__ __forceinline__ void thin_gapless(const TraceParams& tp, const uint32
 // The nibbles sit in local memory (an L2 round trip per dependent load), so each walk fetches the words of EIGHT rows
 // at once -- the rows above the current cell in the same band-slot word, which is where a diagonal step, the common
 // one, stays -- and the two walks' loads are in flight together.
+constexpr int WALK_ROWS = 8;      // (16: measured no faster)
 __device__ __noinline__ void thin_walks(const TraceParams& tp, const ThinConsts& tc, const ThinPair& A, const ThinPair& B,
                                         const bool writeB, const uint32_t* lbits, const int W, const uint32_t finH)
 {
@@ -137,7 +138,7 @@ __device__ __noinline__ void thin_walks(const TraceParams& tp, const ThinConsts&
         int i, j, st, n_cols, gap_runs, gap_bases, cur_op, c_row, c_wc;
         uint32_t cur_len, nops;
         bool bad, live;
-        uint32_t c[8];
+        uint32_t c[WALK_ROWS];
         uint32_t* ops;
     };
     const uint32_t cap = 2u * (uint32_t)W + 3u;
@@ -154,7 +155,7 @@ __device__ __noinline__ void thin_walks(const TraceParams& tp, const ThinConsts&
         const int f = (int)((finH >> (16 * lane)) & 0xFFFFu) >> 3;
         x.bad = (f - tc.beta - tc.e * (R + n) != tp.score[T.p]);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) x.c[k] = 0u;
+        for (int k = 0; k < WALK_ROWS; ++k) x.c[k] = 0u;
     }
     auto emit = [&](Walk& x, int op, uint32_t len) {
         if (op == x.cur_op) { x.cur_len += len; return; }
@@ -175,10 +176,10 @@ __device__ __noinline__ void thin_walks(const TraceParams& tp, const ThinConsts&
             const int jj = x.j - (x.i - off - W);
             if (jj < 0 || jj >= BW) { x.bad = true; x.live = false; continue; }
             const int wc = jj >> 2, d = x.c_row - (x.i - 1);
-            if (wc != x.c_wc || d < 0 || d >= 8) {
+            if (wc != x.c_wc || d < 0 || d >= WALK_ROWS) {
                 x.c_row = x.i - 1; x.c_wc = wc;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
+                for (int k = 0; k < WALK_ROWS; ++k) {
                     const int r = x.i - 1 - k;
                     x.c[k] = r >= 0 ? lbits[r * WPR + wc] : 0u;
                 }
@@ -192,7 +193,7 @@ __device__ __noinline__ void thin_walks(const TraceParams& tp, const ThinConsts&
             const int d = x.c_row - (x.i - 1);
             uint32_t word = x.c[0];
 #pragma unroll
-            for (int k = 1; k < 8; ++k) word = (d == k) ? x.c[k] : word;
+            for (int k = 1; k < WALK_ROWS; ++k) word = (d == k) ? x.c[k] : word;
             const uint32_t f = ((word >> (16u * (uint32_t)lane + 4u * (uint32_t)(3 - (jj & 3)))) & 15u) ^ 7u;
             if (x.st == 0) {
                 if ((f & 3u) == 3u) {

@@ -26,10 +26,11 @@
 // its packing run on the FMA pipe: two integer subtractions, then fp16 FMAs on the small integers as DENORMALS
 // (t = eb*8 + x, byte = t0*16 + t1: exact below 2048), and one PRMT per four cells joins two bytes. Nibbles are
 // left-aligned, four cells per 16-bit lane (cell kk of a word in bits 4*(3 - kk)), and stored step by step:
-//     word((i, w, lane)) = task region + ((s-1) * ceil(K/4) + w) * 32 + lane,   low half = first pair of the two,
+//     word((i, w, lane)) = task region + (((s-1)/2 * ceil(K/4) + w) * 32 + lane) * 2 + (s-1)%2,   low half = first pair,
 // where s = i + SDP_SCORE_SKEW*g is the STEP at which thread g of its group works on row i: the threads of a warp are
 // on different rows at any one time (anti-diagonal wavefront), so only a step-major layout makes a warp-wide
-// store one 128-byte line. One region of (rows + SKEW*(G - 1)) steps per warp task.
+// store whole 128-byte lines; the two steps of one pass sit side by side, so a pass stores 8 bytes per thread and the
+// walk gets two steps per 32-byte sector. One region of (rows + SKEW*(G - 1)) steps, rounded up to pairs, per warp task.
 #pragma once
 #include "score_kernel.cuh"
 
@@ -134,8 +135,11 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
     const uint16_t* const rp0 = reinterpret_cast<const uint16_t*>(ring_w) + rg.mirror - SKEW * g;
 
     const bool st_ok = hasA;                              // hasB implies hasA
-    constexpr uint32_t rowstride = 32u * NW;              // word (step, w, lane): a warp-wide store is one 128-byte line
-    uint32_t* wp = T.bits + T.bits_off[first] + (uint32_t)lane;
+    // word (step pair, w, lane, step parity): the two rows of one pass go out as ONE 8-byte store per thread (a warp-wide
+    // store is two full lines), and the walk finds two consecutive steps of a column group in one 32-byte sector
+    constexpr uint32_t pairstride = 64u * NW;
+    uint32_t* const wbase = T.bits + T.bits_off[first] + 2u * (uint32_t)lane;
+    int tstep = 0;                                        // steps done by this warp (0-based step of the next row)
 
     constexpr uint32_t negOf = SDP_SENT_T_NEGOF, negOe = SDP_SENT_T_NEGOE, c8 = SDP_SENT_T_C8, Cd8 = SDP_SENT_T_CD8;
     constexpr uint32_t H2_8 = 0x48004800u;                // fp16 8.0, both lanes
@@ -172,7 +176,7 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
         if (SLOW && i < 1) {
 #pragma unroll
             for (int k = 0; k < K; ++k) Hn[k] = Hs[k];
-            wp += rowstride;                              // wp follows the STEP, not the row (see the layout above)
+            ++tstep;                                      // the layout follows the STEP, not the row (see above)
             return;
         }
         fv = __vadd2(fv, fstep);
@@ -187,16 +191,17 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
         uint32_t hd = hdiag;
         hdiag = hin;
         NibblePack np; np.reset();
+        uint32_t* const wp = wbase + (uint32_t)(tstep >> 1) * pairstride + (uint32_t)(tstep & 1);
+        ++tstep;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const uint32_t t = cell(hd, Hs[k], F[k], nt, rh[k], Hl, E);
             hd = Hs[k];
             Hn[k] = Hl;
             uint32_t word;
-            if (np.template add<K>(k, t, word)) { if (do_store) wp[(k >> 2) * 32] = word; }
+            if (np.template add<K>(k, t, word)) { if (do_store) wp[(k >> 2) * 64] = word; }
             if (PAD && k == K - 2) { Hsk = Hl; Esk = E; }
         }
-        wp += rowstride;
         if (PAD) { hout = blend(skipmask, Hsk, Hl); eout = blend(skipmask, Esk, E); }
         else     { hout = Hl; eout = E; }
         if (is_last) {
@@ -219,7 +224,9 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
         einB = imad_sel(einB, notfirst, 0u);
         const uint32_t ntA = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[0]);
         const uint32_t ntB = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, (uint32_t)rp[1]);
-        const bool storeA = st_ok && ia <= Rpp, storeB = st_ok && ia + 1 <= Rpp;
+        const bool storeA = st_ok && ia <= Rpp;           // (the region has room for the pass's second row past Rpp)
+        uint2* const wp2 = reinterpret_cast<uint2*>(wbase + (uint32_t)(tstep >> 1) * pairstride);   // tstep is even here
+        tstep += 2;
 
         uint32_t HlA = hinA, EA = einA, HlB = hinB, EB = einB;
         uint32_t hdA = hdiag, hdB = hinA;                 // H7(ia-1, left), H7(ia, left)
@@ -227,15 +234,17 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
         uint32_t HskA = hinA, EskA = einA, HskB = hinB, EskB = einB;
         uint32_t prevA = hinA;                            // H7(ia, k-1)
         NibblePack npA, npB; npA.reset(); npB.reset();
+        uint32_t pendA = 0u;                              // the first row's word, until the second row's word of the same cells
 #pragma unroll
         for (int k = 0; k <= K; ++k) {
             const uint32_t upB = prevA;                   // H7(ia, k-1): the second row's "row above" at column k-1
+            const uint32_t pendB = pendA;                 // (the first row may finish its LAST word in this very iteration)
             if (k < K) {                                  // first row, column k
                 const uint32_t t = cell(hdA, H[k], F[k], ntA, rh[k], HlA, EA);
                 hdA = H[k];
                 prevA = HlA;
                 uint32_t word;
-                if (npA.template add<K>(k, t, word)) { if (storeA) wp[(k >> 2) * 32] = word; }
+                if (npA.template add<K>(k, t, word)) pendA = word;
                 if (PAD && k == K - 2) { HskA = HlA; EskA = EA; }
             }
             if (k >= 1) {                                 // second row, column k-1
@@ -243,11 +252,10 @@ __device__ __forceinline__ void trace_body(const ScoreParams& P, const TraceDP& 
                 hdB = upB;
                 H[k - 1] = HlB;
                 uint32_t word;
-                if (npB.template add<K>(k - 1, t, word)) { if (storeB) wp[rowstride + ((k - 1) >> 2) * 32] = word; }
+                if (npB.template add<K>(k - 1, t, word)) { if (storeA) wp2[((k - 1) >> 2) * 32] = make_uint2(pendB, word); }
                 if (PAD && k - 1 == K - 2) { HskB = HlB; EskB = EB; }
             }
         }
-        wp += 2 * rowstride;
         if (PAD) {
             houtA = blend(skipmask, HskA, HlA); eoutA = blend(skipmask, EskA, EA);
             houtB = blend(skipmask, HskB, HlB); eoutB = blend(skipmask, EskB, EB);

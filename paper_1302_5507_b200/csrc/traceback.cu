@@ -356,7 +356,8 @@ __global__ void k_wide_regions(const uint32_t* __restrict__ order, uint32_t max_
     if (local % ppw == 0) {                               // first pair of a task owns the task's region
         int rows = 0;
         for (uint32_t t = 0; t < ppw && local + t < si.count; ++t) rows = max(rows, tb_rows[order[k + t]]);
-        w = (uint32_t)(rows + SDP_SCORE_SKEW * (si.G - 1)) * 32u * (uint32_t)((si.K + 3) / 4);   // one line set per wavefront step
+        // one line set per wavefront step, steps in pairs (+ one pair: a pass may store its second row past the last)
+        w = (uint32_t)((rows + SDP_SCORE_SKEW * (si.G - 1) + 3) / 2) * 64u * (uint32_t)((si.K + 3) / 4);
     }
     words[k] = w;
 }
@@ -440,7 +441,8 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams wp)
         if (j0 < split) { g = j0 / (K - 1); kk = j0 - g * (K - 1); }
         else { const int j1 = j0 - split; const int t = j1 / K; g = pad + t; kk = j1 - t * K; }
         const int w = kk >> 2;
-        const uint32_t word = __ldg(region + ((size_t)(i - 1 + SDP_SCORE_SKEW * g) * NW + w) * 32u + lane0 + (uint32_t)g);   // step i + SKEW g
+        const int t = i - 1 + SDP_SCORE_SKEW * g;          // 0-based step of row i in thread g (trace_kernel.cuh layout)
+        const uint32_t word = __ldg(region + (((size_t)(t >> 1) * NW + w) * 32u + lane0 + (uint32_t)g) * 2u + (uint32_t)(t & 1));
         const uint32_t f = ((word >> (lane_shift + 4u * (uint32_t)(3 - (kk & 3)))) & 15u) ^ 7u;   // low three bits are stored complemented
         if (st == 0) {
             if ((f & 3u) == 3u) {
