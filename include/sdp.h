@@ -135,10 +135,13 @@ int sdp_create(const sdp_scoring* scoring, int cuda_device, sdp_ctx** out);
  * traceback kernel and requires identical output). flags = OR of the SDP_ROUTE_* bits and SDP_ROUTE_FORCE_G(g):
  *   SDP_ROUTE_NO_THIN      pairs with gap bound W >= 1 go to the wide / generic traceback instead of the narrow-band kernels
  *   SDP_ROUTE_NO_WIDE      wide pairs go to the generic scalar band kernel instead of the wavefront traceback kernel
+ *   SDP_ROUTE_ALWAYS_REVERSE  every wide pair takes the reverse pass (by default only those whose row bound exceeds about
+ *                          twice the read length, where trimming the traceback rectangle pays for the pass)
  *   SDP_ROUTE_FORCE_G(g)   g threads per pair group for every read length that admits it (geometry experiments), 0 = off
  * 0 restores the default routing. SDP_EINVAL for unknown bits. */
 #define SDP_ROUTE_NO_THIN 1u
 #define SDP_ROUTE_NO_WIDE 2u
+#define SDP_ROUTE_ALWAYS_REVERSE 4u
 #define SDP_ROUTE_FORCE_G(g) (((uint32_t)(g) & 0x3Fu) << 8)
 int sdp_set_debug_route(sdp_ctx* ctx, uint32_t flags);
 

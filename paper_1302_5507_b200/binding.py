@@ -20,7 +20,7 @@ SDP_OK, SDP_EINVAL, SDP_ERANGE, SDP_ECUDA, SDP_ENOMEM = 0, -1, -2, -3, -4
 SDP_MAX_READ_LEN = 1024
 SDP_MAX_SEQ_LEN = 1000000
 SDP_MAX_CELL_VALUE = 32000
-SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE = 1, 2
+SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE, SDP_ROUTE_ALWAYS_REVERSE = 1, 2, 4
 
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
@@ -254,9 +254,10 @@ class Context:
     def set_prefilter(self, enabled: bool):
         self._lib.sdp_set_prefilter(self._h, int(bool(enabled)))
 
-    def set_debug_route(self, no_thin: bool = False, no_wide: bool = False, force_g: int = 0):
+    def set_debug_route(self, no_thin: bool = False, no_wide: bool = False, force_g: int = 0, always_reverse: bool = False):
         """sdp_set_debug_route: route pairs through the other traceback kernels / force a thread-group size (tests)."""
-        flags = (SDP_ROUTE_NO_THIN if no_thin else 0) | (SDP_ROUTE_NO_WIDE if no_wide else 0) | ((int(force_g) & 0x3F) << 8)
+        flags = ((SDP_ROUTE_NO_THIN if no_thin else 0) | (SDP_ROUTE_NO_WIDE if no_wide else 0) |
+                 (SDP_ROUTE_ALWAYS_REVERSE if always_reverse else 0) | ((int(force_g) & 0x3F) << 8))
         self._check(self._lib.sdp_set_debug_route(self._h, flags))
 
     def set_mode(self, local: bool):

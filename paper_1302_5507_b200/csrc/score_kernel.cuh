@@ -303,8 +303,11 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
 
     const int nA = (int)dA.n, nB = (int)dB.n;
     const int mA = (int)dA.m, mB = (int)dB.m;
-    const int Mmin = __reduce_min_sync(0xffffffffu, min(mA, mB));
+    // (reverse pass: a descriptor with m == 0 is a pair whose rectangle the reverse pass would not pay for; it keeps
+    // its place in the task but takes no part: not in the row bounds, no output, no check)
+    const int Mmin = __reduce_min_sync(0xffffffffu, REV ? min(mA > 0 ? mA : 0x7fffffff, mB > 0 ? mB : 0x7fffffff) : min(mA, mB));
     const int Mmax = __reduce_max_sync(0xffffffffu, max(mA, mB));
+    if (REV && Mmax == 0) return;                         // warp-uniform: nothing to do for this task
 
     // ---- columns of this thread: the first pad = G*K - n threads skip their last column
     const int padA = PAD ? G * K - nA : 0, padB = PAD ? G * K - nB : 0;
@@ -548,7 +551,8 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
                                                              (nB - jB + 1) * M - e * (jB - 1) + e * SKEW * g), acc);
             }
             const int tA = dA.aux + P.c.beta + e * send, tB = dB.aux + P.c.beta + e * send;
-            const bool alive = (hasA && (int)(int16_t)(acc & 0xFFFFu) >= tA) || (hasB && (int)(int16_t)(acc >> 16) >= tB);
+            const bool alive = (hasA && mA > 0 && (int)(int16_t)(acc & 0xFFFFu) >= tA) ||
+                               (hasB && mB > 0 && (int)(int16_t)(acc >> 16) >= tB);
             if (!__any_sync(0xffffffffu, alive)) break;
         }
     }
@@ -561,8 +565,8 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
         if (REV) {
             // idx = rows of the reversed window consumed by the longest alignment scoring S;
             // the lowest co-optimal start is s_lo = ref_end + 1 - idx
-            if (hasA) { P.rev_rows[dA.pid] = idxA; if (sA != dA.aux) atomicOr(P.err_flag, SDP_ERRF_REVERSE); }
-            if (hasB) { P.rev_rows[dB.pid] = idxB; if (sB != dB.aux) atomicOr(P.err_flag, SDP_ERRF_REVERSE); }
+            if (hasA && mA > 0) { P.rev_rows[dA.pid] = idxA; if (sA != dA.aux) atomicOr(P.err_flag, SDP_ERRF_REVERSE); }
+            if (hasB && mB > 0) { P.rev_rows[dB.pid] = idxB; if (sB != dB.aux) atomicOr(P.err_flag, SDP_ERRF_REVERSE); }
         } else {
             if (hasA) { P.score[dA.pid] = sA; P.ref_end[dA.pid] = idxA - 1; }
             if (hasB) { P.score[dB.pid] = sB; P.ref_end[dB.pid] = idxB - 1; }

@@ -89,6 +89,8 @@ struct sdp_ctx {
     int wide_fits = 0;               // wide_ok before sdp_set_debug_route masked it
     int no_thin = 0;                 // sdp_set_debug_route: keep W >= 1 pairs off the narrow-band kernel
     int thin_ok = 0;                 // scoring fits the x8 tagged int16 domain of thin_kernel.cu
+    int force_rev = 0;               // sdp_set_debug_route: the reverse pass for every wide pair, not only where it pays
+    uint32_t resident_warps = 1776;  // SMs x warps of the score kernels resident per SM (12 at 168 registers)
     char err[512] = {0};
     bool timing = false;
     bool prefilter = false;          // sdp_set_prefilter: ungapped pre-pass before the forward DP
@@ -353,6 +355,11 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaEventCreate(&ctx->ev_start));
         CU(cudaEventCreate(&ctx->ev_end));
         for (int k = 0; k < SDP_MAX_LANES; ++k) CU(cudaEventCreateWithFlags(&ctx->ev_cig[k], cudaEventDisableTiming));
+        {
+            int sms = 148;
+            CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device));
+            ctx->resident_warps = (uint32_t)sms * 12u;
+        }
         CU(cudaMalloc(&ctx->cig_total, (SDP_MAX_LANES + 1) * 8));
         CU(cudaMemset(ctx->cig_total, 0, (SDP_MAX_LANES + 1) * 8));
         return lanes_init(ctx, 1);
@@ -404,8 +411,10 @@ int sdp_set_debug_route(sdp_ctx* ctx, uint32_t flags)
     if (!ctx) return SDP_EINVAL;
     ctx->err[0] = 0;
     const int force_g = (int)((flags >> 8) & 0x3Fu);
-    if ((flags & ~(SDP_ROUTE_NO_THIN | SDP_ROUTE_NO_WIDE | 0x3F00u)) || force_g > 32) return fail(ctx, SDP_EINVAL, "unknown route flags");
+    if ((flags & ~(SDP_ROUTE_NO_THIN | SDP_ROUTE_NO_WIDE | SDP_ROUTE_ALWAYS_REVERSE | 0x3F00u)) || force_g > 32)
+        return fail(ctx, SDP_EINVAL, "unknown route flags");
     ctx->no_thin = (flags & SDP_ROUTE_NO_THIN) ? 1 : 0;
+    ctx->force_rev = (flags & SDP_ROUTE_ALWAYS_REVERSE) ? 1 : 0;
     ctx->wide_ok = (flags & SDP_ROUTE_NO_WIDE) ? 0 : ctx->wide_fits;
     choose_geometry(ctx, force_g);
     CU(cudaSetDevice(ctx->device));
@@ -622,6 +631,7 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     pp.keys_wide = L.keys_wide.as<uint32_t>();
     pp.wide_ok = ctx->wide_ok; pp.no_thin = ctx->no_thin; pp.thin_ok = ctx->thin_ok;
     pp.local = local; pp.slow_words = L.slow_words.as<uint32_t>(); pp.end_col = L.rev_rows.as<int32_t>();
+
     pp.err_flag = L.err_flag;
     pp.bits_words = L.bits_words.as<uint32_t>(); pp.ops_cap = L.ops_cap.as<uint32_t>();
     pp.hist_tb = L.hist[2]; pp.hist_wide = L.hist[3]; pp.counters = L.counters;
@@ -678,8 +688,12 @@ int lane_phase_c(sdp_ctx* ctx, Lane& L, const int local)
     int32_t* ref_end = ctx->ref_end.as<int32_t>() + L.p0;
 
     // ---- a4 reverse pass over the wide pairs (same buckets and task table as their traceback DP)
-    launch_fill_desc_rev(b, L.order_wide.as<uint32_t>(), n_wide, score, ref_end, L.tbW.as<int32_t>(),
-                         L.desc_rev.as<PairDesc>(), st);
+    // a4 where it pays (k_fill_desc_rev): with fewer wide-pair tasks than four waves of resident warps the kernels'
+    // time follows the longest task, not the total work, and every wide pair takes the pass
+    const uint32_t wide_tasks = L.mb->task_prefix[2][SDP_NSLOTS];
+    const int ratio10 = (ctx->force_rev || wide_tasks < 4u * ctx->resident_warps) ? 0 : 24;
+    launch_fill_desc_rev(b, L.order_wide.as<uint32_t>(), n_wide, score, ref_end, L.tbW.as<int32_t>(), ratio10,
+                         L.rev_rows.as<int32_t>(), L.counters, L.desc_rev.as<PairDesc>(), st);
     ++L.nl;
     {
         int rc = launch_score_stage(ctx, L, 1, L.desc_rev.as<PairDesc>(), st, ctx->fan_post, &L.nl);
@@ -753,6 +767,7 @@ int lane_phase_d(sdp_ctx* ctx, Lane& L, const int li)
     ++L.nl;
     CU(cudaMemcpyAsync(&L.mb->totals[2], ctx->cig_total + li + 1, 8, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(&L.mb->err_flag, L.err_flag, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(L.mb->counters, L.counters, 3 * 8, cudaMemcpyDeviceToHost, st));   // reverse counters: k_fill_desc_rev
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_END], st));
     CU(cudaEventRecord(L.evD, st));
     return SDP_OK;

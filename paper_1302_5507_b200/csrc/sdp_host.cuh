@@ -72,8 +72,10 @@ struct PostParams {
     unsigned long long* counters;   // [0] reverse cells, [1] traceback cells, [2] reverse pairs
 };
 void launch_post_forward(const PostParams& pp, cudaStream_t st);
+// ratio10: the pair takes the reverse pass when its row bound exceeds ratio10 / 10 read lengths (0 = always)
 void launch_fill_desc_rev(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
-                          const int32_t* ref_end, const int32_t* tbW, PairDesc* desc, cudaStream_t st);
+                          const int32_t* ref_end, const int32_t* tbW, int ratio10, int32_t* rev_rows,
+                          unsigned long long* counters, PairDesc* desc, cudaStream_t st);
 
 struct TraceParams {
     sdp_batch b;

@@ -59,7 +59,7 @@ __global__ void k_post_forward(const PostParams pp)
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = p < pp.n_pairs;
     uint32_t ktb = SDP_KEY_SKIP, kwide = SDP_KEY_SKIP;
-    unsigned long long c_rev = 0, c_tb = 0, n_rev = 0;
+    unsigned long long c_tb = 0;
     bool too_big = false;
     if (valid) {
         // slow = the int32 lane (slow_lane.cu): pairs outside the int16 kernels' domain, and every pair in local mode,
@@ -110,7 +110,7 @@ __global__ void k_post_forward(const PostParams pp)
             // so that the pairs of one warp walk nearly the same number of rows
             const uint32_t rbin = (uint32_t)min(63, (rows * 64) / (5 * n / 2 + 1));
             kwide = (uint32_t)(n - 1) * 64u + rbin;         // the reverse pass and the traceback DP share this order
-            c_rev = (unsigned long long)n * rows; c_tb = c_rev; n_rev = 1;
+            c_tb = (unsigned long long)n * rows;            // (whether the pair takes the reverse pass: k_fill_desc_rev)
         } else {
             const int cls = slow ? TB_NCLASS - 1 : tb_class_of(bw);
             const unsigned long long w64 = (unsigned long long)rows * (unsigned long long)((bw + 7) / 8) +
@@ -127,14 +127,8 @@ __global__ void k_post_forward(const PostParams pp)
     }
     hist_add(pp.hist_tb, ktb, ktb != SDP_KEY_SKIP);
     hist_add(pp.hist_wide, kwide, kwide != SDP_KEY_SKIP);
-    for (int o = 16; o > 0; o >>= 1) {
-        c_rev += __shfl_down_sync(0xffffffffu, c_rev, o);
-        c_tb += __shfl_down_sync(0xffffffffu, c_tb, o);
-        n_rev += __shfl_down_sync(0xffffffffu, n_rev, o);
-    }
-    if ((threadIdx.x & 31) == 0 && (c_tb | n_rev)) {
-        atomicAdd(pp.counters + 0, c_rev); atomicAdd(pp.counters + 1, c_tb); atomicAdd(pp.counters + 2, n_rev);
-    }
+    for (int o = 16; o > 0; o >>= 1) c_tb += __shfl_down_sync(0xffffffffu, c_tb, o);
+    if ((threadIdx.x & 31) == 0 && c_tb) atomicAdd(pp.counters + 1, c_tb);
 }
 
 void launch_post_forward(const PostParams& pp, cudaStream_t st)
@@ -143,28 +137,48 @@ void launch_post_forward(const PostParams& pp, cudaStream_t st)
 }
 
 // descriptors of the reverse pass, in its bucket order: DP row 1 is window base ref_end, the
-// read is walked from its last base, rows = min(ref_end + 1, n + W)
+// read is walked from its last base, rows = min(ref_end + 1, n + W).
+// a4 WHERE IT PAYS. The pass costs `rows` score-kernel rows and trims the traceback rectangle from `rows` to the
+// alignment's span (about n) rows, each worth ~2.2 score-kernel rows (measured on config 4: DESIGN.md "Traceback").
+// With enough wide pairs to fill the GPU many times over, that is worth it only when the bound exceeds ratio10/10
+// read lengths (2.4 by measurement); such a pair gets m = 0 here (the kernel skips it) and rev_rows = rows, i.e. its
+// rectangle is the whole bound. With few wide pairs the kernels' time is set by the longest task, not by the total
+// work, and the host passes ratio10 = 0: every wide pair takes the pass.
 __global__ void k_fill_desc_rev(const sdp_batch b, const uint32_t* __restrict__ order, uint32_t count,
                                 const int32_t* __restrict__ score, const int32_t* __restrict__ ref_end,
-                                const int32_t* __restrict__ tbW, PairDesc* __restrict__ desc)
+                                const int32_t* __restrict__ tbW, int ratio10, int32_t* __restrict__ rev_rows,
+                                unsigned long long* __restrict__ counters, PairDesc* __restrict__ desc)
 {
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= count) return;
-    const uint32_t p = order[k];
-    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
-    PairDesc d;
-    d.n = b.read_len[ri];
-    d.roff = b.read_off[ri];
-    d.woff = b.win_off[wi] + (uint64_t)ref_end[p];
-    d.m = (uint32_t)min(ref_end[p] + 1, (int)d.n + tbW[p]);
-    d.pid = p; d.aux = score[p];
-    desc[k] = d;
+    unsigned long long c_rev = 0, n_rev = 0;
+    if (k < count) {
+        const uint32_t p = order[k];
+        const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
+        PairDesc d;
+        d.n = b.read_len[ri];
+        d.roff = b.read_off[ri];
+        d.woff = b.win_off[wi] + (uint64_t)ref_end[p];
+        const int rows = min(ref_end[p] + 1, (int)d.n + tbW[p]);
+        const bool use_rev = 10 * rows > ratio10 * (int)d.n + 80 || ratio10 == 0;
+        d.m = use_rev ? (uint32_t)rows : 0u;
+        rev_rows[p] = use_rev ? 0 : rows;                   // (the kernel overwrites the 0)
+        d.pid = p; d.aux = score[p];
+        desc[k] = d;
+        if (use_rev) { c_rev = (unsigned long long)d.n * rows; n_rev = 1; }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        c_rev += __shfl_down_sync(0xffffffffu, c_rev, o);
+        n_rev += __shfl_down_sync(0xffffffffu, n_rev, o);
+    }
+    if ((threadIdx.x & 31) == 0 && n_rev) { atomicAdd(counters + 0, c_rev); atomicAdd(counters + 2, n_rev); }
 }
 
 void launch_fill_desc_rev(const sdp_batch& b, const uint32_t* order, uint32_t count, const int32_t* score,
-                          const int32_t* ref_end, const int32_t* tbW, PairDesc* desc, cudaStream_t st)
+                          const int32_t* ref_end, const int32_t* tbW, int ratio10, int32_t* rev_rows,
+                          unsigned long long* counters, PairDesc* desc, cudaStream_t st)
 {
-    if (count) k_fill_desc_rev<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, score, ref_end, tbW, desc);
+    if (count) k_fill_desc_rev<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, score, ref_end, tbW, ratio10, rev_rows,
+                                                                    counters, desc);
 }
 
 // ---------------------------------------------------------------------------------------------

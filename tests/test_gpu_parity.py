@@ -273,16 +273,20 @@ def test_other_scorings(sc):
         c.destroy()
 
 
-@pytest.mark.parametrize("route", [dict(no_thin=True), dict(no_wide=True), dict(no_thin=True, no_wide=True)],
-                         ids=["no_thin", "no_wide", "generic_only"])
+@pytest.mark.parametrize("route", [dict(no_thin=True), dict(no_wide=True), dict(no_thin=True, no_wide=True),
+                                   dict(always_reverse=True), dict(no_thin=True, always_reverse=True)],
+                         ids=["no_thin", "no_wide", "generic_only", "always_reverse", "no_thin_always_reverse"])
 def test_alternative_traceback_paths(route):
     # route the same pairs through the other traceback kernels (wide wavefront for every W >= 1; generic scalar band
-    # kernel instead of the wavefront; generic kernel for everything): all must agree with the oracle
+    # kernel instead of the wavefront; generic kernel for everything; the reverse pass for every wide pair instead of
+    # only where it pays): all must agree with the oracle
     c = make_ctx(DEFAULT)
     try:
         c.set_debug_route(**route)
         parity.check_batch(c, W.make_config(3, n_pairs=1200, ref_bases=500_000), DEFAULT, f"cfg3 {route}", host_path=False)
         parity.check_batch(c, W.make_config(5, n_pairs=1500, ref_bases=500_000), DEFAULT, f"cfg5 {route}", host_path=False)
+        parity.check_batch(c, W.make_config(4, n_pairs=600, ref_bases=500_000), DEFAULT, f"cfg4 {route}", host_path=False)
+        parity.check_batch(c, W.make_config(2, n_pairs=2000, ref_bases=500_000), DEFAULT, f"cfg2 {route}", host_path=False)
         c.set_debug_route()                                   # back to the default routing
         parity.check_batch(c, W.make_config(5, n_pairs=700, ref_bases=500_000), DEFAULT, "cfg5 default route", host_path=False)
     finally:
