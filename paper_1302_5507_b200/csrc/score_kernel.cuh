@@ -520,7 +520,7 @@ __device__ __forceinline__ void score_body(const ScoreParams& P, uint32_t (*ring
         for (; s <= fe; ++s, ++rp) row_step1(s - SKEW * g, rp, std::false_type{});
 #pragma unroll 1
         for (; s <= send; ++s, ++rp) row_step1(s - SKEW * g, rp, std::true_type{});
-        rows_done = send - lead;
+        if (REV) rows_done = send - lead;
         if (REV && can_exit && send < all_end) {
             // Early exit of the reverse pass. The pass looks for the LAST row whose M(i,n) equals the forward score S
             // (dA.aux), so it may stop as soon as no later row can reach S. Any path to a later cell of column n leaves
