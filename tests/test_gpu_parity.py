@@ -273,6 +273,28 @@ def test_other_scorings(sc):
         c.destroy()
 
 
+@pytest.mark.parametrize("sc", [OracleScoring(20, -60, 100, 40, 0.6), OracleScoring(1, -3, 5, 400, 0.6),
+                                OracleScoring(1, -3, 2000, 2, 0.6), OracleScoring(1, -4000, 5, 2, 0.6),
+                                OracleScoring(250, -3, 5, 375, 0.6), OracleScoring(4000, -4000, 4000, 4000, 0.6),
+                                OracleScoring(200, -39, 3, 1, 0.6), OracleScoring(240, 0, 7, 3, 0.6)],
+                         ids=lambda s: f"{s.match}_{s.mismatch}_{s.gap_open}_{s.gap_extend}")
+def test_scorings_at_the_accepted_extremes(sc):
+    # large constants: the int16 range rule, the fp16 bit-pattern tricks (match - mismatch up to 8000, 8 times
+    # that in the tagged traceback kernels) and the patched immediates near their limits; pairs that leave the int16
+    # domain must take the int32 lane and the generic band kernel, never a wrong fast path
+    c = make_ctx(sc)
+    try:
+        for cfg, n_pairs in ((2, 400), (4, 200), (5, 400)):
+            parity.check_batch(c, W.make_config(cfg, n_pairs=n_pairs, ref_bases=300_000), sc, f"cfg{cfg} scoring {sc}",
+                               host_path=False)
+        rng = random.Random(16)
+        wins = ["".join(rng.choice("ACGT") for _ in range(rng.randint(1, 80))) for _ in range(200)]
+        reads = ["".join(rng.choice("ACGT") for _ in range(rng.randint(1, 40))) for _ in range(200)]
+        parity.check_batch(c, W.batch_from_strings(wins, reads), sc, f"scoring {sc} short", host_path=False)
+    finally:
+        c.destroy()
+
+
 @pytest.mark.parametrize("route", [dict(no_thin=True), dict(no_wide=True), dict(no_thin=True, no_wide=True),
                                    dict(always_reverse=True), dict(no_thin=True, always_reverse=True)],
                          ids=["no_thin", "no_wide", "generic_only", "always_reverse", "no_thin_always_reverse"])
