@@ -198,7 +198,8 @@ int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* re
  * CIGAR as soft clips (BAM op 4), n_cols counts aligned columns only, and the filter counts clipped bases as columns
  * that do not match: pass iff n_cols > 0 and n_match * 1e6 >= q * (n_cols + clipped). A pair without any positive-
  * scoring alignment reports score 0, ref_start 0, ref_end -1, read_start 0, read_end -1, CIGAR <n>S, pass 0.
- * In this release local mode runs on the int32 lane (exact, not tuned). SDP_EINVAL for an unknown mode.
+ * Local mode runs on the int32 lane (exact; one warp per pair, about one fifteenth of the default mode's throughput).
+ * SDP_EINVAL for an unknown mode.
  */
 #define SDP_MODE_SEMIGLOBAL 0
 #define SDP_MODE_LOCAL 1
