@@ -112,7 +112,10 @@ __global__ void k_post_forward(const PostParams pp)
             kwide = (uint32_t)(n - 1) * 64u + rbin;         // the reverse pass and the traceback DP share this order
             c_tb = (unsigned long long)n * rows;            // (whether the pair takes the reverse pass: k_fill_desc_rev)
         } else {
-            const int cls = slow ? TB_NCLASS - 1 : tb_class_of(bw);
+            // int32-lane pairs keep their row arrays in global scratch (any width); in local mode a read of up to 1,024
+            // bases has a band of at most 1,025 cells, which fits the local-memory classes
+            const bool any_width = slow && !(pp.local && pp.pn[p] <= 1024u);
+            const int cls = any_width ? TB_NCLASS - 1 : tb_class_of(bw);
             const unsigned long long w64 = (unsigned long long)rows * (unsigned long long)((bw + 7) / 8) +
                                            (cls == TB_NCLASS - 1 ? 2ull * (unsigned long long)(bw + 2) : 0ull);   // + the two row arrays
             if (w64 > 0xFFFFFFFFull) { words = 0; too_big = true; } else words = (uint32_t)w64;
@@ -220,7 +223,7 @@ __global__ void __launch_bounds__(128) k_traceback(const TraceParams tp)
 
     if (LOCAL && tp.score[p] == 0) {
         emit(4, (uint32_t)n_full);                        // no alignment: everything is clipped
-    } else if (W == 0 && MAXBW != 0) {
+    } else if (W == 0 && MAXBW != 0 && !LOCAL) {
         // gapless: the only co-optimal alignments are ungapped, so the CIGAR is nM
         ref_start = i_end - n;
         if (ref_start < 0) { bad = true; ref_start = 0; }
@@ -342,7 +345,16 @@ void launch_traceback(int cls, bool local, const TraceParams& tp, cudaStream_t s
 {
     if (tp.count == 0) return;
     const uint32_t grid = (tp.count + 127) / 128;
-    if (local) { k_traceback<0, true><<<grid, 128, 0, st>>>(tp); return; }
+    if (local) {
+        switch (cls) {
+            case 0: k_traceback<16, true><<<grid, 128, 0, st>>>(tp); break;
+            case 1: k_traceback<64, true><<<grid, 128, 0, st>>>(tp); break;
+            case 2: k_traceback<256, true><<<grid, 128, 0, st>>>(tp); break;
+            case 3: k_traceback<1032, true><<<grid, 128, 0, st>>>(tp); break;
+            default: k_traceback<0, true><<<grid, 128, 0, st>>>(tp); break;
+        }
+        return;
+    }
     switch (cls) {
         case 0: k_traceback<16, false><<<grid, 128, 0, st>>>(tp); break;
         case 1: k_traceback<64, false><<<grid, 128, 0, st>>>(tp); break;
