@@ -391,9 +391,10 @@ def test_local_mode_edges():
         alpha = rng.choice(["A", "AC", "AC", "ACG", "ACGTN"])
         wins.append("".join(rng.choice(alpha) for _ in range(rng.randint(1, 70))))
         reads.append("".join(rng.choice(alpha) for _ in range(rng.randint(1, 40))))
-    wins += ["CCCC", "A", "ACGTACGTAC", "TTTTACGTACGTTTTT"]
-    reads += ["GGGG", "CACA", "GTAC", "GGGACGTACGGGG"]
-    for sc in (DEFAULT, OracleScoring(2, -1, 1, 1, 0.5), OracleScoring(3, -9, 1, 1, 0.6), OracleScoring(1, -4, 6, 1, 0.9)):
+    wins += ["CCCC", "A", "ACGTACGTAC", "TTTTACGTACGTTTTT", "ACGTCANTGCATC", "ACGTCANTG"]
+    reads += ["GGGG", "CACA", "GTAC", "GGGACGTACGGGG", "ACGTCANTGCATC", "ACGTCANTG"]     # N against N inside / beside an alignment
+    for sc in (DEFAULT, OracleScoring(2, -1, 1, 1, 0.5), OracleScoring(3, -9, 1, 1, 0.6), OracleScoring(1, -4, 6, 1, 0.9),
+               OracleScoring(1, -3, 5, 2, 0.0)):                      # threshold 0: an empty alignment still fails the filter
         c = make_ctx(sc)
         try:
             c.set_mode(local=True)

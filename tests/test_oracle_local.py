@@ -114,6 +114,16 @@ def test_hand_computed_local_cases():
     assert (r["cigar"], r["pass"]) == ("8M2S", 1)
     r = oracle.align_pair("ACGTACGT", "ACGTACGTGG", OracleScoring(1, -3, 5, 2, 0.800001), local=True)
     assert r["pass"] == 0
+    # an empty alignment never passes, not even with the threshold at zero (0 * 1e6 >= 0 * 4 would hold)
+    r = oracle.align_pair("CCCC", "GGGG", OracleScoring(1, -3, 5, 2, 0.0), local=True)
+    assert (r["score"], r["n_cols"], r["pass"]) == (0, 0, 0)
+    # N against N is a mismatch inside a local alignment too and is not counted as a match (R8): the two 6-mers around
+    # it outweigh it, 6 - 3 + 6 = 9 > 6, so the column is aligned: 13 columns, 12 matches
+    r = oracle.align_pair("ACGTCANTGCATC", "ACGTCANTGCATC", sc, local=True)
+    assert (r["score"], r["cigar"], r["n_match"], r["n_cols"], r["pass"]) == (9, "13M", 12, 13, 1)
+    # ... and a lone N-N column next to one flank only is clipped with the shorter side: ACGTCA | N | TG
+    r = oracle.align_pair("ACGTCANTG", "ACGTCANTG", sc, local=True)
+    assert (r["score"], r["cigar"], r["n_match"], r["n_cols"]) == (6, "6M3S", 6, 6)
 
 
 def test_closed_form_exact_core_in_junk():
