@@ -160,10 +160,12 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
 int sdp_set_chunks(sdp_ctx* ctx, int chunks);
 
 /* Same operation with HOST pointers in `batch`: copies the inputs into device buffers owned by the ctx
- * (cudaMemcpyAsync on an internal stream, straight from the caller's arrays: pass page-locked memory for full PCIe
+ * (cudaMemcpyAsync on internal streams, straight from the caller's arrays: pass page-locked memory for full PCIe
  * speed; pageable memory is accepted, the driver then stages the copies and they run synchronously), runs
- * sdp_align_batch's pipeline, and copies every result array back into one pinned slab; `out` then holds pinned HOST
- * pointers owned by the ctx, valid until the next call on this ctx. */
+ * sdp_align_batch's pipeline, and copies every result array back into pinned memory; `out` then holds pinned HOST
+ * pointers owned by the ctx, valid until the next call on this ctx. The offsets, lengths and the pair list go first,
+ * so that validation and bucketing run while the sequences are still uploading; score and ref_end are downloaded as
+ * soon as the forward pass is done. To hide the remaining copies, drive two contexts from two host threads. */
 int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* batch, sdp_result* out);
 
 /*

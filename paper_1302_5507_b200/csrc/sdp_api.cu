@@ -106,6 +106,11 @@ struct sdp_ctx {
     Lane lane[SDP_MAX_LANES];
     int lanes_ready = 0;                  // lanes whose streams, events and fixed-size buffers exist
     cudaStream_t own_stream = nullptr;    // sdp_align_batch_host
+    cudaStream_t copy_stream = nullptr;   // sdp_align_batch_host: sequence upload beside the bucket stage, early result download
+    cudaEvent_t ev_seq_ready = nullptr;   // ... the sequences have arrived
+    bool wait_seq = false;                // this call's forward pass (and pre-pass) must wait for ev_seq_ready
+    int32_t* h_early_score = nullptr;     // host arrays score / ref_end go to as soon as a lane's forward pass is done
+    int32_t* h_early_ref_end = nullptr;
     cudaStream_t fwd_stream = nullptr;    // every lane's forward score kernels, lowest priority
     cudaStream_t fan_fwd[SDP_FAN_STREAMS] = {};    // [0] unused; forward / reverse / trace launches of several K classes
     cudaStream_t fan_post[SDP_FAN_STREAMS] = {};   // [0] unused; the short sort and scan chains after the forward pass
@@ -116,7 +121,7 @@ struct sdp_ctx {
     DevBuf score, ref_start, ref_end, read_start, read_end, pass, n_match, n_cols, cigar_off, cigar_len, cigar_ops;
     // sdp_align_batch_host: device copies of the inputs and pinned host copies of the outputs
     DevBuf in_reads, in_read_off, in_read_len, in_read_nmask, in_wins, in_win_off, in_win_len, in_win_nmask, in_pairs;
-    DevBuf h_out;                    // one pinned slab, carved per call
+    DevBuf h_out, h_ops;             // pinned: the per-pair result arrays (one slab, carved per call) and the CIGAR runs
     // sdp_best_per_read
     DevBuf rb_key, rb_pair, rb_score, rb_second, rb_ncand;
     DevBuf mp_flag, mp_off;          // sdp_mate_pairs
@@ -340,6 +345,8 @@ int sdp_create(const sdp_scoring* s, int cuda_device, sdp_ctx** out)
         CU(cudaMalloc(&ctx->d_slot_of_n, SDP_NSLOTS * 2));
         CU(cudaMemcpy(ctx->d_slot_of_n, ctx->h_slot_of_n, SDP_NSLOTS * 2, cudaMemcpyHostToDevice));
         CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->ev_seq_ready, cudaEventDisableTiming));
         // Three priority levels (numerically lower = higher priority): the forward kernels of all lanes at the lowest,
         // the narrow-band traceback kernels in the middle, each lane's own stream (bookkeeping, reverse pass, wide
         // traceback: the lane's critical path) at the highest, so that a lane's tail runs under the next lane's
@@ -384,6 +391,9 @@ void sdp_destroy(sdp_ctx* ctx)
                       &ctx->rb_ncand, &ctx->mp_flag, &ctx->mp_off};
     for (DevBuf* b : bufs) if (b->p) cudaFree(b->p);
     if (ctx->h_out.p) cudaFreeHost(ctx->h_out.p);
+    if (ctx->h_ops.p) cudaFreeHost(ctx->h_ops.p);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_seq_ready) cudaEventDestroy(ctx->ev_seq_ready);
     cudaFree(ctx->cig_total);
     cudaFree(ctx->d_slot_n); cudaFree(ctx->d_slot_G); cudaFree(ctx->d_slot_K); cudaFree(ctx->d_slot_of_n);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
@@ -555,6 +565,7 @@ int lane_phase_a(sdp_ctx* ctx, Lane& L, const int local)
     cudaStream_t st = L.st;
     L.nl = 0; L.fwd_launches = 0; L.n_wide = 0;
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A0], st));
+    if (ctx->wait_seq && ctx->prefilter) CU(cudaStreamWaitEvent(st, ctx->ev_seq_ready, 0));   // the pre-pass reads sequences
     CU(cudaMemsetAsync(L.zero_block, 0, L.zero_bytes, st));
     launch_validate_key(b, ctx->sc, L.keys.as<uint32_t>(), L.pn.as<uint32_t>(), L.pm.as<uint32_t>(),
                         L.hist[0], L.err_flag, L.counters + 3, (ctx->prefilter && !local) ? 1 : 0,
@@ -587,6 +598,7 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A1], st));
     CU(cudaEventRecord(L.ev_desc, st));
     CU(cudaStreamWaitEvent(fs, L.ev_desc, 0));
+    if (ctx->wait_seq) CU(cudaStreamWaitEvent(fs, ctx->ev_seq_ready, 0));     // host path: sequences upload beside a1/a2
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_F0], fs));
     {
         uint32_t before = L.nl;
@@ -605,6 +617,12 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_F1], fs));
     CU(cudaEventRecord(L.ev_fwd, fs));
     CU(cudaStreamWaitEvent(st, L.ev_fwd, 0));
+    if (ctx->h_early_score) {
+        // host path: score and ref_end are final now; their download runs under the rest of the path
+        CU(cudaStreamWaitEvent(ctx->copy_stream, L.ev_fwd, 0));
+        CU(cudaMemcpyAsync(ctx->h_early_score + L.p0, ctx->score.as<int32_t>() + L.p0, P * 4, cudaMemcpyDeviceToHost, ctx->copy_stream));
+        CU(cudaMemcpyAsync(ctx->h_early_ref_end + L.p0, ctx->ref_end.as<int32_t>() + L.p0, P * 4, cudaMemcpyDeviceToHost, ctx->copy_stream));
+    }
 
     if (ctx->score_only) {
         // candidate screening (step-3 shape): score and ref_end only; everything the traceback would fill reads
@@ -1020,42 +1038,51 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
     // the caller's buffers are only guaranteed readable to the end of the last word in use
     const size_t rb = (size_t)((hb->reads_bases + 15) / 16) * 4, wb = (size_t)((hb->wins_bases + 15) / 16) * 4;
     const size_t rnb = (size_t)((hb->reads_bases + 31) / 32) * 4, wnb = (size_t)((hb->wins_bases + 31) / 32) * 4;
+    // The small arrays (all the bucket stage needs) go first on the call's stream; the sequences follow on the copy
+    // stream, so that they upload beside a1/a2, and the forward pass waits for them.
     Cp cps[] = {
-        {&ctx->in_reads, hb->reads_packed, rb, (const void**)&d.reads_packed},
+        {&ctx->in_pairs, hb->pairs, (size_t)P * 8, (const void**)&d.pairs},
         {&ctx->in_read_off, hb->read_off, (size_t)hb->n_reads * 8, (const void**)&d.read_off},
         {&ctx->in_read_len, hb->read_len, (size_t)hb->n_reads * 4, (const void**)&d.read_len},
-        {&ctx->in_read_nmask, hb->read_nmask, rnb, (const void**)&d.read_nmask},
-        {&ctx->in_wins, hb->wins_packed, wb, (const void**)&d.wins_packed},
         {&ctx->in_win_off, hb->win_off, (size_t)hb->n_wins * 8, (const void**)&d.win_off},
         {&ctx->in_win_len, hb->win_len, (size_t)hb->n_wins * 4, (const void**)&d.win_len},
+        {&ctx->in_reads, hb->reads_packed, rb, (const void**)&d.reads_packed},
+        {&ctx->in_read_nmask, hb->read_nmask, rnb, (const void**)&d.read_nmask},
+        {&ctx->in_wins, hb->wins_packed, wb, (const void**)&d.wins_packed},
         {&ctx->in_win_nmask, hb->win_nmask, wnb, (const void**)&d.win_nmask},
-        {&ctx->in_pairs, hb->pairs, (size_t)P * 8, (const void**)&d.pairs},
     };
+    int ci = 0;
     for (Cp& c : cps) {
+        const cudaStream_t cs = ci++ < 5 ? st : ctx->copy_stream;
         if (!c.src) { *c.dst = nullptr; continue; }
         int rc = ensure(ctx, *c.buf, c.bytes + 64);
         if (rc != SDP_OK) return rc;
-        if (c.bytes) CU(cudaMemcpyAsync(c.buf->p, c.src, c.bytes, cudaMemcpyHostToDevice, st));
+        if (c.bytes) CU(cudaMemcpyAsync(c.buf->p, c.src, c.bytes, cudaMemcpyHostToDevice, cs));
         *c.dst = c.buf->p;
     }
-    sdp_result dr{};
-    int rc = sdp_align_batch(ctx, &d, st, &dr);
-    if (rc != SDP_OK) return rc;
-    // results back into one pinned slab
+    CU(cudaEventRecord(ctx->ev_seq_ready, ctx->copy_stream));
+    // per-pair results go into one pinned slab (sized before the call: score and ref_end leave early), the runs into another
     const size_t Pp = (size_t)(P ? P : 1);
-    const size_t n_ops = (size_t)dr.n_cigar_ops;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off += (bytes + 63) / 64 * 64; return o; };
     const size_t o_score = carve(Pp * 4), o_rs = carve(Pp * 4), o_re = carve(Pp * 4), o_qs = carve(Pp * 4),
                  o_qe = carve(Pp * 4), o_pass = carve(Pp), o_nm = carve(Pp * 4), o_nc = carve(Pp * 4),
-                 o_coff = carve(Pp * 8), o_clen = carve(Pp * 4), o_ops = carve((n_ops + 1) * 4);
-    rc = ensure_pinned(ctx, ctx->h_out, off);
+                 o_coff = carve(Pp * 8), o_clen = carve(Pp * 4);
+    int rc = ensure_pinned(ctx, ctx->h_out, off);
     if (rc != SDP_OK) return rc;
     char* h = (char*)ctx->h_out.p;
+    sdp_result dr{};
+    ctx->wait_seq = true;
+    ctx->h_early_score = (int32_t*)(h + o_score); ctx->h_early_ref_end = (int32_t*)(h + o_re);
+    rc = sdp_align_batch(ctx, &d, st, &dr);
+    ctx->wait_seq = false; ctx->h_early_score = nullptr; ctx->h_early_ref_end = nullptr;
+    if (rc != SDP_OK) { cudaStreamSynchronize(ctx->copy_stream); return rc; }
+    const size_t n_ops = (size_t)dr.n_cigar_ops;
+    rc = ensure_pinned(ctx, ctx->h_ops, (n_ops + 1) * 4);
+    if (rc != SDP_OK) { cudaStreamSynchronize(ctx->copy_stream); return rc; }
+    char* hops = (char*)ctx->h_ops.p;
     if (P) {
-        CU(cudaMemcpyAsync(h + o_score, dr.score, P * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_rs, dr.ref_start, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_re, dr.ref_end, P * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_qs, dr.read_start, P * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_qe, dr.read_end, P * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_pass, dr.pass, P, cudaMemcpyDeviceToHost, st));
@@ -1063,15 +1090,16 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
         CU(cudaMemcpyAsync(h + o_nc, dr.n_cols, P * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_coff, dr.cigar_off, P * 8, cudaMemcpyDeviceToHost, st));
         CU(cudaMemcpyAsync(h + o_clen, dr.cigar_len, P * 4, cudaMemcpyDeviceToHost, st));
-        if (n_ops) CU(cudaMemcpyAsync(h + o_ops, dr.cigar_ops, n_ops * 4, cudaMemcpyDeviceToHost, st));
+        if (n_ops) CU(cudaMemcpyAsync(hops, dr.cigar_ops, n_ops * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
     }
+    CU(cudaStreamSynchronize(ctx->copy_stream));
     out->score = (const int32_t*)(h + o_score); out->ref_start = (const int32_t*)(h + o_rs);
     out->ref_end = (const int32_t*)(h + o_re); out->read_start = (const int32_t*)(h + o_qs);
     out->read_end = (const int32_t*)(h + o_qe); out->pass = (const uint8_t*)(h + o_pass);
     out->n_match = (const int32_t*)(h + o_nm); out->n_cols = (const int32_t*)(h + o_nc);
     out->cigar_off = (const uint64_t*)(h + o_coff); out->cigar_len = (const uint32_t*)(h + o_clen);
-    out->cigar_ops = (const uint32_t*)(h + o_ops); out->n_cigar_ops = n_ops; out->n_pairs = P;
+    out->cigar_ops = (const uint32_t*)hops; out->n_cigar_ops = n_ops; out->n_pairs = P;
     return SDP_OK;
 }
 
