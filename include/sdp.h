@@ -106,20 +106,21 @@ typedef struct sdp_result {
     uint64_t        n_pairs;
 } sdp_result;
 
-/* Per-call counters; times are CUDA-event milliseconds on the caller's stream and are only
- * filled when timing was switched on with sdp_set_timing(ctx, 1). */
+/* Per-call counters; times are CUDA-event milliseconds on the library's streams and are only
+ * filled when timing was switched on with sdp_set_timing(ctx, 1). With more than one lane (sdp_set_chunks) the
+ * per-stage times are summed over the lanes, whose stages overlap: only ms_total is wall time then. */
 typedef struct sdp_stats {
     uint64_t n_pairs;
     uint64_t cells_forward;       /* sum n*m: the CUPS numerator                                 */
     uint64_t cells_reverse;       /* cells of the reverse pass                                   */
     uint64_t cells_traceback;     /* band cells of the traceback pass                            */
-    uint64_t n_reverse_pairs;     /* pairs whose score allows a gap (W > 0)                      */
+    uint64_t n_reverse_pairs;     /* pairs that took the reverse pass (a4)                       */
     uint32_t kernel_launches;     /* kernels of this library launched by the call                */
     uint32_t forward_launches;    /* launches of the forward score kernel                        */
     float ms_total;               /* whole call, first kernel to last                            */
     float ms_bucket;              /* a1 + a2 validate, histogram, scan, scatter, task build      */
     float ms_forward;             /* a3 forward score kernels                                    */
-    float ms_reverse;             /* a4                                                          */
+    float ms_reverse;             /* post-forward bookkeeping (gap bounds, bucket sorts, one host round trip) + a4 */
     float ms_traceback;           /* a5 + a6                                                     */
     float ms_compact;             /* a7 + a8                                                     */
     uint64_t cells_prefiltered;   /* sum n*m of the pairs the ungapped pre-pass settled (sdp_set_prefilter);
