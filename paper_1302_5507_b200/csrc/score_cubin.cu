@@ -16,14 +16,14 @@
     extern "C" __global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))                 \
     SDP_CAT3(sdp_score_k, K, SUFFIX)(const ScoreParams P)                                                  \
     {                                                                                                      \
-        __shared__ uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];                                   \
+        __shared__ __align__(16) uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];                                 \
         sdp::score_body<K, REV, PAD>(P, ring_mem);                                                         \
     }
 #define SDP_DEFINE_TRACE(K, SUFFIX, PAD)                                                                   \
     extern "C" __global__ void __launch_bounds__(SDP_SCORE_THREADS, SDP_SCORE_MIN_CTAS(K))                 \
     SDP_CAT3(sdp_trace_k, K, SUFFIX)(const ScoreParams P, const TraceDP T)                                 \
     {                                                                                                      \
-        __shared__ uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];                                   \
+        __shared__ __align__(16) uint32_t ring_mem[SDP_WARPS_PER_CTA][SDP_RING_WORDS];                                 \
         sdp::trace_body<K, PAD>(P, T, ring_mem);                                                           \
     }
 #define SDP_DEFINE_SCORE_ALL(K)         \
