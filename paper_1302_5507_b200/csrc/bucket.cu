@@ -70,7 +70,7 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
                                unsigned long long* __restrict__ cells, int prefilter,
                                int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
                                unsigned long long* __restrict__ cells_skipped, int local,
-                               uint32_t* __restrict__ slow_words)
+                               uint32_t* __restrict__ slow_words, unsigned long long* __restrict__ slow_total)
 {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t key = SDP_KEY_SKIP, err = 0, slow = 0;
@@ -127,16 +127,21 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
             if ((threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(hist + key, (uint32_t)__popc(peers));
         }
     }
-    // cells: one atomic per block
+    // cells and int32-lane words: one atomic each per block
     {
-        __shared__ unsigned long long s_cells[8];
-        for (int o = 16; o > 0; o >>= 1) my_cells += __shfl_down_sync(0xffffffffu, my_cells, o);
-        if ((threadIdx.x & 31) == 0) s_cells[threadIdx.x >> 5] = my_cells;
+        __shared__ unsigned long long s_cells[8], s_slow[8];
+        unsigned long long my_slow = slow;
+        for (int o = 16; o > 0; o >>= 1) {
+            my_cells += __shfl_down_sync(0xffffffffu, my_cells, o);
+            my_slow += __shfl_down_sync(0xffffffffu, my_slow, o);
+        }
+        if ((threadIdx.x & 31) == 0) { s_cells[threadIdx.x >> 5] = my_cells; s_slow[threadIdx.x >> 5] = my_slow; }
         __syncthreads();
         if (threadIdx.x == 0) {
-            unsigned long long t = 0;
-            for (int k = 0; k < (int)(blockDim.x >> 5); ++k) t += s_cells[k];
+            unsigned long long t = 0, u = 0;
+            for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { t += s_cells[k]; u += s_slow[k]; }
             if (t) atomicAdd(cells, t);
+            if (u) atomicAdd(slow_total, u);
         }
     }
 }
@@ -203,9 +208,21 @@ __global__ void __launch_bounds__(1024) k_scan_bins_finish(uint32_t* __restrict_
 // then serialises on that bin's cursor (31,250 atomics on one address for a million pairs: 75 us). So the key of the
 // block's first thread is handled per BLOCK (one atomic for all threads that share it, positions from a ballot /
 // warp-count scan); every other key takes the warp-aggregated path.
+// DESC: the forward sort. Instead of the pair's index the thread writes the pair's forward descriptor straight to its
+// place in bucket order (one kernel and one pass over `order` less than scatter + gather).
+template <bool DESC>
 __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ keys, uint64_t n, uint32_t* __restrict__ cursor,
-                                                 uint32_t* __restrict__ order)
+                                                 uint32_t* __restrict__ order, const sdp_batch b, PairDesc* __restrict__ desc)
 {
+    auto put = [&](const uint32_t pos, const uint64_t pp) {
+        if (DESC) {
+            const uint32_t ri = b.pairs[2 * pp], wi = b.pairs[2 * pp + 1];
+            PairDesc d;
+            d.roff = b.read_off[ri]; d.woff = b.win_off[wi];
+            d.n = b.read_len[ri]; d.m = b.win_len[wi]; d.pid = (uint32_t)pp; d.aux = 0;
+            desc[pos] = d;
+        } else order[pos] = (uint32_t)pp;
+    };
     __shared__ uint32_t s_key, s_base, s_wcnt[8];
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t key = p < n ? keys[p] : SDP_KEY_SKIP;
@@ -228,7 +245,7 @@ __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ ke
         uint32_t pre = 0;
 #pragma unroll
         for (int k = 0; k < 8; ++k) pre += (k < (int)w) ? s_wcnt[k] : 0u;
-        order[s_base + pre + (uint32_t)__popc(same_mask & ((1u << lane) - 1u))] = (uint32_t)p;
+        put(s_base + pre + (uint32_t)__popc(same_mask & ((1u << lane) - 1u)), p);
     }
     const bool other = !same && key != SDP_KEY_SKIP;
     const uint32_t active = __ballot_sync(0xffffffffu, other);
@@ -238,7 +255,7 @@ __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ ke
         uint32_t base = 0;
         if (lane == (uint32_t)leader) base = atomicAdd(cursor + key, (uint32_t)__popc(peers));
         base = __shfl_sync(peers, base, leader);
-        order[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)p;
+        put(base + (uint32_t)__popc(peers & ((1u << lane) - 1u)), p);
     }
 }
 
@@ -266,21 +283,6 @@ __global__ void __launch_bounds__(1024) k_tasks(const uint32_t* __restrict__ bin
     task_prefix[t] = pre;
     host_prefix[t] = pre;                                 // pinned host mailbox: the host sizes the launches from it
     if (t == 0) { task_prefix[SDP_NSLOTS] = total; host_prefix[SDP_NSLOTS] = total; *host_total = bin_start[SDP_NBINS]; }
-}
-
-// ---------------------------------------------------------------------------------------------
-// pair descriptors in bucket order for the forward pass
-__global__ void k_fill_desc_fwd(const sdp_batch b, const uint32_t* __restrict__ order, uint32_t count,
-                                PairDesc* __restrict__ desc)
-{
-    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= count) return;
-    const uint32_t p = order[k];
-    const uint32_t ri = b.pairs[2 * (uint64_t)p], wi = b.pairs[2 * (uint64_t)p + 1];
-    PairDesc d;
-    d.roff = b.read_off[ri]; d.woff = b.win_off[wi];
-    d.n = b.read_len[ri]; d.m = b.win_len[wi]; d.pid = p; d.aux = 0;
-    desc[k] = d;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -410,27 +412,24 @@ void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbou
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
                          int32_t* ref_end, unsigned long long* cells_skipped, int local, uint32_t* slow_words,
-                         cudaStream_t st)
+                         unsigned long long* slow_total, cudaStream_t st)
 {
     const uint32_t grid = (uint32_t)((b.n_pairs + 255) / 256);
     k_validate_key<<<grid, 256, 0, st>>>(b, sc, keys, pn, pm, hist, err_flag, cells, prefilter, score, ref_end, cells_skipped,
-                                         local, slow_words);
+                                         local, slow_words, slow_total);
 }
 
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
-                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st)
+                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st,
+                      const sdp_batch* b_desc, PairDesc* desc)
 {
     uint32_t* tile_sums = bin_start + SDP_NBINS + 4;        // scratch behind the total (SDP_BIN_SCRATCH words)
     k_scan_bins_tiles<<<BIN_TILES, 1024, 0, st>>>(hist, bin_start, tile_sums);
     k_scan_bins_finish<<<BIN_TILES, 1024, 0, st>>>(hist, bin_start, tile_sums);
-    k_scatter<<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist, order);
+    if (b_desc) k_scatter<true><<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist, order, *b_desc, desc);
+    else        k_scatter<false><<<(uint32_t)((n + 255) / 256), 256, 0, st>>>(keys, n, hist, order, sdp_batch{}, nullptr);
     if (slots) k_tasks<<<1, 1024, 0, st>>>(bin_start, slot_n, slot_G, slot_K, slots, task_prefix, host_prefix, host_total);
-}
-
-void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st)
-{
-    if (count) k_fill_desc_fwd<<<(count + 255) / 256, 256, 0, st>>>(b, order, count, desc);
 }
 
 }  // namespace sdp

@@ -570,15 +570,14 @@ int lane_phase_a(sdp_ctx* ctx, Lane& L, const int local)
     launch_validate_key(b, ctx->sc, L.keys.as<uint32_t>(), L.pn.as<uint32_t>(), L.pm.as<uint32_t>(),
                         L.hist[0], L.err_flag, L.counters + 3, (ctx->prefilter && !local) ? 1 : 0,
                         ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0, L.counters + 4, local,
-                        L.slow_words.as<uint32_t>(), st);
-    // row arrays of the int32 lane: offsets now, so that the arrays can be allocated after the host has seen the total
-    exclusive_scan_u32_u64(L.slow_words.as<uint32_t>(), P, L.slow_off.as<uint64_t>(), L.totals + 0, nullptr,
-                           L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
-                           L.scan_tile_base[0].as<uint64_t>(), st, &L.nl);
-    CU(cudaMemcpyAsync(&L.mb->slow_total, L.totals + 0, 8, cudaMemcpyDeviceToHost, st));
+                        L.slow_words.as<uint32_t>(), L.counters + 5, st);
+    // (row arrays of the int32 lane: the host learns their total here; their offsets are scanned in phase B, and only
+    // when there are any)
+    CU(cudaMemcpyAsync(&L.mb->slow_total, L.counters + 5, 8, cudaMemcpyDeviceToHost, st));
+    // bucket sort; the scatter writes the forward descriptors straight into bucket order
     launch_sort_tail(L.keys.as<uint32_t>(), P, L.hist[0], L.bin_start[0], L.order.as<uint32_t>(),
                      ctx->d_slot_n, ctx->d_slot_G, ctx->d_slot_K, L.slots[0], L.task_prefix[0],
-                     L.mb->task_prefix[0], &L.mb->bin_total[0], st);
+                     L.mb->task_prefix[0], &L.mb->bin_total[0], st, &L.b, L.desc.as<PairDesc>());
     L.nl += 5;
     CU(cudaMemcpyAsync(&L.mb->err_flag, L.err_flag, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaEventRecord(L.evA, st));
@@ -592,9 +591,6 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     const sdp_batch& b = L.b;
     const uint64_t P = L.P;
     cudaStream_t st = L.st, fs = ctx->fwd_stream;
-    // (with the ungapped pre-pass on, fewer than P pairs are in the forward buckets)
-    launch_fill_desc_fwd(b, L.order.as<uint32_t>(), L.mb->bin_total[0], L.desc.as<PairDesc>(), st);
-    ++L.nl;
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A1], st));
     CU(cudaEventRecord(L.ev_desc, st));
     CU(cudaStreamWaitEvent(fs, L.ev_desc, 0));
@@ -609,6 +605,9 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     if (L.mb->slow_total) {
         // the int32 lane: pairs outside the int16 kernels' domain, and every pair in local mode (slow_lane.cu)
         LEN(slow_rows, (L.mb->slow_total + 4) * 4);
+        exclusive_scan_u32_u64(L.slow_words.as<uint32_t>(), P, L.slow_off.as<uint64_t>(), L.totals + 0, nullptr,
+                               L.scan_local[0].as<uint32_t>(), L.scan_tiles[0].as<uint32_t>(),
+                               L.scan_tile_base[0].as<uint64_t>(), fs, &L.nl);
         launch_forward_i32(b, ctx->sc, local, L.slow_words.as<uint32_t>(), L.slow_off.as<uint64_t>(),
                            L.slow_rows.as<int32_t>(), ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0,
                            L.rev_rows.as<int32_t>(), fs);

@@ -14,15 +14,16 @@ struct Scoring {
 void launch_validate_key(const sdp_batch& b, const Scoring& sc, uint32_t* keys, uint32_t* pn, uint32_t* pm,
                          uint32_t* hist, uint32_t* err_flag, unsigned long long* cells, int prefilter, int32_t* score,
                          int32_t* ref_end, unsigned long long* cells_skipped, int local, uint32_t* slow_words,
-                         cudaStream_t st);
-// scan bins, scatter into `order`, and (if slots != nullptr) build the per-read-length task table
+                         unsigned long long* slow_total, cudaStream_t st);
+// scan bins, scatter into `order` (or, with b_desc != nullptr, write the forward descriptors of *b_desc straight into
+// `desc` in bucket order), and (if slots != nullptr) build the per-read-length task table
 void launch_sort_tail(const uint32_t* keys, uint64_t n, uint32_t* hist, uint32_t* bin_start, uint32_t* order,
                       const uint16_t* slot_n, const uint16_t* slot_G, const uint16_t* slot_K,
-                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st);
+                      SlotInfo* slots, uint32_t* task_prefix, uint32_t* host_prefix, uint32_t* host_total, cudaStream_t st,
+                      const sdp_batch* b_desc = nullptr, PairDesc* desc = nullptr);
 void launch_mailbox(const uint32_t* tb_bin_start, uint32_t stride, uint32_t nbounds, const uint64_t* totals,
                     const unsigned long long* counters, uint32_t* host_bounds, uint64_t* host_totals,
                     unsigned long long* host_counters, cudaStream_t st);
-void launch_fill_desc_fwd(const sdp_batch& b, const uint32_t* order, uint32_t count, PairDesc* desc, cudaStream_t st);
 // exclusive scan of n 32-bit values into 64-bit offsets starting at *base_dev (0 when null); *total_dev = base + sum
 void exclusive_scan_u32_u64(const uint32_t* in, uint64_t n, uint64_t* out, uint64_t* total_dev, const uint64_t* base_dev,
                             uint32_t* tmp_local, uint32_t* tmp_tiles, uint64_t* tmp_tile_base,
