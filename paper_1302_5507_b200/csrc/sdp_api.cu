@@ -567,6 +567,7 @@ int lane_phase_a(sdp_ctx* ctx, Lane& L, const int local)
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_A0], st));
     if (ctx->wait_seq && ctx->prefilter) CU(cudaStreamWaitEvent(st, ctx->ev_seq_ready, 0));   // the pre-pass reads sequences
     CU(cudaMemsetAsync(L.zero_block, 0, L.zero_bytes, st));
+    CU(cudaMemsetAsync(L.wide_words.p, 0, P * 4, st));       // region sizes of the wide traceback (filled after the forward pass)
     launch_validate_key(b, ctx->sc, L.keys.as<uint32_t>(), L.pn.as<uint32_t>(), L.pm.as<uint32_t>(),
                         L.hist[0], L.err_flag, L.counters + 3, (ctx->prefilter && !local) ? 1 : 0,
                         ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0, L.counters + 4, local,
@@ -667,7 +668,6 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
     L.nl += 8;
     // one region of direction nibbles per warp task of wide pairs (every slot of order_wide beyond the wide
     // pairs reads as a zero-size region)
-    CU(cudaMemsetAsync(L.wide_words.p, 0, P * 4, st));
     launch_wide_regions(L.order_wide.as<uint32_t>(), (uint32_t)P, L.bin_start[3] + SDP_NBINS, L.pn.as<uint32_t>(),
                         L.tb_rows.as<int32_t>(), ctx->d_slot_of_n, L.slots[2], L.wide_words.as<uint32_t>(), st);
     ++L.nl;
