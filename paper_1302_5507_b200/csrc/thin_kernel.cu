@@ -398,7 +398,8 @@ __device__ __forceinline__ void thin_dispatch(const int w, const TraceParams& tp
 template <int LO, int HI>
 __global__ void __launch_bounds__(128) k_thin_range(const TraceParams tp, const ThinConsts tc, const ThinRanges r)
 {
-    const uint32_t b = blockIdx.x + r.block_start[LO];
+    // widest bands and longest rows first (blocks are dispatched in index order): the cheap classes fill the tail
+    const uint32_t b = (gridDim.x - 1u - blockIdx.x) + r.block_start[LO];
     int w = LO;
 #pragma unroll
     for (int c = LO + 1; c < HI; ++c) w += (b >= r.block_start[c]) ? 1 : 0;
