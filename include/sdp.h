@@ -193,6 +193,35 @@ int sdp_best_per_read(sdp_ctx* ctx, const sdp_batch* batch, const sdp_result* re
                       sdp_read_best* out);
 
 /*
+ * The same per-read choice (same rule, same four outputs, bit for bit) for callers that must not allocate device
+ * memory: programs that gave the whole card to their own pool at start-up (a later cudaMalloc may fail or fragment
+ * it), and programs with several busy streams, which cudaMalloc / cudaFree would stall device-wide. It takes no
+ * sdp_ctx (sdp_create allocates) and calls no cudaMalloc, cudaFree or allocating library routine. `pairs` [2*n_pairs]
+ * and `score` [n_pairs] are DEVICE inputs (for instance sdp_batch.pairs and sdp_result.score of an earlier
+ * sdp_align_batch); best_pair, best_score, second_score and n_candidates are caller-owned DEVICE arrays of n_reads
+ * entries, filled as sdp_read_best describes. A pair whose read index is >= n_reads is ignored.
+ *
+ * The method's working memory, one 64-bit key per read, is a fixed array inside the library:
+ * SDP_STATIC_MAX_READS * 8 bytes = 8 MiB, held by every GPU that loads libsdp.so until the process exits. That array
+ * is the limit: n_reads > SDP_STATIC_MAX_READS returns SDP_ERANGE and does nothing (split the batch by read, or use
+ * sdp_best_per_read). Every call on a device uses the same array and clears the part it needs first, so calls run
+ * one after another in any mix of sizes; two calls that can overlap on one GPU (different streams with no ordering
+ * between them, or two host threads) race on it and give garbage: order them yourself.
+ *
+ * The work is enqueued on `cuda_stream` (NULL = default stream) of device `cuda_device` and the call returns without
+ * waiting; the outputs are complete when the stream reaches that point. The first call on each device also looks up
+ * the array's device address (cudaGetSymbolAddress, which loads the library's device code there if nothing has yet):
+ * make that first call during start-up, before any stream capture begins. The caller's current device is restored.
+ * Returns SDP_OK, SDP_EINVAL (null array, device outside 0..63), SDP_ERANGE (n_reads as above, or n_pairs beyond
+ * 32 bits), SDP_ECUDA. sdp_static_last_error() gives the message of the calling thread's last failure ("" if none).
+ */
+#define SDP_STATIC_MAX_READS (1u << 20)
+int sdp_best_per_read_static(int cuda_device, const uint32_t* pairs, const int32_t* score, uint64_t n_pairs,
+                             uint32_t n_reads, void* cuda_stream, uint32_t* best_pair, int32_t* best_score,
+                             int32_t* second_score, uint32_t* n_candidates);
+const char* sdp_static_last_error(void);
+
+/*
  * Alignment mode. SDP_MODE_SEMIGLOBAL (default) is the paper's formulation: the whole read against any sub-region of
  * the window. SDP_MODE_LOCAL is the soft-clipping variant (the paper names
  * Smith-Waterman, and soft-clipped alignments; R18): M(i,0) = M(0,j) = 0,

@@ -13,10 +13,11 @@ from .binding import (  # noqa: E402,F401
     HostResult,
     SDP_NO_PAIR,
     SdpError,
+    best_per_read_static,
     load_library,
     sdp_measure_dpx_rate,
     sdp_version,
 )
 
-__all__ += ["Context", "DeviceBatch", "HostResult", "SdpError", "load_library", "sdp_measure_dpx_rate",
+__all__ += ["Context", "DeviceBatch", "HostResult", "SdpError", "best_per_read_static", "load_library", "sdp_measure_dpx_rate",
             "sdp_version"]

@@ -25,7 +25,7 @@ SDP_ROUTE_NO_THIN, SDP_ROUTE_NO_WIDE, SDP_ROUTE_ALWAYS_REVERSE = 1, 2, 4
 EXPORTS = ["sdp_create", "sdp_align_batch", "sdp_align_batch_host", "sdp_get_stats", "sdp_set_timing",
            "sdp_last_error", "sdp_destroy", "sdp_measure_dpx_rate", "sdp_version", "sdp_best_per_read",
            "sdp_set_score_only", "sdp_set_prefilter", "sdp_set_debug_route", "sdp_set_mode", "sdp_set_chunks", "sdp_mate_windows", "sdp_mate_pairs",
-           "sdp_proper_pairs"]
+           "sdp_proper_pairs", "sdp_best_per_read_static", "sdp_static_last_error"]
 
 
 class SdpError(RuntimeError):
@@ -103,6 +103,11 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.sdp_best_per_read.restype = ctypes.c_int
     lib.sdp_best_per_read.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_batch), ctypes.POINTER(sdp_result),
                                       ctypes.c_void_p, ctypes.POINTER(sdp_read_best)]
+    lib.sdp_best_per_read_static.restype = ctypes.c_int
+    lib.sdp_best_per_read_static.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32,
+                                             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    lib.sdp_static_last_error.restype = ctypes.c_char_p
+    lib.sdp_static_last_error.argtypes = []
     lib.sdp_mate_windows.restype = ctypes.c_int
     lib.sdp_mate_windows.argtypes = [ctypes.c_void_p, ctypes.POINTER(sdp_mates), ctypes.c_uint32, ctypes.c_uint32,
                                      ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
@@ -150,6 +155,32 @@ def sdp_measure_dpx_rate(device: int = 0) -> dict:
     if rc != SDP_OK:
         raise SdpError(rc, "sdp_measure_dpx_rate")
     return dict(instr_per_clk_per_sm=rate.value, sm_count=sms.value, sm_mhz=mhz.value)
+
+
+SDP_STATIC_MAX_READS = 1 << 20
+
+
+def best_per_read_static(pairs, score, n_pairs: int, n_reads: int, best_pair, best_score, second_score, n_candidates,
+                         device: int = 0, stream=None) -> None:
+    """sdp_best_per_read_static: the per-read choice without a context and without any device allocation by the
+    library, for callers whose GPU memory is all spoken for. Every array is device memory the caller made beforehand,
+    given as a torch CUDA tensor or a raw device address (e.g. ``sdp_result.score``): ``pairs`` (int32 [n_pairs, 2])
+    and ``score`` (int32 [n_pairs]) in, the four int32 [n_reads] arrays out (best_pair and n_candidates hold unsigned
+    values). Only enqueues on ``stream`` (default: torch's current stream): synchronise before reading. Raises
+    SdpError, e.g. SDP_ERANGE when n_reads > SDP_STATIC_MAX_READS."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+
+    def ptr(x):
+        return ctypes.c_void_p(x.data_ptr() if hasattr(x, "data_ptr") else x)
+
+    lib = load_library()
+    rc = lib.sdp_best_per_read_static(device, ptr(pairs), ptr(score), int(n_pairs), int(n_reads),
+                                      ctypes.c_void_p(stream.cuda_stream), ptr(best_pair), ptr(best_score),
+                                      ptr(second_score), ptr(n_candidates))
+    if rc != SDP_OK:
+        raise SdpError(rc, lib.sdp_static_last_error().decode())
 
 
 @dataclass

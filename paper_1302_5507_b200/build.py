@@ -50,7 +50,8 @@ SENTINELS = {"negOc": 0x5D1A37C2, "negO": 0x2B6E4A91, "c2": 0x63C5195D, "Cd": 0x
 
 def _units():
     units = [("sdp_api", "sdp_api.cu", []), ("bucket", "bucket.cu", []), ("traceback", "traceback.cu", []), ("thin_kernel", "thin_kernel.cu", []),
-             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("mate", "mate.cu", []),
+             ("microbench", "microbench.cu", []), ("best_read", "best_read.cu", []), ("best_read_static", "best_read_static.cu", []),
+             ("mate", "mate.cu", []),
              ("score_modules", "score_modules.cu", []), ("slow_lane", "slow_lane.cu", [])]
     for r, (lo, hi) in enumerate(K_RANGES):
         units.append((f"cubin_r{r}", "score_cubin.cu", [f"-DSDP_K_LO={lo}", f"-DSDP_K_HI={hi}"]))
