@@ -47,11 +47,19 @@ extern "C" {
  * The int16 kernels store H + gap_extend*(i+j) + bias in 16-bit lanes; the left side bounds every stored value and
  * every intermediate sum (R13). A pair that breaks the rule, or whose read is longer than SDP_MAX_READ_LEN,
  * is never clamped and never rejected for that: it takes the int32 lane (one thread per pair, much slower, same
- * results). SDP_ERANGE is left for what that lane cannot hold either: a sequence longer than SDP_MAX_SEQ_LEN, or
- * traceback scratch of one pair beyond 16 GiB.
+ * results). SDP_ERANGE is left for what that lane cannot hold either: a sequence longer than SDP_MAX_SEQ_LEN, a pair
+ * outside the int32 range rule below, or traceback scratch of one pair beyond 16 GiB.
  */
 #define SDP_MAX_CELL_VALUE 32000
 #define SDP_MAX_SEQ_LEN 1000000
+/*
+ * int32 range rule (per pair): match*n + gap_extend*(n + 2) + 2*gap_open + |mismatch| < SDP_MAX_CELL_VALUE_I32.
+ * The int32 lane and the band traceback mark cells outside the table with -2^28; the rule keeps that mark, even after
+ * n matches were added to it, below every real cell value. It only binds for scorings far from the default: with
+ * 1/-3/5/2 a read of SDP_MAX_SEQ_LEN bases is inside it, with all four parameters at SDP_MAX_SCORE_PARAM reads up to
+ * about 33,000 bases are. A pair that breaks it makes the call return SDP_ERANGE (nothing is clamped).
+ */
+#define SDP_MAX_CELL_VALUE_I32 (1 << 28)
 /* Largest magnitude of match, mismatch, gap_open and gap_extend sdp_create accepts. */
 #define SDP_MAX_SCORE_PARAM 4000
 
@@ -125,7 +133,8 @@ typedef struct sdp_stats {
     float ms_compact;             /* a7 + a8                                                     */
     uint64_t cells_prefiltered;   /* sum n*m of the pairs the ungapped pre-pass settled (sdp_set_prefilter);
                                      cells_forward counts only the pairs that went through the DP   */
-    uint64_t n_slow_words;        /* int32 row-array words of the pairs that took the int32 lane (0 = none did)     */
+    uint64_t n_slow_words;        /* int32 scratch words of the pairs that took the int32 lane: 2*(n+1) per read over
+                                     SDP_MAX_READ_LEN bases, 1 per shorter read (0 = no pair took that lane)        */
 } sdp_stats;
 
 /* Create a context on CUDA device `cuda_device`. SDP_EINVAL for bad scoring or null arguments,

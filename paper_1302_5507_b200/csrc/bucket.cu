@@ -85,14 +85,23 @@ __global__ void k_validate_key(const sdp_batch b, const Scoring sc, uint32_t* __
                 err = SDP_ERRF_INDEX;
             else if (n > SDP_MAX_SEQ_LEN || m > SDP_MAX_SEQ_LEN)
                 err = SDP_ERRF_RANGE;                      // beyond even the int32 lane
+            else if ((long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + 2) + 2LL * sc.gap_open -
+                             (long long)sc.mismatch >= SDP_MAX_CELL_VALUE_I32)
+                // the int32 lane's minus infinity is -2^28 (traceback) / -2^29 (forward): every real cell value lies
+                // in [-(2*gap_open + gap_extend*(n+1)), match*n], and a sentinel plus up to n matches must stay below
+                // that range, or an out-of-band cell would beat a real one (sdp.h, int32 range rule)
+                err = SDP_ERRF_RANGE;
             else if (local || n > SDP_MAX_READ_LEN ||
                      (long long)sc.match * n + (long long)sc.gap_extend * ((long long)n + m + 32) + 3LL * sc.gap_open + 8 +
                              llabs(2LL * sc.gap_extend + sc.mismatch) > SDP_MAX_CELL_VALUE) {
                 // outside the int16 kernels' domain (or local mode): the int32 lane (slow_lane.cu) takes the pair; it
-                // never enters the forward buckets. slow_words = its two row arrays of n + 1 entries.
+                // never enters the forward buckets. slow_words = its two row arrays of n + 1 entries when the read is
+                // longer than SDP_MAX_READ_LEN (k_forward_i32); up to that length the warp kernels keep the rows in
+                // registers and the word is only the "took the int32 lane" flag (local mode on a full batch would
+                // otherwise reserve gigabytes nobody touches).
                 pn[p] = n; pm[p] = m;
                 my_cells = (unsigned long long)n * m;
-                slow = 2u * (n + 1u);
+                slow = n > SDP_MAX_READ_LEN ? 2u * (n + 1u) : 1u;
             } else {
                 key = (n - 1) * 64u + min(63u, m >> 6);
                 pn[p] = n; pm[p] = m;

@@ -441,6 +441,78 @@ def test_int32_lane(ctx):
         c.destroy()
 
 
+@pytest.mark.parametrize("route", ["local", "long_window", "large_scoring"])
+def test_int32_lane_reads_257_to_1024(route):
+    # reads of 257..1,024 bases on the int32 lane (forward_i32_warp<16> for 257..512, <32> for
+    # 513..1,024; row arrays of up to 1,025 cells in k_traceback<1032, .>), reached in each of the three ways a pair
+    # gets there: local mode, a window long enough to break the int16 range rule (PAPER.md:117,
+    # sdp.h), and a scoring whose constants alone break it. Placed, gapped, clipped and unplaceable reads.
+    rng = random.Random(63)
+
+    def rnd(k):
+        return "".join(rng.choice("ACGT") for _ in range(k))
+
+    wins, reads = [], []
+    for n in (257, 300, 400, 512, 513, 700, 1000, 1024):
+        for kind in ("placed", "indels", "clipped", "unplaceable"):
+            for _ in range(1 if route == "long_window" else 2):
+                m = 16500 + rng.randint(0, 300) if route == "long_window" else n + rng.randint(40, 600)
+                T = rnd(m)
+                s = rng.randrange(0, m - n + 1)
+                R = list(T[s:s + n])
+                for _ in range(rng.randint(0, n // 25)):
+                    R[rng.randrange(n)] = rng.choice("ACGT")
+                if kind == "indels":
+                    for _ in range(rng.randint(1, 4)):
+                        k, g = rng.randrange(10, len(R) - 40), rng.randint(1, 30)
+                        R = R[:k] + (list(rnd(g)) if rng.random() < 0.5 else []) + R[k + (0 if rng.random() < 0.5 else g):]
+                elif kind == "clipped":                          # foreign ends: soft clips in local mode, wide bands otherwise
+                    a, z = rng.randint(5, n // 3), rng.randint(5, n // 3)
+                    R = list(rnd(a)) + R[a:n - z] + list(rnd(z))
+                elif kind == "unplaceable":
+                    R = list(rnd(n))
+                reads.append(("".join(R) + rnd(n))[:n])
+                wins.append(T)
+    sc = OracleScoring(300, -400, 600, 200, 0.6) if route == "large_scoring" else DEFAULT
+    c = make_ctx(sc)
+    try:
+        c.set_mode(local=route == "local")
+        b = W.batch_from_strings(wins, reads)
+        exp, got = parity.check_batch(c, b, sc, f"int32 lane, n = 257..1024, {route}", local=route == "local")
+        assert c.stats()["n_slow_words"] == b.n_pairs           # every pair took the lane; none needs global row arrays
+        if route == "local":
+            n = b.read_len[b.pairs[:, 0]].astype(np.int64)
+            assert ((got.read_start > 0) | (got.read_end < n - 1)).any()
+    finally:
+        c.destroy()
+
+
+def test_int32_range_rule():
+    # beyond match*n + gap_extend*(n+2) + 2*gap_open + |mismatch| < 2^28 the int32 lane's minus infinity
+    # would no longer sit below every real cell value: such a pair is SDP_ERANGE (sdp.h), and a pair just inside the
+    # rule, at the largest scoring constants sdp_create accepts, is still exact.
+    rng = random.Random(64)
+
+    def rnd(k):
+        return "".join(rng.choice("ACGT") for _ in range(k))
+
+    sc = OracleScoring(4000, -4000, 4000, 4000, 0.6)
+    c = make_ctx(sc)
+    try:
+        T = rnd(4200)
+        placed = T[100:1600] + rnd(7) + T[1600:4100]             # 4,007 bases with one insertion
+        b = W.batch_from_strings([rnd(40), rnd(300), T], [rnd(30000), rnd(33000), placed])
+        parity.check_batch(c, b, sc, "inside the int32 range rule", host_path=False)
+        assert c.stats()["n_slow_words"] > 0
+        too_long = W.batch_from_strings([rnd(50), rnd(60)], [rnd(100), rnd(34000)])
+        with pytest.raises(SdpError) as e:
+            c.align_batch(c.upload(too_long))
+        assert e.value.code == -2
+        parity.check_batch(c, W.batch_from_strings([rnd(50)], [rnd(100)]), sc, "after SDP_ERANGE", host_path=False)
+    finally:
+        c.destroy()
+
+
 def test_errors(ctx):
     b = W.make_config(1, n_pairs=10, ref_bases=100_000)
     bad = W.Batch(b.reads_packed, b.read_off, b.read_len, b.wins_packed, b.win_off, b.win_len,
