@@ -174,8 +174,14 @@ def time_config(S, W, torch, dev, local, cfg, n_pairs, ref_bases, seed, steps, w
     """One BASELINE.json config at full size on this GPU: device-resident timing of the whole sdp_align_batch call
     (CUDA events on the launching stream, L2 flushed between steps), its own clocks sample, stage split."""
     batch = W.make_config(cfg, n_pairs=n_pairs, ref_bases=ref_bases if cfg != 1 else 1_000_000, seed=seed)
+    return time_batch(S, torch, dev, local, batch, W_NAME[cfg], steps, warmup, flush, peak)
+
+
+def time_batch(S, torch, dev, local, batch, workload, steps, warmup, flush, peak, local_mode=False):
+    """The same timing for any batch; local_mode = SDP_MODE_LOCAL (every pair then runs on the int32 lane)."""
     ctx = S.Context(device=local)
     try:
+        ctx.set_mode(local=local_mode)
         dbatch = ctx.upload(batch)
         stream = torch.cuda.current_stream(dev)
         ctx.set_timing(True)
@@ -200,12 +206,14 @@ def time_config(S, W, torch, dev, local, cfg, n_pairs, ref_bases, seed, steps, w
         clocks = sampler.stop(t0, time.time())
         mean = statistics.mean(ms)
         fwd_gcups = batch.cells / (statistics.mean(fwd) * 1e-3) / 1e9
-        return {"workload": W_NAME[cfg], "pairs": batch.n_pairs, "cells": batch.cells, "steps": steps, "warmup": warmup,
+        return {"workload": workload, "mode": "local" if local_mode else "semi-global",
+                "pairs": batch.n_pairs, "cells": batch.cells, "steps": steps, "warmup": warmup,
                 "ms_per_step": mean, "ms_best": min(ms), "ms_median": statistics.median(ms),
                 "gcups": batch.cells / (mean * 1e-3) / 1e9, "pairs_per_s": batch.n_pairs / (mean * 1e-3),
                 "stages_ms": {k: stats.get(k) for k in ("ms_total", "ms_bucket", "ms_forward", "ms_reverse", "ms_traceback",
                                                         "ms_compact")},
                 "kernel_launches_per_step": stats.get("kernel_launches"),
+                "pairs_on_int32_lane": bool(stats.get("n_slow_words")),
                 "forward_gcups": fwd_gcups, "forward_frac": fwd_gcups / peak,
                 "whole_path_frac": batch.cells / (mean * 1e-3) / 1e9 / peak, "clocks": clocks}
     finally:
@@ -510,6 +518,28 @@ def main():
             except Exception as ex:  # noqa: BLE001
                 per[f"cfg{c}"] = {"error": repr(ex)}
         out["per_config"] = per
+        # the lanes beside the int16 hot path, device-resident, same timing rules. `local`:
+        # SDP_MODE_LOCAL on config 2's shape and on long reads; `int32_lane`: the default mode on
+        # pairs outside the int16 kernels' domain (reads beyond SDP_MAX_READ_LEN), and for scale the
+        # int16 path on the 600 bp x 2,000 bp shape. forward_frac / whole_path_frac stay relative to the int16x2 DPX
+        # roofline of the headline, so that the distance of these lanes from the hot path is one number.
+        def lane_block(name, make, **kw):
+            try:
+                return time_batch(S, torch, dev, local, make(), name, steps=3, warmup=2, flush=flush, peak=peak, **kw)
+            except Exception as ex:  # noqa: BLE001
+                return {"error": repr(ex)}
+
+        out["local"] = {
+            "cfg2_shape": lane_block(W_NAME[2] + ", SDP_MODE_LOCAL",
+                                     lambda: W.make_config(2, ref_bases=args.ref_bases), local_mode=True),
+            "long_reads": lane_block("50,000 pairs 600bp x 2,000bp (config 2's recipe at long-read lengths), SDP_MODE_LOCAL",
+                                     lambda: W.make_long_reads(50_000, 600, 2000, ref_bases=args.ref_bases), local_mode=True)}
+        out["int32_lane"] = {
+            "reads_over_1024": lane_block("20,000 pairs 1,500bp x 3,000bp: reads beyond SDP_MAX_READ_LEN, one thread per "
+                                          "pair with row arrays in global memory (k_forward_i32)",
+                                          lambda: W.make_long_reads(20_000, 1500, 3000, ref_bases=args.ref_bases)),
+            "int16_path_600x2000_for_scale": lane_block("50,000 pairs 600bp x 2,000bp on the int16 path (inside the range rule)",
+                                                        lambda: W.make_long_reads(50_000, 600, 2000, ref_bases=args.ref_bases))}
         try:
             out["step3"] = time_step3(S, W, torch, dev, local, args.ref_bases, flush, peak)
         except Exception as ex:  # noqa: BLE001

@@ -58,26 +58,52 @@ def _units():
     return units
 
 
+SCORE_SENTINELS = ("negOc", "negO", "c2", "Cd", "e2")
+TRACE_SENTINELS = ("t_negOf", "t_negOe", "t_c8", "t_Cd8")
+
+
 def check_cubin_sentinels(path: str) -> dict:
     """Every sentinel must occur in the cubin, and only as the 32-bit immediate of an instruction: bytes 4..7 of a
-    16-byte slot of an executable section. Returns the hit counts. (Same walk as patch_score_image in score_modules.cu.)"""
+    16-byte slot of an executable section. Every kernel must use every sentinel of its family at least once (a score
+    kernel the five of score_kernel.cuh, a traceback DP kernel the four of trace_kernel.cuh): a kernel in which ptxas
+    derived a constant some other way would otherwise hide behind the hits of its neighbours in the same image.
+    Returns the hit counts per sentinel, which the build embeds next to the image and score_modules.cu compares with
+    what it patches at load time. (Same walk as patch_score_image in score_modules.cu.)"""
     import struct
     img = open(path, "rb").read()
     assert img[:4] == b"\x7fELF" and img[4] == 2 and img[5] == 1, f"{path}: not a little-endian ELF64"
     shoff, = struct.unpack_from("<Q", img, 0x28)
-    shentsize, shnum = struct.unpack_from("<HH", img, 0x3A)
+    shentsize, shnum, shstrndx = struct.unpack_from("<HHH", img, 0x3A)
     assert shentsize == 64
+    str_off, = struct.unpack_from("<Q", img, shoff + 64 * shstrndx + 0x18)
     hits = {k: 0 for k in SENTINELS}
     by_val = {v: k for k, v in SENTINELS.items()}
+    kernels = 0
     for s in range(shnum):
-        _, typ, flags, _, off, size = struct.unpack_from("<IIQQQQ", img, shoff + 64 * s)
+        name_off, typ, flags, _, off, size = struct.unpack_from("<IIQQQQ", img, shoff + 64 * s)
         if typ != 1 or not (flags & 4):
             continue
         assert off % 16 == 0
+        name = img[str_off + name_off:img.index(b"\0", str_off + name_off)].decode()
+        mine = {k: 0 for k in SENTINELS}
         for at in range(off, off + size - 15, 16):
             w, = struct.unpack_from("<I", img, at + 4)
             if w in by_val:
-                hits[by_val[w]] += 1
+                mine[by_val[w]] += 1
+        family = SCORE_SENTINELS if name.startswith(".text.sdp_score_k") else \
+            TRACE_SENTINELS if name.startswith(".text.sdp_trace_k") else None
+        if family is None:
+            if any(mine.values()):
+                raise RuntimeError(f"{path}: sentinel immediates in unexpected section {name}")
+            continue
+        kernels += 1
+        for k in SENTINELS:
+            if (mine[k] == 0) != (k not in family):
+                raise RuntimeError(f"{path}: kernel {name[6:]} uses sentinel {k} {mine[k]} times: each kernel must use "
+                                   "exactly the sentinels of its family, each at least once")
+            hits[k] += mine[k]
+    if kernels != 12:
+        raise RuntimeError(f"{path}: {kernels} score / traceback kernels found, 12 expected (2 K x 6 variants)")
     for name, v in SENTINELS.items():
         total = img.count(struct.pack("<I", v))
         if hits[name] == 0 or total != hits[name]:
@@ -112,12 +138,15 @@ def build(force: bool = False, verbose: bool = False, jobs: int | None = None) -
         if verbose:
             sys.stderr.write(r.stderr)
         if name.startswith("cubin_"):
-            check_cubin_sentinels(cubin)
-            sym = "sdp_" + name                       # sdp_cubin_r<r>_start / _end
+            hits = check_cubin_sentinels(cubin)
+            sym = "sdp_" + name                       # sdp_cubin_r<r>_start / _end / _hits
             asm = os.path.join(OBJ, name + ".S")
             with open(asm, "w") as f:
-                f.write(f'.section .rodata\n.balign 64\n.global {sym}_start\n.global {sym}_end\n{sym}_start:\n'
-                        f'.incbin "{cubin}"\n{sym}_end:\n.section .note.GNU-stack,"",@progbits\n')
+                # _hits: how often each sentinel occurs in this image, in SENTINELS order (= ScorePatch order)
+                f.write(f'.section .rodata\n.balign 64\n.global {sym}_start\n.global {sym}_end\n.global {sym}_hits\n'
+                        f'{sym}_start:\n.incbin "{cubin}"\n{sym}_end:\n.balign 4\n{sym}_hits:\n.long '
+                        + ", ".join(str(hits[k]) for k in SENTINELS)
+                        + '\n.section .note.GNU-stack,"",@progbits\n')
             r2 = subprocess.run(["gcc", "-c", "-fPIC", asm, "-o", obj], capture_output=True, text=True)
             if r2.returncode != 0:
                 raise RuntimeError(f"embedding {cubin} failed:\n{r2.stderr}")

@@ -14,7 +14,8 @@
 #include "sdp_host.cuh"
 #include "trace_kernel.cuh"
 
-#define SDP_UNIT_SYMS(r) extern "C" const unsigned char sdp_cubin_r##r##_start[], sdp_cubin_r##r##_end[];
+#define SDP_UNIT_SYMS(r) extern "C" const unsigned char sdp_cubin_r##r##_start[], sdp_cubin_r##r##_end[]; \
+    extern "C" const uint32_t sdp_cubin_r##r##_hits[];
 SDP_UNIT_SYMS(0) SDP_UNIT_SYMS(1) SDP_UNIT_SYMS(2) SDP_UNIT_SYMS(3) SDP_UNIT_SYMS(4) SDP_UNIT_SYMS(5) SDP_UNIT_SYMS(6)
 SDP_UNIT_SYMS(7) SDP_UNIT_SYMS(8) SDP_UNIT_SYMS(9) SDP_UNIT_SYMS(10) SDP_UNIT_SYMS(11) SDP_UNIT_SYMS(12)
 SDP_UNIT_SYMS(13) SDP_UNIT_SYMS(14) SDP_UNIT_SYMS(15)
@@ -24,8 +25,9 @@ namespace sdp {
 
 namespace {
 
-struct Image { const unsigned char* begin; const unsigned char* end; };
-#define SDP_UNIT_IMG(r) {sdp_cubin_r##r##_start, sdp_cubin_r##r##_end},
+// hits: occurrences of each sentinel (ScorePatch order) that build.py counted in the image it embedded
+struct Image { const unsigned char* begin; const unsigned char* end; const uint32_t* hits; };
+#define SDP_UNIT_IMG(r) {sdp_cubin_r##r##_start, sdp_cubin_r##r##_end, sdp_cubin_r##r##_hits},
 const Image kImages[SDP_SCORE_UNITS_N] = {SDP_UNIT_IMG(0) SDP_UNIT_IMG(1) SDP_UNIT_IMG(2) SDP_UNIT_IMG(3) SDP_UNIT_IMG(4)
                                           SDP_UNIT_IMG(5) SDP_UNIT_IMG(6) SDP_UNIT_IMG(7) SDP_UNIT_IMG(8) SDP_UNIT_IMG(9)
                                           SDP_UNIT_IMG(10) SDP_UNIT_IMG(11) SDP_UNIT_IMG(12) SDP_UNIT_IMG(13)
@@ -88,8 +90,13 @@ static int load_unit(ScoreModules* m, const ScorePatch& pv, int r, char* err, si
         free(img); snprintf(err, errlen, "score kernel image %d is not a cubin", r); return SDP_ECUDA;
     }
     for (int k = 0; k < SDP_N_SENTINELS; ++k)
-        if (hits[k] == 0) {      // every kernel uses every constant: a missing sentinel means the build changed under us
-            free(img); snprintf(err, errlen, "score kernel image %d: sentinel %d not found", r, k); return SDP_ECUDA;
+        if (hits[k] == 0 || hits[k] != kImages[r].hits[k]) {
+            // the build counted every use of every sentinel in this very image: any other count means the image and
+            // its table do not belong together, or the patch walk and the build's walk disagree
+            free(img);
+            snprintf(err, errlen, "score kernel image %d: sentinel %d patched %u times, the build counted %u", r, k,
+                     hits[k], kImages[r].hits[k]);
+            return SDP_ECUDA;
         }
     const cudaError_t e = cudaLibraryLoadData(&m->lib[r], img, nullptr, nullptr, 0, nullptr, nullptr, 0);
     free(img);

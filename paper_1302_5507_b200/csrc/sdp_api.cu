@@ -840,16 +840,25 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         const int rc = lanes_init(ctx, NL);
         if (rc != SDP_OK) return rc;
     }
-    CU(cudaEventRecord(ctx->ev_start, st));
-    CU(cudaStreamWaitEvent(ctx->fwd_stream, ctx->ev_start, 0));
+    // from here on work is in flight on the ctx's streams: every failure leaves through bail(), which waits for all of
+    // it, so that a later call (or a reallocation's cudaFree) never meets leftover kernels
+    auto bail = [&](int rc) { drain(ctx); return rc; };
+#define CUB(call)                                                                                        \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return bail(fail(ctx, e_ == cudaErrorMemoryAllocation ? SDP_ENOMEM : SDP_ECUDA,              \
+                             "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__));      \
+    } while (0)
+    CUB(cudaEventRecord(ctx->ev_start, st));
+    CUB(cudaStreamWaitEvent(ctx->fwd_stream, ctx->ev_start, 0));
     for (int li = 0; li < NL; ++li) {
         Lane& L = ctx->lane[li];
         L.p0 = P * (uint64_t)li / (uint64_t)NL;
         L.P = P * (uint64_t)(li + 1) / (uint64_t)NL - L.p0;
         L.b = b; L.b.pairs = b.pairs + 2 * L.p0; L.b.n_pairs = L.P;
-        CU(cudaStreamWaitEvent(L.st, ctx->ev_start, 0));
+        CUB(cudaStreamWaitEvent(L.st, ctx->ev_start, 0));
     }
-    auto bail = [&](int rc) { drain(ctx); return rc; };
 
     for (int li = 0; li < NL; ++li) {
         const int rc = lane_phase_a(ctx, ctx->lane[li], local);
@@ -857,11 +866,12 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
     }
     for (int li = 0; li < NL; ++li) {
         Lane& L = ctx->lane[li];
-        CU(cudaEventSynchronize(L.evA));
+        CUB(cudaEventSynchronize(L.evA));
         if (L.mb->err_flag & SDP_ERRF_INDEX)
             return bail(fail(ctx, SDP_EINVAL, "pair index, offset or length out of range (or empty sequence)"));
         if (L.mb->err_flag & SDP_ERRF_RANGE)
-            return bail(fail(ctx, SDP_ERANGE, "a sequence is longer than SDP_MAX_SEQ_LEN (see sdp.h)"));
+            return bail(fail(ctx, SDP_ERANGE, "a sequence is longer than SDP_MAX_SEQ_LEN, or a pair is outside the int32 "
+                             "range rule (see sdp.h)"));
     }
     for (int li = 0; li < NL; ++li) {
         const int rc = lane_phase_b(ctx, ctx->lane[li], local);
@@ -872,7 +882,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         uint64_t ops_capacity = 0;
         for (int li = 0; li < NL; ++li) {
             Lane& L = ctx->lane[li];
-            CU(cudaEventSynchronize(L.evB));
+            CUB(cudaEventSynchronize(L.evB));
             ops_capacity += L.mb->totals[1];
             const int rc = lane_phase_c(ctx, L, local);
             if (rc != SDP_OK) return bail(rc);
@@ -885,15 +895,15 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
             const int rc = lane_phase_d(ctx, ctx->lane[li], li);
             if (rc != SDP_OK) return bail(rc);
         }
-        for (int li = 0; li < NL; ++li) CU(cudaStreamWaitEvent(st, ctx->lane[li].evD, 0));
+        for (int li = 0; li < NL; ++li) CUB(cudaStreamWaitEvent(st, ctx->lane[li].evD, 0));
     } else {
         const int rc = ensure(ctx, ctx->cigar_ops, 16);
         if (rc != SDP_OK) return bail(rc);
-        for (int li = 0; li < NL; ++li) CU(cudaStreamWaitEvent(st, ctx->lane[li].evB, 0));
+        for (int li = 0; li < NL; ++li) CUB(cudaStreamWaitEvent(st, ctx->lane[li].evB, 0));
     }
-    CU(cudaEventRecord(ctx->ev_end, st));
-    CU(cudaStreamSynchronize(st));
-    CU(cudaGetLastError());
+    CUB(cudaEventRecord(ctx->ev_end, st));
+    CUB(cudaStreamSynchronize(st));
+    CUB(cudaGetLastError());
     uint32_t errf = 0;
     for (int li = 0; li < NL; ++li) errf |= ctx->lane[li].mb->err_flag;
     if (!ctx->score_only) {
@@ -905,6 +915,7 @@ int sdp_align_batch(sdp_ctx* ctx, const sdp_batch* batch, void* cuda_stream, sdp
         n_ops = ctx->lane[NL - 1].mb->totals[2];
     }
 
+#undef CUB
     if (ctx->timing) cudaEventElapsedTime(&stats.ms_total, ctx->ev_start, ctx->ev_end);
     for (int li = 0; li < NL; ++li) {
         Lane& L = ctx->lane[li];

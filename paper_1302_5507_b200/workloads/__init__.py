@@ -236,7 +236,6 @@ def reference(ref_bases: int, seed: int, with_n: bool):
 def make_config(cfg: int, n_pairs: Optional[int] = None, ref_bases: Optional[int] = None,
                 seed: Optional[int] = None) -> Batch:
     """One of the five BASELINE.json workloads; ``n_pairs`` / ``ref_bases`` shrink it for tests."""
-    lib = _load()
     full = _FULL[cfg]
     n_pairs = full["n_pairs"] if n_pairs is None else int(n_pairs)
     ref_bases = full["ref_bases"] if ref_bases is None else int(ref_bases)
@@ -245,6 +244,30 @@ def make_config(cfg: int, n_pairs: Optional[int] = None, ref_bases: Optional[int
     ref_seed = SEED_BASE + (1 if cfg == 1 else 2)
     ref_packed, ref_nmask = reference(ref_bases, ref_seed, with_n=(cfg == 5))
     P = _params(cfg, n_pairs, ref_bases, seed)
+    return _generate(P, ref_packed, ref_nmask, name=f"cfg{cfg}",
+                     meta=dict(cfg=cfg, n_pairs=n_pairs, ref_bases=ref_bases, seed=seed))
+
+
+def make_long_reads(n_pairs: int, read_len: int, win_len: int, ref_bases: Optional[int] = None,
+                    seed: Optional[int] = None) -> Batch:
+    """Config 2's recipe (mate-rescue shape: 5 % unrelated reads, 1 % substitutions, indels at 0.2 % per base, true
+    start normal around the window's middle) at another read and window length: the long-read case of PAPER.md:117
+    ("read length is not capped"). Windows are views into the shared seeded reference."""
+    ref_bases = _FULL[2]["ref_bases"] if ref_bases is None else int(ref_bases)
+    seed = SEED_BASE + 900 + read_len if seed is None else int(seed)
+    ref_packed, ref_nmask = reference(ref_bases, SEED_BASE + 2, with_n=False)
+    P = _params(2, int(n_pairs), ref_bases, seed)
+    P.read_len_min = P.read_len_max = int(read_len)
+    P.win_len = int(win_len)
+    P.start_center, P.start_sd = max(0, (int(win_len) - int(read_len)) // 2), max(1.0, (win_len - read_len) / 8.0)
+    return _generate(P, ref_packed, ref_nmask, name=f"long{read_len}x{win_len}",
+                     meta=dict(n_pairs=int(n_pairs), read_len=int(read_len), win_len=int(win_len), ref_bases=ref_bases,
+                               seed=seed))
+
+
+def _generate(P: _Params, ref_packed, ref_nmask, name: str, meta: dict) -> Batch:
+    lib = _load()
+    n_pairs = int(P.n_pairs)
     read_len = np.zeros(n_pairs, dtype=np.uint32)
     read_off = np.zeros(n_pairs, dtype=np.uint64)
     win_len = np.zeros(n_pairs, dtype=np.uint32)
@@ -265,8 +288,7 @@ def make_config(cfg: int, n_pairs: Optional[int] = None, ref_bases: Optional[int
     pairs = np.ascontiguousarray(np.stack([idx, idx], axis=1))
     return Batch(reads_packed, read_off, read_len,
                  wins_out if P.private_windows else ref_packed, win_off, win_len, pairs,
-                 None, None if P.private_windows else ref_nmask,
-                 name=f"cfg{cfg}", meta=dict(cfg=cfg, n_pairs=n_pairs, ref_bases=ref_bases, seed=seed))
+                 None, None if P.private_windows else ref_nmask, name=name, meta=meta)
 
 
 def make_step3(n_reads: int, max_candidates: int = 30, ref_bases: Optional[int] = None,
