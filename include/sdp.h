@@ -239,7 +239,7 @@ const char* sdp_static_last_error(void);
  * CIGAR as soft clips (BAM op 4), n_cols counts aligned columns only, and the filter counts clipped bases as columns
  * that do not match: pass iff n_cols > 0 and n_match * 1e6 >= q * (n_cols + clipped). A pair without any positive-
  * scoring alignment reports score 0, ref_start 0, ref_end -1, read_start 0, read_end -1, CIGAR <n>S, pass 0.
- * Local mode runs on the int32 lane (exact; one warp per pair, about one fifteenth of the default mode's throughput).
+ * Local mode runs on the int32 lane (exact; one warp per pair, about one tenth of the default mode's throughput).
  * SDP_EINVAL for an unknown mode.
  */
 #define SDP_MODE_SEMIGLOBAL 0
