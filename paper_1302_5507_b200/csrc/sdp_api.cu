@@ -1061,16 +1061,26 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
         {&ctx->in_wins, hb->wins_packed, wb, (const void**)&d.wins_packed},
         {&ctx->in_win_nmask, hb->win_nmask, wnb, (const void**)&d.win_nmask},
     };
+    // uploads and downloads are in flight from here on: a failure waits for them (and for whatever the pipeline left
+    // behind) before it returns, so that the caller may free its buffers and a later call finds the streams idle
+    auto hbail = [&](int rc_) { cudaStreamSynchronize(st); cudaStreamSynchronize(ctx->copy_stream); drain(ctx); return rc_; };
+#define CUH(call)                                                                                        \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return hbail(fail(ctx, e_ == cudaErrorMemoryAllocation ? SDP_ENOMEM : SDP_ECUDA,             \
+                              "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__));     \
+    } while (0)
     int ci = 0;
     for (Cp& c : cps) {
         const cudaStream_t cs = ci++ < 5 ? st : ctx->copy_stream;
         if (!c.src) { *c.dst = nullptr; continue; }
         int rc = ensure(ctx, *c.buf, c.bytes + 64);
-        if (rc != SDP_OK) return rc;
-        if (c.bytes) CU(cudaMemcpyAsync(c.buf->p, c.src, c.bytes, cudaMemcpyHostToDevice, cs));
+        if (rc != SDP_OK) return hbail(rc);
+        if (c.bytes) CUH(cudaMemcpyAsync(c.buf->p, c.src, c.bytes, cudaMemcpyHostToDevice, cs));
         *c.dst = c.buf->p;
     }
-    CU(cudaEventRecord(ctx->ev_seq_ready, ctx->copy_stream));
+    CUH(cudaEventRecord(ctx->ev_seq_ready, ctx->copy_stream));
     // per-pair results go into one pinned slab (sized before the call: score and ref_end leave early), the runs into another
     const size_t Pp = (size_t)(P ? P : 1);
     size_t off = 0;
@@ -1079,31 +1089,32 @@ int sdp_align_batch_host(sdp_ctx* ctx, const sdp_batch* hb, sdp_result* out)
                  o_qe = carve(Pp * 4), o_pass = carve(Pp), o_nm = carve(Pp * 4), o_nc = carve(Pp * 4),
                  o_coff = carve(Pp * 8), o_clen = carve(Pp * 4);
     int rc = ensure_pinned(ctx, ctx->h_out, off);
-    if (rc != SDP_OK) return rc;
+    if (rc != SDP_OK) return hbail(rc);
     char* h = (char*)ctx->h_out.p;
     sdp_result dr{};
     ctx->wait_seq = true;
     ctx->h_early_score = (int32_t*)(h + o_score); ctx->h_early_ref_end = (int32_t*)(h + o_re);
     rc = sdp_align_batch(ctx, &d, st, &dr);
     ctx->wait_seq = false; ctx->h_early_score = nullptr; ctx->h_early_ref_end = nullptr;
-    if (rc != SDP_OK) { cudaStreamSynchronize(ctx->copy_stream); return rc; }
+    if (rc != SDP_OK) return hbail(rc);
     const size_t n_ops = (size_t)dr.n_cigar_ops;
     rc = ensure_pinned(ctx, ctx->h_ops, (n_ops + 1) * 4);
-    if (rc != SDP_OK) { cudaStreamSynchronize(ctx->copy_stream); return rc; }
+    if (rc != SDP_OK) return hbail(rc);
     char* hops = (char*)ctx->h_ops.p;
     if (P) {
-        CU(cudaMemcpyAsync(h + o_rs, dr.ref_start, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_qs, dr.read_start, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_qe, dr.read_end, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_pass, dr.pass, P, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_nm, dr.n_match, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_nc, dr.n_cols, P * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_coff, dr.cigar_off, P * 8, cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h + o_clen, dr.cigar_len, P * 4, cudaMemcpyDeviceToHost, st));
-        if (n_ops) CU(cudaMemcpyAsync(hops, dr.cigar_ops, n_ops * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        CUH(cudaMemcpyAsync(h + o_rs, dr.ref_start, P * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_qs, dr.read_start, P * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_qe, dr.read_end, P * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_pass, dr.pass, P, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_nm, dr.n_match, P * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_nc, dr.n_cols, P * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_coff, dr.cigar_off, P * 8, cudaMemcpyDeviceToHost, st));
+        CUH(cudaMemcpyAsync(h + o_clen, dr.cigar_len, P * 4, cudaMemcpyDeviceToHost, st));
+        if (n_ops) CUH(cudaMemcpyAsync(hops, dr.cigar_ops, n_ops * 4, cudaMemcpyDeviceToHost, st));
+        CUH(cudaStreamSynchronize(st));
     }
-    CU(cudaStreamSynchronize(ctx->copy_stream));
+    CUH(cudaStreamSynchronize(ctx->copy_stream));
+#undef CUH
     out->score = (const int32_t*)(h + o_score); out->ref_start = (const int32_t*)(h + o_rs);
     out->ref_end = (const int32_t*)(h + o_re); out->read_start = (const int32_t*)(h + o_qs);
     out->read_end = (const int32_t*)(h + o_qe); out->pass = (const uint8_t*)(h + o_pass);

@@ -56,6 +56,19 @@ def test_step3_workload_shape():
     assert int(b.win_off.max()) + int(b.win_len[0]) <= b.wins_packed.shape[0] * 16
 
 
+def test_long_read_workload_shape():
+    # bench.py's local / int32_lane blocks: config 2's recipe at other lengths, seeded and reproducible
+    a = W.make_long_reads(40, 600, 2000, ref_bases=400_000)
+    b = W.make_long_reads(40, 600, 2000, ref_bases=400_000)
+    assert a.n_pairs == 40 and (a.read_len == 600).all() and (a.win_len == 2000).all() and a.cells == 40 * 600 * 2000
+    assert np.array_equal(a.reads_packed, b.reads_packed) and np.array_equal(a.win_off, b.win_off)
+    assert int(a.win_off.max()) + 2000 <= a.wins_packed.shape[0] * 16
+    r = oracle.align_batch(a.reads_packed, a.read_off, a.read_len, a.wins_packed, a.win_off, a.win_len, a.pairs,
+                           OracleScoring(), threads=2)
+    # most reads are cut from their window with about 1 % substitutions: they score near their length
+    assert (r.score > 480).mean() > 0.8 and (r.score < 0).sum() <= 8
+
+
 @pytest.mark.gpu
 def test_gpu_step3_alignment_and_choice():
     import parity
