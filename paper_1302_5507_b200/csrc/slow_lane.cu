@@ -10,6 +10,7 @@
 // Local variant (R18; the paper names Smith-Waterman, and soft-clipped alignments,
 // PAPER.md:228): M(i,0) = M(0,j) = 0, M(i,j) = max(0, ...), S = max over all cells, lowest row then lowest column.
 #include "sdp_host.cuh"
+#include "score_kernel.cuh"      // the fp16-pipe delta helpers (hsub2_u, hfma2_relu_negsq, read_code_half, prmt_raw)
 
 namespace sdp {
 
@@ -140,6 +141,172 @@ __device__ __forceinline__ void forward_i32_warp(const sdp_batch& b, const Scori
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Local mode, int16x2: one warp scores TWO pairs (pair 2w in the low halves, pair 2w + 1 in the high halves) with the DPX
+// max/add instructions, for reads up to 256 bases inside the value rule below. Same recurrences, same results as the
+// int32 kernels (every quantity is exact in 16 bits under the rule); about 2.5 times their throughput.
+//
+// Per cell of two pairs, six ALU-pipe instructions. With beta = |mismatch|, every H carries +beta (the zero floor is the
+// constant beta), D carries + e*i and I + e*(column within the lane), so that extending a gap needs no add:
+//     D~ = max(S(i-1,j) + (e*i - oe - mismatch), D~(i-1,j))        S = H + beta + mismatch, the stored row
+//     I~ = max(H^(i,j-1) + (e*jr - oe), I~(i,j-1))
+//     a  = max(D~ - e*i, beta)         b = max(I~ - e*jr, a)         H^ = max(S(i-1,j-1) + q, b)
+//     best = max(best, H^)
+// q = match - mismatch or 0 comes from the FMA pipe (score_kernel.cuh: HADD2 + HFMA2.RELU on fp16 base codes), and so
+// does S = H^ - beta as one 32-bit integer subtraction (no borrow between the halves: H^ >= beta in both).
+// The position of the best cell is resolved once per row and lane, only when the row raised the lane's best: the row's
+// values are still in S[]. Cells of padded read columns (a shorter partner, columns past n) and padded window rows hold
+// N codes, which match nothing: such a cell never exceeds its real ancestors, all of which have a lower row or column,
+// so it can tie but never win under the rule "highest score, then lowest row, then lowest column".
+__device__ __forceinline__ uint32_t pack2(int v) { return ((uint32_t)v & 0xFFFFu) * 0x00010001u; }
+
+// value rule of the int16x2 local kernel: largest stored magnitude match*n + beta + e*rows, and -(oe + e*rows) below
+__device__ __forceinline__ bool local_i16_rule(const Scoring& sc, int n, int m) {
+    const long long oe = (long long)sc.gap_open + sc.gap_extend;
+    return n <= 256 && sc.match - sc.mismatch < 0x3C00 &&
+           (long long)sc.match * n + (long long)sc.gap_extend * (m + 48) + 2 * oe - 2LL * sc.mismatch <= 32000;
+}
+// Does the int16x2 kernel score pair p (local mode)? Pairs 2w and 2w + 1 share a warp there when both reads fit and
+// the rule holds for the larger of their lengths; a pair whose partner is absent or too long runs alone. Evaluated the
+// same way by k_forward_local_i16 and by the int32 kernels, which skip what it takes.
+__device__ __forceinline__ bool local_i16_taken(const sdp_batch& b, const Scoring& sc, uint64_t p, uint64_t n_pairs,
+                                                const uint32_t* __restrict__ slow_words)
+{
+    const int n = (int)b.read_len[b.pairs[2 * p]], m = (int)b.win_len[b.pairs[2 * p + 1]];
+    if (n > 256) return false;
+    const uint64_t q = p ^ 1ull;
+    if (q < n_pairs && slow_words[q] != 0) {
+        const int nq = (int)b.read_len[b.pairs[2 * q]], mq = (int)b.win_len[b.pairs[2 * q + 1]];
+        if (nq <= 256) return local_i16_rule(sc, max(n, nq), max(m, mq));
+    }
+    return local_i16_rule(sc, n, m);
+}
+
+template <int KC>
+__device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, const Scoring& sc, const uint64_t pA,
+                                                         const uint64_t pB, const bool hasB, int32_t* __restrict__ score,
+                                                         int32_t* __restrict__ ref_end, int32_t* __restrict__ end_col)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t riA = b.pairs[2 * pA], wiA = b.pairs[2 * pA + 1];
+    const int nA = (int)b.read_len[riA], mA = (int)b.win_len[wiA];
+    const uint64_t roffA = b.read_off[riA], woffA = b.win_off[wiA];
+    int nB = 0, mB = 0;
+    uint64_t roffB = 0, woffB = 0;
+    if (hasB) {
+        const uint32_t riB = b.pairs[2 * pB], wiB = b.pairs[2 * pB + 1];
+        nB = (int)b.read_len[riB]; mB = (int)b.win_len[wiB];
+        roffB = b.read_off[riB]; woffB = b.win_off[wiB];
+    }
+    const int e = sc.gap_extend, oe = sc.gap_open + sc.gap_extend, beta = -sc.mismatch;
+    const int mmax = max(mA, mB);
+    const int j0 = lane * KC;                              // this lane owns columns j0 + 1 .. j0 + KC of both pairs
+    uint32_t S[KC], Dt[KC], rh[KC], ck[KC], negek[KC];
+#pragma unroll
+    for (int k = 0; k < KC; ++k) {
+        const int j = j0 + k + 1;
+        const uint32_t cA = j <= nA ? code_at(b.reads_packed, b.read_nmask, roffA + (uint64_t)(j - 1), SDP_CODE_READ_N) : SDP_CODE_READ_N;
+        const uint32_t cB = j <= nB ? code_at(b.reads_packed, b.read_nmask, roffB + (uint64_t)(j - 1), SDP_CODE_READ_N) : SDP_CODE_READ_N;
+        rh[k] = read_code_half(cA) | (read_code_half(cB) << 16);
+        S[k] = 0u;                                         // M(0,j) = 0: S = 0 + beta + mismatch
+        Dt[k] = pack2(beta - oe);                          // D(0,j): anything <= -oe + e acts as minus infinity under the zero floor
+        ck[k] = pack2(e * (k + 1) - oe);
+        negek[k] = pack2(-e * (k + 1));
+    }
+    const uint32_t BETA2 = pack2(beta), E2 = pack2(e), NEGE2 = pack2(-e), NEG2 = 0x80008000u, NEGEK2 = pack2(-e * KC);
+    const uint32_t MISABS2 = (uint32_t)beta * 0x00010001u, Cd = pack2(sc.match - sc.mismatch);
+    const uint32_t EDGE_I = pack2(beta - oe);              // I(i,0), in the frame of column 0
+    uint32_t ci = pack2(-e * lane - oe - sc.mismatch);     // e*i - oe - mismatch for the row before this lane's first step
+    uint32_t negei = pack2(e * lane);
+    uint32_t best = BETA2;
+    int biA = 0, bjA = 0, biB = 0, bjB = 0;
+    uint32_t h_out = BETA2, i_out = EDGE_I, sel_out = 0u;
+    uint32_t diag = 0u;                                    // S(i-1, j0); row 0 is all zeros
+    uint32_t wsel = 0u;
+    const int steps = mmax + 31;
+    for (int s = 1; s <= steps; ++s) {
+        if (((s - 1) & 31) == 0) {                         // window codes of rows s .. s + 31, one row per lane, as PRMT selectors
+            const int r = s + lane;
+            const uint32_t cA = r <= mA ? code_at(b.wins_packed, b.win_nmask, woffA + (uint64_t)(r - 1), SDP_CODE_WIN_N) : SDP_CODE_WIN_N;
+            const uint32_t cB = r <= mB ? code_at(b.wins_packed, b.win_nmask, woffB + (uint64_t)(r - 1), SDP_CODE_WIN_N) : SDP_CODE_WIN_N;
+            wsel = cA * 0x11u | cB * 0x1100u;
+        }
+        const uint32_t sel0 = __shfl_sync(0xffffffffu, wsel, (s - 1) & 31);
+        uint32_t left = __shfl_up_sync(0xffffffffu, h_out, 1);
+        uint32_t ileft = __shfl_up_sync(0xffffffffu, i_out, 1);
+        uint32_t sel = __shfl_up_sync(0xffffffffu, sel_out, 1);
+        ci = __viaddmax_s16x2(ci, E2, NEG2);               // packed add (max with the most negative value)
+        negei = __viaddmax_s16x2(negei, NEGE2, NEG2);
+        const int i = s - lane;
+        if (lane == 0) { left = BETA2; ileft = EDGE_I; sel = sel0; }      // M(i,0) = 0, I(i,0) = -inf
+        else ileft = __viaddmax_s16x2(ileft, NEGEK2, NEG2);               // from the left lane's column frame into this one
+        if (i >= 1 && i <= mmax) {
+            const uint32_t left_in = left, bprev = best;
+            const uint32_t nt = prmt_raw(SDP_TBL_LO, SDP_TBL_HI, sel);
+#pragma unroll
+            for (int k = 0; k < KC; ++k) {
+                const uint32_t up = S[k];
+                const uint32_t dt = __viaddmax_s16x2(up, ci, Dt[k]);
+                const uint32_t it = __viaddmax_s16x2(left, ck[k], ileft);
+                const uint32_t q = hfma2_relu_negsq(hsub2_u(nt, rh[k]), Cd);
+                const uint32_t a = __viaddmax_s16x2(dt, negei, BETA2);
+                const uint32_t bb = __viaddmax_s16x2(it, negek[k], a);
+                const uint32_t h = __viaddmax_s16x2(diag, q, bb);
+                diag = up;
+                S[k] = h - MISABS2;
+                Dt[k] = dt; left = h; ileft = it;
+                best = __vmaxs2(best, h);
+            }
+            if (best != bprev) {                           // this row raised the lane's best in one half or both
+                const uint32_t target = best - MISABS2;
+                if ((best ^ bprev) & 0xFFFFu) {
+                    biA = i;
+#pragma unroll
+                    for (int k = KC - 1; k >= 0; --k) if (((S[k] ^ target) & 0xFFFFu) == 0u) bjA = j0 + k + 1;
+                }
+                if ((best ^ bprev) >> 16) {
+                    biB = i;
+#pragma unroll
+                    for (int k = KC - 1; k >= 0; --k) if (((S[k] ^ target) >> 16) == 0u) bjB = j0 + k + 1;
+                }
+            }
+            diag = left_in - MISABS2;                      // S(i, j0): the next row's diagonal neighbour
+        }
+        h_out = left; i_out = ileft; sel_out = sel;
+    }
+    int bA = (int)(int16_t)(best & 0xFFFFu) - beta, bB = (int)(int16_t)(best >> 16) - beta;
+    // over the lanes, per pair: highest score, then lowest row, then lowest column
+    for (int o = 16; o > 0; o >>= 1) {
+        int ob = __shfl_down_sync(0xffffffffu, bA, o), oi = __shfl_down_sync(0xffffffffu, biA, o), oj = __shfl_down_sync(0xffffffffu, bjA, o);
+        if (ob > bA || (ob == bA && (oi < biA || (oi == biA && oj < bjA)))) { bA = ob; biA = oi; bjA = oj; }
+        ob = __shfl_down_sync(0xffffffffu, bB, o); oi = __shfl_down_sync(0xffffffffu, biB, o); oj = __shfl_down_sync(0xffffffffu, bjB, o);
+        if (ob > bB || (ob == bB && (oi < biB || (oi == biB && oj < bjB)))) { bB = ob; biB = oi; bjB = oj; }
+    }
+    if (lane == 0) {
+        score[pA] = bA; ref_end[pA] = biA - 1; end_col[pA] = bjA;          // S == 0: row 0, column 0 -> ref_end -1
+        if (hasB) { score[pB] = bB; ref_end[pB] = biB - 1; end_col[pB] = bjB; }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_forward_local_i16(const sdp_batch b, const Scoring sc, uint64_t n_pairs,
+                                                           const uint32_t* __restrict__ slow_words,
+                                                           int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
+                                                           int32_t* __restrict__ end_col)
+{
+    const uint64_t p0 = (((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 2ull;
+    if (p0 >= n_pairs) return;                             // warp-uniform, like everything below
+    const bool inA = slow_words[p0] != 0, inB = p0 + 1 < n_pairs && slow_words[p0 + 1] != 0;
+    const bool runA = inA && local_i16_taken(b, sc, p0, n_pairs, slow_words);
+    const bool runB = inB && local_i16_taken(b, sc, p0 + 1, n_pairs, slow_words);
+    if (!runA && !runB) return;
+    const uint64_t pA = runA ? p0 : p0 + 1;
+    const bool hasB = runA && runB;
+    int nmax = (int)b.read_len[b.pairs[2 * pA]];
+    if (hasB) nmax = max(nmax, (int)b.read_len[b.pairs[2 * (p0 + 1)]]);
+    if (nmax <= 128) forward_local_i16x2_warp<4>(b, sc, pA, p0 + 1, hasB, score, ref_end, end_col);
+    else             forward_local_i16x2_warp<8>(b, sc, pA, p0 + 1, hasB, score, ref_end, end_col);
+}
+
 // LARGE = false: reads up to 256 bases (4 or 8 columns per lane); true: up to 1,024 (16 or 32). Two kernels because
 // their register budgets differ by a factor of three.
 template <bool LARGE>
@@ -157,6 +324,7 @@ __global__ void __launch_bounds__(256) k_forward_i32_warp(const sdp_batch b, con
         else          forward_i32_warp<32>(b, sc, local, p, score, ref_end, end_col);
     } else {
         if (n > 256) return;
+        if (local && local_i16_taken(b, sc, p, n_pairs, slow_words)) return;      // k_forward_local_i16 scores it
         if (n <= 128) forward_i32_warp<4>(b, sc, local, p, score, ref_end, end_col);
         else          forward_i32_warp<8>(b, sc, local, p, score, ref_end, end_col);
     }
@@ -167,6 +335,9 @@ void launch_forward_i32(const sdp_batch& b, const Scoring& sc, int local, const 
 {
     if (b.n_pairs) {
         const uint32_t wgrid = (uint32_t)((b.n_pairs * 32 + 255) / 256);
+        if (local)      // two pairs per warp on the int16x2 DPX instructions, where the reads and the values fit
+            k_forward_local_i16<<<(uint32_t)(((b.n_pairs + 1) / 2 * 32 + 255) / 256), 256, 0, st>>>(b, sc, b.n_pairs, slow_words, score,
+                                                                                                  ref_end, end_col);
         k_forward_i32_warp<false><<<wgrid, 256, 0, st>>>(b, sc, local, b.n_pairs, slow_words, score, ref_end, end_col);
         k_forward_i32_warp<true><<<wgrid, 256, 0, st>>>(b, sc, local, b.n_pairs, slow_words, score, ref_end, end_col);
         k_forward_i32<<<(uint32_t)((b.n_pairs + 63) / 64), 64, 0, st>>>(b, sc, local, b.n_pairs, slow_words, slow_off, rows, score,

@@ -487,6 +487,40 @@ def test_int32_lane_reads_257_to_1024(route):
         c.destroy()
 
 
+@pytest.mark.parametrize("sc", [DEFAULT, OracleScoring(2, 0, 3, 1, 0.5), OracleScoring(60, -60, 100, 40, 0.6),
+                                OracleScoring(1, -1, 0, 1, 0.6), OracleScoring(120, -7, 30, 9, 0.6)],
+                         ids=lambda s: f"{s.match}_{s.mismatch}_{s.gap_open}_{s.gap_extend}")
+def test_local_mode_int16_pairing(sc):
+    # The int16x2 local kernel (slow_lane.cu) scores pairs 2w and 2w+1 in one warp when both reads have at most 256
+    # bases and the value rule holds for the larger of their lengths; everything else stays on the int32 kernels. Mixed
+    # neighbours: every read length class next to every other, windows from 1 base to lengths that break the rule for
+    # the larger scorings, an odd pair count, mismatch = 0 (a padded cell can then tie with a real one: it must lose).
+    rng = random.Random(65)
+
+    def rnd(k, alpha="ACGT"):
+        return "".join(rng.choice(alpha) for _ in range(k))
+
+    wins, reads = [], []
+    for _ in range(301):
+        n = rng.choice([1, 2, 7, 31, 64, 100, 127, 128, 129, 200, 255, 256, 257, 300, 520])
+        m = rng.choice([1, 3, 40, 150, 300, 301, 640, 900, 2500])
+        alpha = rng.choice(["ACGT", "ACGT", "AC", "ACGTN"])
+        T = rnd(m, alpha)
+        if rng.random() < 0.7 and m > 4:                         # a read that shares a stretch with its window
+            a = rng.randrange(0, m - 1)
+            core = T[a:a + n]
+            R = (rnd(rng.randint(0, 6), alpha) + core + rnd(n, alpha))[:n]
+        else:
+            R = rnd(n, alpha)
+        wins.append(T); reads.append(R)
+    c = make_ctx(sc)
+    try:
+        c.set_mode(local=True)
+        parity.check_batch(c, W.batch_from_strings(wins, reads), sc, f"local int16 pairing {sc}", local=True)
+    finally:
+        c.destroy()
+
+
 def test_int32_range_rule():
     # beyond match*n + gap_extend*(n+2) + 2*gap_open + |mismatch| < 2^28 the int32 lane's minus infinity
     # would no longer sit below every real cell value: such a pair is SDP_ERANGE (sdp.h), and a pair just inside the
