@@ -612,7 +612,7 @@ int lane_phase_b(sdp_ctx* ctx, Lane& L, const int local)
         launch_forward_i32(b, ctx->sc, local, L.slow_words.as<uint32_t>(), L.slow_off.as<uint64_t>(),
                            L.slow_rows.as<int32_t>(), ctx->score.as<int32_t>() + L.p0, ctx->ref_end.as<int32_t>() + L.p0,
                            L.rev_rows.as<int32_t>(), fs);
-        L.nl += local ? 4 : 3;
+        L.nl += local ? 5 : 3;
     }
     if (ctx->timing) CU(cudaEventRecord(L.tev[LEV_F1], fs));
     CU(cudaEventRecord(L.ev_fwd, fs));

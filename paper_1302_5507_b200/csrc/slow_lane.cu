@@ -182,25 +182,32 @@ __device__ __forceinline__ bool local_i16_taken(const sdp_batch& b, const Scorin
     return local_i16_rule(sc, n, m);
 }
 
-template <int KC>
+// LANES = 32: the warp is one group (reads up to 256 bases); LANES = 16: two groups of 16 lanes, each with its own two
+// pairs (reads up to 128 bases): the per-row work that does not depend on the column count (shuffles, row constants,
+// selector expansion, best-cell bookkeeping) is then shared by four pairs instead of two.
+template <int KC, int LANES>
 __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, const Scoring& sc, const uint64_t pA,
-                                                         const uint64_t pB, const bool hasB, int32_t* __restrict__ score,
-                                                         int32_t* __restrict__ ref_end, int32_t* __restrict__ end_col)
+                                                         const uint64_t pB, const bool hasA, const bool hasB,
+                                                         int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
+                                                         int32_t* __restrict__ end_col)
 {
-    const int lane = threadIdx.x & 31;
-    const uint32_t riA = b.pairs[2 * pA], wiA = b.pairs[2 * pA + 1];
-    const int nA = (int)b.read_len[riA], mA = (int)b.win_len[wiA];
-    const uint64_t roffA = b.read_off[riA], woffA = b.win_off[wiA];
-    int nB = 0, mB = 0;
-    uint64_t roffB = 0, woffB = 0;
+    const int gl = (threadIdx.x & 31) & (LANES - 1);       // lane within the group
+    int nA = 0, mA = 0, nB = 0, mB = 0;
+    uint64_t roffA = 0, woffA = 0, roffB = 0, woffB = 0;
+    if (hasA) {
+        const uint32_t riA = b.pairs[2 * pA], wiA = b.pairs[2 * pA + 1];
+        nA = (int)b.read_len[riA]; mA = (int)b.win_len[wiA];
+        roffA = b.read_off[riA]; woffA = b.win_off[wiA];
+    }
     if (hasB) {
         const uint32_t riB = b.pairs[2 * pB], wiB = b.pairs[2 * pB + 1];
         nB = (int)b.read_len[riB]; mB = (int)b.win_len[wiB];
         roffB = b.read_off[riB]; woffB = b.win_off[wiB];
     }
     const int e = sc.gap_extend, oe = sc.gap_open + sc.gap_extend, beta = -sc.mismatch;
-    const int mmax = max(mA, mB);
-    const int j0 = lane * KC;                              // this lane owns columns j0 + 1 .. j0 + KC of both pairs
+    const int mmax = max(mA, mB);                          // rows of this group
+    const int mwarp = LANES == 32 ? mmax : __reduce_max_sync(0xffffffffu, mmax);
+    const int j0 = gl * KC;                                // this lane owns columns j0 + 1 .. j0 + KC of both pairs
     uint32_t S[KC], Dt[KC], rh[KC], ck[KC], negek[KC];
 #pragma unroll
     for (int k = 0; k < KC; ++k) {
@@ -216,29 +223,29 @@ __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, con
     const uint32_t BETA2 = pack2(beta), E2 = pack2(e), NEGE2 = pack2(-e), NEG2 = 0x80008000u, NEGEK2 = pack2(-e * KC);
     const uint32_t MISABS2 = (uint32_t)beta * 0x00010001u, Cd = pack2(sc.match - sc.mismatch);
     const uint32_t EDGE_I = pack2(beta - oe);              // I(i,0), in the frame of column 0
-    uint32_t ci = pack2(-e * lane - oe - sc.mismatch);     // e*i - oe - mismatch for the row before this lane's first step
-    uint32_t negei = pack2(e * lane);
+    uint32_t ci = pack2(-e * gl - oe - sc.mismatch);       // e*i - oe - mismatch for the row before this lane's first step
+    uint32_t negei = pack2(e * gl);
     uint32_t best = BETA2;
     int biA = 0, bjA = 0, biB = 0, bjB = 0;
     uint32_t h_out = BETA2, i_out = EDGE_I, sel_out = 0u;
     uint32_t diag = 0u;                                    // S(i-1, j0); row 0 is all zeros
     uint32_t wsel = 0u;
-    const int steps = mmax + 31;
+    const int steps = mwarp + LANES - 1;
     for (int s = 1; s <= steps; ++s) {
-        if (((s - 1) & 31) == 0) {                         // window codes of rows s .. s + 31, one row per lane, as PRMT selectors
-            const int r = s + lane;
+        if (((s - 1) & (LANES - 1)) == 0) {                // window codes of the next LANES rows, one row per lane, as PRMT selectors
+            const int r = s + gl;
             const uint32_t cA = r <= mA ? code_at(b.wins_packed, b.win_nmask, woffA + (uint64_t)(r - 1), SDP_CODE_WIN_N) : SDP_CODE_WIN_N;
             const uint32_t cB = r <= mB ? code_at(b.wins_packed, b.win_nmask, woffB + (uint64_t)(r - 1), SDP_CODE_WIN_N) : SDP_CODE_WIN_N;
             wsel = cA * 0x11u | cB * 0x1100u;
         }
-        const uint32_t sel0 = __shfl_sync(0xffffffffu, wsel, (s - 1) & 31);
-        uint32_t left = __shfl_up_sync(0xffffffffu, h_out, 1);
-        uint32_t ileft = __shfl_up_sync(0xffffffffu, i_out, 1);
-        uint32_t sel = __shfl_up_sync(0xffffffffu, sel_out, 1);
+        const uint32_t sel0 = __shfl_sync(0xffffffffu, wsel, (s - 1) & (LANES - 1), LANES);
+        uint32_t left = __shfl_up_sync(0xffffffffu, h_out, 1, LANES);
+        uint32_t ileft = __shfl_up_sync(0xffffffffu, i_out, 1, LANES);
+        uint32_t sel = __shfl_up_sync(0xffffffffu, sel_out, 1, LANES);
         ci = __viaddmax_s16x2(ci, E2, NEG2);               // packed add (max with the most negative value)
         negei = __viaddmax_s16x2(negei, NEGE2, NEG2);
-        const int i = s - lane;
-        if (lane == 0) { left = BETA2; ileft = EDGE_I; sel = sel0; }      // M(i,0) = 0, I(i,0) = -inf
+        const int i = s - gl;
+        if (gl == 0) { left = BETA2; ileft = EDGE_I; sel = sel0; }        // M(i,0) = 0, I(i,0) = -inf
         else ileft = __viaddmax_s16x2(ileft, NEGEK2, NEG2);               // from the left lane's column frame into this one
         if (i >= 1 && i <= mmax) {
             const uint32_t left_in = left, bprev = best;
@@ -275,37 +282,79 @@ __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, con
         h_out = left; i_out = ileft; sel_out = sel;
     }
     int bA = (int)(int16_t)(best & 0xFFFFu) - beta, bB = (int)(int16_t)(best >> 16) - beta;
-    // over the lanes, per pair: highest score, then lowest row, then lowest column
-    for (int o = 16; o > 0; o >>= 1) {
-        int ob = __shfl_down_sync(0xffffffffu, bA, o), oi = __shfl_down_sync(0xffffffffu, biA, o), oj = __shfl_down_sync(0xffffffffu, bjA, o);
+    // over the lanes of the group, per pair: highest score, then lowest row, then lowest column
+    for (int o = LANES / 2; o > 0; o >>= 1) {
+        int ob = __shfl_down_sync(0xffffffffu, bA, o, LANES), oi = __shfl_down_sync(0xffffffffu, biA, o, LANES),
+            oj = __shfl_down_sync(0xffffffffu, bjA, o, LANES);
         if (ob > bA || (ob == bA && (oi < biA || (oi == biA && oj < bjA)))) { bA = ob; biA = oi; bjA = oj; }
-        ob = __shfl_down_sync(0xffffffffu, bB, o); oi = __shfl_down_sync(0xffffffffu, biB, o); oj = __shfl_down_sync(0xffffffffu, bjB, o);
+        ob = __shfl_down_sync(0xffffffffu, bB, o, LANES); oi = __shfl_down_sync(0xffffffffu, biB, o, LANES);
+        oj = __shfl_down_sync(0xffffffffu, bjB, o, LANES);
         if (ob > bB || (ob == bB && (oi < biB || (oi == biB && oj < bjB)))) { bB = ob; biB = oi; bjB = oj; }
     }
-    if (lane == 0) {
-        score[pA] = bA; ref_end[pA] = biA - 1; end_col[pA] = bjA;          // S == 0: row 0, column 0 -> ref_end -1
+    if (gl == 0) {
+        if (hasA) { score[pA] = bA; ref_end[pA] = biA - 1; end_col[pA] = bjA; }        // S == 0: row 0, column 0 -> ref_end -1
         if (hasB) { score[pB] = bB; ref_end[pB] = biB - 1; end_col[pB] = bjB; }
     }
 }
 
+// Four consecutive pairs q0 .. q0 + 3 share one warp (two groups of 16 lanes) when every one of them that exists goes to
+// the int16x2 kernel and has a read of at most 128 bases. *nmax receives the longest read.
+__device__ __forceinline__ bool local_i16_quad(const sdp_batch& b, const Scoring& sc, uint64_t q0, uint64_t n_pairs,
+                                               const uint32_t* __restrict__ slow_words, int* nmax)
+{
+    int nm = 0;
+    for (int t = 0; t < 4; ++t) {
+        const uint64_t p = q0 + (uint64_t)t;
+        if (p >= n_pairs) break;
+        if (slow_words[p] == 0) return false;
+        const int n = (int)b.read_len[b.pairs[2 * p]];
+        if (n > 128 || !local_i16_taken(b, sc, p, n_pairs, slow_words)) return false;
+        nm = max(nm, n);
+    }
+    *nmax = nm;
+    return true;
+}
+
+#define SDP_LOCAL_I16_DISPATCH(KEXPR, LANES_, ...)                                                      \
+    switch (KEXPR) {                                                                                    \
+    case 1: forward_local_i16x2_warp<1, LANES_>(__VA_ARGS__); break;                                    \
+    case 2: forward_local_i16x2_warp<2, LANES_>(__VA_ARGS__); break;                                    \
+    case 3: forward_local_i16x2_warp<3, LANES_>(__VA_ARGS__); break;                                    \
+    case 4: forward_local_i16x2_warp<4, LANES_>(__VA_ARGS__); break;                                    \
+    case 5: forward_local_i16x2_warp<5, LANES_>(__VA_ARGS__); break;                                    \
+    case 6: forward_local_i16x2_warp<6, LANES_>(__VA_ARGS__); break;                                    \
+    case 7: forward_local_i16x2_warp<7, LANES_>(__VA_ARGS__); break;                                    \
+    default: forward_local_i16x2_warp<8, LANES_>(__VA_ARGS__); break;                                   \
+    }
+
+// QUAD = true: warp w takes pairs 4w .. 4w + 3 if local_i16_quad says so; QUAD = false: warp w takes pairs 2w, 2w + 1
+// unless their quad went to the other kernel. Every decision is warp-uniform.
+template <bool QUAD>
 __global__ void __launch_bounds__(256) k_forward_local_i16(const sdp_batch b, const Scoring sc, uint64_t n_pairs,
                                                            const uint32_t* __restrict__ slow_words,
                                                            int32_t* __restrict__ score, int32_t* __restrict__ ref_end,
                                                            int32_t* __restrict__ end_col)
 {
-    const uint64_t p0 = (((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 2ull;
-    if (p0 >= n_pairs) return;                             // warp-uniform, like everything below
-    const bool inA = slow_words[p0] != 0, inB = p0 + 1 < n_pairs && slow_words[p0 + 1] != 0;
-    const bool runA = inA && local_i16_taken(b, sc, p0, n_pairs, slow_words);
-    const bool runB = inB && local_i16_taken(b, sc, p0 + 1, n_pairs, slow_words);
-    if (!runA && !runB) return;
-    const uint64_t pA = runA ? p0 : p0 + 1;
-    const bool hasB = runA && runB;
-    int nmax = (int)b.read_len[b.pairs[2 * pA]];
-    if (hasB) nmax = max(nmax, (int)b.read_len[b.pairs[2 * (p0 + 1)]]);
-    if (nmax <= 128) forward_local_i16x2_warp<4>(b, sc, pA, p0 + 1, hasB, score, ref_end, end_col);
-    else             forward_local_i16x2_warp<8>(b, sc, pA, p0 + 1, hasB, score, ref_end, end_col);
+    const uint64_t w = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int nmax = 0;
+    if (QUAD) {
+        const uint64_t q0 = 4ull * w;
+        if (q0 >= n_pairs || !local_i16_quad(b, sc, q0, n_pairs, slow_words, &nmax)) return;
+        const uint64_t pA = q0 + 2ull * (uint64_t)((threadIdx.x & 31) >> 4), pB = pA + 1;
+        const bool hasA = pA < n_pairs, hasB = pB < n_pairs;
+        SDP_LOCAL_I16_DISPATCH((nmax + 15) >> 4, 16, b, sc, pA, pB, hasA, hasB, score, ref_end, end_col)
+    } else {
+        const uint64_t p0 = 2ull * w;
+        if (p0 >= n_pairs) return;
+        if (local_i16_quad(b, sc, p0 & ~3ull, n_pairs, slow_words, &nmax)) return;
+        const bool runA = slow_words[p0] != 0 && local_i16_taken(b, sc, p0, n_pairs, slow_words);
+        const bool runB = p0 + 1 < n_pairs && slow_words[p0 + 1] != 0 && local_i16_taken(b, sc, p0 + 1, n_pairs, slow_words);
+        if (!runA && !runB) return;
+        nmax = max(runA ? (int)b.read_len[b.pairs[2 * p0]] : 0, runB ? (int)b.read_len[b.pairs[2 * (p0 + 1)]] : 0);
+        SDP_LOCAL_I16_DISPATCH((nmax + 31) >> 5, 32, b, sc, p0, p0 + 1, runA, runB, score, ref_end, end_col)
+    }
 }
+#undef SDP_LOCAL_I16_DISPATCH
 
 // LARGE = false: reads up to 256 bases (4 or 8 columns per lane); true: up to 1,024 (16 or 32). Two kernels because
 // their register budgets differ by a factor of three.
@@ -335,9 +384,12 @@ void launch_forward_i32(const sdp_batch& b, const Scoring& sc, int local, const 
 {
     if (b.n_pairs) {
         const uint32_t wgrid = (uint32_t)((b.n_pairs * 32 + 255) / 256);
-        if (local)      // two pairs per warp on the int16x2 DPX instructions, where the reads and the values fit
-            k_forward_local_i16<<<(uint32_t)(((b.n_pairs + 1) / 2 * 32 + 255) / 256), 256, 0, st>>>(b, sc, b.n_pairs, slow_words, score,
-                                                                                                  ref_end, end_col);
+        if (local) {    // int16x2 DPX instructions where the reads and the values fit: four or two pairs per warp
+            k_forward_local_i16<true><<<(uint32_t)(((b.n_pairs + 3) / 4 * 32 + 255) / 256), 256, 0, st>>>(b, sc, b.n_pairs, slow_words,
+                                                                                                        score, ref_end, end_col);
+            k_forward_local_i16<false><<<(uint32_t)(((b.n_pairs + 1) / 2 * 32 + 255) / 256), 256, 0, st>>>(b, sc, b.n_pairs, slow_words,
+                                                                                                         score, ref_end, end_col);
+        }
         k_forward_i32_warp<false><<<wgrid, 256, 0, st>>>(b, sc, local, b.n_pairs, slow_words, score, ref_end, end_col);
         k_forward_i32_warp<true><<<wgrid, 256, 0, st>>>(b, sc, local, b.n_pairs, slow_words, score, ref_end, end_col);
         k_forward_i32<<<(uint32_t)((b.n_pairs + 63) / 64), 64, 0, st>>>(b, sc, local, b.n_pairs, slow_words, slow_off, rows, score,

@@ -517,6 +517,12 @@ def test_local_mode_int16_pairing(sc):
     try:
         c.set_mode(local=True)
         parity.check_batch(c, W.batch_from_strings(wins, reads), sc, f"local int16 pairing {sc}", local=True)
+        # four pairs per warp (two 16-lane groups) when a whole quad has reads of at most 128 bases: every tail size
+        short = [k for k in range(len(reads)) if len(reads[k]) <= 128]
+        for count in (1, 2, 3, 4, 5, 6, 7, 41):
+            pick = short[:count]
+            parity.check_batch(c, W.batch_from_strings([wins[k] for k in pick], [reads[k] for k in pick]), sc,
+                               f"local int16 quads, {count} pairs {sc}", host_path=False, local=True)
     finally:
         c.destroy()
 
