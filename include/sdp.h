@@ -239,7 +239,8 @@ const char* sdp_static_last_error(void);
  * CIGAR as soft clips (BAM op 4), n_cols counts aligned columns only, and the filter counts clipped bases as columns
  * that do not match: pass iff n_cols > 0 and n_match * 1e6 >= q * (n_cols + clipped). A pair without any positive-
  * scoring alignment reports score 0, ref_start 0, ref_end -1, read_start 0, read_end -1, CIGAR <n>S, pass 0.
- * Local mode runs on the int32 lane (exact; one warp per pair, about one tenth of the default mode's throughput).
+ * Local mode has its own forward kernels (an int16x2 one for reads up to 256 bases, the int32 lane beyond) and the generic
+ * traceback: exact, about one fifth of the default mode's throughput on 100-base reads.
  * SDP_EINVAL for an unknown mode.
  */
 #define SDP_MODE_SEMIGLOBAL 0

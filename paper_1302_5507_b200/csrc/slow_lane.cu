@@ -154,11 +154,15 @@ __device__ __forceinline__ void forward_i32_warp(const sdp_batch& b, const Scori
 //     best = max(best, H^)
 // q = match - mismatch or 0 comes from the FMA pipe (score_kernel.cuh: HADD2 + HFMA2.RELU on fp16 base codes), and so
 // does S = H^ - beta as one 32-bit integer subtraction (no borrow between the halves: H^ >= beta in both).
-// The position of the best cell is resolved once per row and lane, only when the row raised the lane's best: the row's
-// values are still in S[]. Cells of padded read columns (a shorter partner, columns past n) and padded window rows hold
+// The position of the best cell: when a row raises the lane's best in one half, the lane notes the row number and keeps
+// that half of the row's values (one LOP3 per column); the column is read off the kept row after the last step. Cells of padded read columns (a shorter partner, columns past n) and padded window rows hold
 // N codes, which match nothing: such a cell never exceeds its real ancestors, all of which have a lower row or column,
 // so it can tie but never win under the rule "highest score, then lowest row, then lowest column".
 __device__ __forceinline__ uint32_t pack2(int v) { return ((uint32_t)v & 0xFFFFu) * 0x00010001u; }
+// bitwise (mask ? b : a) in one LOP3
+__device__ __forceinline__ uint32_t lop3_pick(uint32_t a, uint32_t b, uint32_t mask) {
+    uint32_t r; asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(r) : "r"(a), "r"(b), "r"(mask)); return r;
+}
 
 // value rule of the int16x2 local kernel: largest stored magnitude match*n + beta + e*rows, and -(oe + e*rows) below
 __device__ __forceinline__ bool local_i16_rule(const Scoring& sc, int n, int m) {
@@ -208,10 +212,11 @@ __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, con
     const int mmax = max(mA, mB);                          // rows of this group
     const int mwarp = LANES == 32 ? mmax : __reduce_max_sync(0xffffffffu, mmax);
     const int j0 = gl * KC;                                // this lane owns columns j0 + 1 .. j0 + KC of both pairs
-    uint32_t S[KC], Dt[KC], rh[KC], ck[KC], negek[KC];
+    uint32_t S[KC], Dt[KC], rh[KC], ck[KC], negek[KC], snap[KC];
 #pragma unroll
     for (int k = 0; k < KC; ++k) {
         const int j = j0 + k + 1;
+        snap[k] = 0u;
         const uint32_t cA = j <= nA ? code_at(b.reads_packed, b.read_nmask, roffA + (uint64_t)(j - 1), SDP_CODE_READ_N) : SDP_CODE_READ_N;
         const uint32_t cB = j <= nB ? code_at(b.reads_packed, b.read_nmask, roffB + (uint64_t)(j - 1), SDP_CODE_READ_N) : SDP_CODE_READ_N;
         rh[k] = read_code_half(cA) | (read_code_half(cB) << 16);
@@ -223,6 +228,7 @@ __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, con
     const uint32_t BETA2 = pack2(beta), E2 = pack2(e), NEGE2 = pack2(-e), NEG2 = 0x80008000u, NEGEK2 = pack2(-e * KC);
     const uint32_t MISABS2 = (uint32_t)beta * 0x00010001u, Cd = pack2(sc.match - sc.mismatch);
     const uint32_t EDGE_I = pack2(beta - oe);              // I(i,0), in the frame of column 0
+    const uint32_t one = opaque_u32(1u), NEGMIS2 = 0u - MISABS2;           // (a multiplier the compiler cannot fold: the add stays an IMAD)
     uint32_t ci = pack2(-e * gl - oe - sc.mismatch);       // e*i - oe - mismatch for the row before this lane's first step
     uint32_t negei = pack2(e * gl);
     uint32_t best = BETA2;
@@ -260,28 +266,31 @@ __device__ __forceinline__ void forward_local_i16x2_warp(const sdp_batch& b, con
                 const uint32_t bb = __viaddmax_s16x2(it, negek[k], a);
                 const uint32_t h = __viaddmax_s16x2(diag, q, bb);
                 diag = up;
-                S[k] = h - MISABS2;
+                S[k] = imad_sel(h, one, NEGMIS2);          // h - beta per half, on the FMA pipe
                 Dt[k] = dt; left = h; ileft = it;
                 best = __vmaxs2(best, h);
             }
-            if (best != bprev) {                           // this row raised the lane's best in one half or both
-                const uint32_t target = best - MISABS2;
-                if ((best ^ bprev) & 0xFFFFu) {
-                    biA = i;
+            if (best != bprev) {                           // this row raised the lane's best in one half or both:
+                const uint32_t d = best ^ bprev;           // keep the row's values of that half; the column is read off at the end
+                const uint32_t mask = ((d & 0xFFFFu) ? 0x0000FFFFu : 0u) | ((d >> 16) ? 0xFFFF0000u : 0u);
+                if (mask & 0x0000FFFFu) biA = i;
+                if (mask & 0xFFFF0000u) biB = i;
 #pragma unroll
-                    for (int k = KC - 1; k >= 0; --k) if (((S[k] ^ target) & 0xFFFFu) == 0u) bjA = j0 + k + 1;
-                }
-                if ((best ^ bprev) >> 16) {
-                    biB = i;
-#pragma unroll
-                    for (int k = KC - 1; k >= 0; --k) if (((S[k] ^ target) >> 16) == 0u) bjB = j0 + k + 1;
-                }
+                for (int k = 0; k < KC; ++k) snap[k] = lop3_pick(snap[k], S[k], mask);
             }
             diag = left_in - MISABS2;                      // S(i, j0): the next row's diagonal neighbour
         }
         h_out = left; i_out = ileft; sel_out = sel;
     }
     int bA = (int)(int16_t)(best & 0xFFFFu) - beta, bB = (int)(int16_t)(best >> 16) - beta;
+    {   // lowest column of the lane's best cell: the first entry of the kept row that equals the best (bi == 0: none)
+        const uint32_t target = best - MISABS2;
+#pragma unroll
+        for (int k = KC - 1; k >= 0; --k) {
+            if (biA && ((snap[k] ^ target) & 0xFFFFu) == 0u) bjA = j0 + k + 1;
+            if (biB && ((snap[k] ^ target) >> 16) == 0u) bjB = j0 + k + 1;
+        }
+    }
     // over the lanes of the group, per pair: highest score, then lowest row, then lowest column
     for (int o = LANES / 2; o > 0; o >>= 1) {
         int ob = __shfl_down_sync(0xffffffffu, bA, o, LANES), oi = __shfl_down_sync(0xffffffffu, biA, o, LANES),
